@@ -1,0 +1,183 @@
+"""CPU oracle for the AVU-GSR LSQR hot path -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+Thin ctypes loader around ``oracle/gsr_oracle.c`` (plain C, FP64, single thread,
+``gcc -O2 -ffp-contract=off``).  Only ``tests/``, ``__graft_entry__.smoke()`` and the
+``cpu_baseline`` / ``--impl reference`` legs of ``bench.py`` may import this package.
+It imports nothing from ``paper_2308_00778_b200`` and that package never imports it.
+
+The arithmetic lives entirely in the C file; this module only marshals numpy arrays.
+See the header of ``gsr_oracle.c`` for the citations (PAPER.md lines) and for what pins
+each function.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "gsr_oracle.c")
+_LIB = os.path.join(_HERE, "libgsr_oracle.so")
+
+N_PAR = 24
+
+
+def build(force: bool = False) -> str:
+    """Compile the oracle (gcc, no FMA contraction).  Returns the path of the library."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + f".tmp{os.getpid()}"
+        subprocess.check_call(
+            ["gcc", "-O2", "-ffp-contract=off", "-fno-fast-math", "-std=c11", "-shared", "-fPIC",
+             "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+class _Sys(C.Structure):
+    _fields_ = [
+        ("n_obs", C.c_int64), ("n_stars", C.c_int64), ("n_dof_att", C.c_int64),
+        ("n_instr", C.c_int64), ("n_con", C.c_int64),
+        ("V", C.c_void_p), ("ia", C.c_void_p), ("iatt", C.c_void_p), ("ic", C.c_void_p),
+        ("con_rowptr", C.c_void_p), ("con_col", C.c_void_p), ("con_val", C.c_void_p),
+    ]
+
+
+class _Res(C.Structure):
+    _fields_ = [("istop", C.c_int32), ("itn", C.c_int64), ("anorm", C.c_double),
+                ("acond", C.c_double), ("rnorm", C.c_double), ("arnorm", C.c_double),
+                ("xnorm", C.c_double)]
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        lib = C.CDLL(build())
+        P = C.c_void_p
+        lib.gsr_oracle_ncols.restype = C.c_int64
+        lib.gsr_oracle_ncols.argtypes = [P]
+        lib.gsr_oracle_col.restype = C.c_int64
+        lib.gsr_oracle_col.argtypes = [P, C.c_int64, C.c_int]
+        lib.gsr_oracle_aprod1.restype = None
+        lib.gsr_oracle_aprod1.argtypes = [P, P, P, P]
+        lib.gsr_oracle_aprod2.restype = None
+        lib.gsr_oracle_aprod2.argtypes = [P, P, P, P]
+        lib.gsr_oracle_norm.restype = C.c_double
+        lib.gsr_oracle_norm.argtypes = [P, C.c_int64]
+        lib.gsr_oracle_precondition.restype = None
+        lib.gsr_oracle_precondition.argtypes = [P, P]
+        lib.gsr_oracle_lsqr.restype = C.c_int
+        lib.gsr_oracle_lsqr.argtypes = [P, P, C.c_int64, C.c_double, C.c_double, C.c_double,
+                                        P, P, P, P, P]
+        _lib = lib
+    return _lib
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data
+
+
+@dataclass
+class LsqrResult:
+    x: np.ndarray
+    se: np.ndarray
+    istop: int
+    itn: int
+    anorm: float
+    acond: float
+    rnorm: float
+    arnorm: float
+    xnorm: float
+    trace: np.ndarray | None = None  # [itn, 5]: rnorm, arnorm, anorm, acond, xnorm
+
+
+class OracleSystem:
+    """Holds (private copies of) the upload-format arrays of one system.
+
+    values [m,24] f64 row-major; matrixIndexAstro [m] i64 (= 5*star, non-decreasing);
+    matrixIndexAtt [m] i64 (axis-0 start); instrCol [m,6] i32; optional constraint rows
+    as CSR with absolute columns.
+    """
+
+    def __init__(self, n_stars, n_dof_att, n_instr, values, matrixIndexAstro, matrixIndexAtt,
+                 instrCol, con_rowptr=None, con_col=None, con_val=None):
+        self.lib = _load()
+        self.V = np.array(values, dtype=np.float64, order="C", copy=True).reshape(-1, N_PAR)
+        self.m = self.V.shape[0]
+        self.ia = np.array(matrixIndexAstro, dtype=np.int64, copy=True).reshape(-1)
+        self.iatt = np.array(matrixIndexAtt, dtype=np.int64, copy=True).reshape(-1)
+        self.ic = np.array(instrCol, dtype=np.int32, order="C", copy=True).reshape(-1, 6)
+        assert self.ia.shape[0] == self.m and self.iatt.shape[0] == self.m and self.ic.shape[0] == self.m
+        self.n_stars, self.n_dof_att, self.n_instr = int(n_stars), int(n_dof_att), int(n_instr)
+        if con_rowptr is not None:
+            self.con_rowptr = np.array(con_rowptr, dtype=np.int64, copy=True)
+            self.con_col = np.array(con_col, dtype=np.int64, copy=True)
+            self.con_val = np.array(con_val, dtype=np.float64, copy=True)
+            self.n_con = self.con_rowptr.shape[0] - 1
+        else:
+            self.con_rowptr = np.zeros(1, dtype=np.int64)
+            self.con_col = np.zeros(0, dtype=np.int64)
+            self.con_val = np.zeros(0, dtype=np.float64)
+            self.n_con = 0
+        self.p = None
+        self._s = _Sys(self.m, self.n_stars, self.n_dof_att, self.n_instr, self.n_con,
+                       _ptr(self.V), _ptr(self.ia), _ptr(self.iatt), _ptr(self.ic),
+                       _ptr(self.con_rowptr), _ptr(self.con_col), _ptr(self.con_val))
+        self._sp = C.addressof(self._s)
+        self.n = int(self.lib.gsr_oracle_ncols(self._sp))
+        self.m_tot = self.m + self.n_con
+
+    def col(self, i: int, k: int) -> int:
+        return int(self.lib.gsr_oracle_col(self._sp, i, k))
+
+    def aprod1(self, x, y, want_abs=False):
+        """y += A x (in place on a float64 copy of y); returns y or (y, abs bound)."""
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        y = np.array(y, dtype=np.float64, copy=True)
+        assert x.shape == (self.n,) and y.shape == (self.m_tot,)
+        ab = np.zeros(self.m_tot) if want_abs else None
+        self.lib.gsr_oracle_aprod1(self._sp, _ptr(x), _ptr(y), _ptr(ab))
+        return (y, ab) if want_abs else y
+
+    def aprod2(self, y, x, want_abs=False):
+        """x += A^T y; returns x or (x, abs bound)."""
+        y = np.ascontiguousarray(y, dtype=np.float64)
+        x = np.array(x, dtype=np.float64, copy=True)
+        assert x.shape == (self.n,) and y.shape == (self.m_tot,)
+        ab = np.zeros(self.n) if want_abs else None
+        self.lib.gsr_oracle_aprod2(self._sp, _ptr(y), _ptr(x), _ptr(ab))
+        return (x, ab) if want_abs else x
+
+    def precondition(self):
+        """Compute p, scale the stored A in place; returns p."""
+        assert self.p is None, "already preconditioned"
+        self.p = np.zeros(self.n)
+        self.lib.gsr_oracle_precondition(self._sp, _ptr(self.p))
+        return self.p
+
+    def lsqr(self, b, itnlim, atol, btol, conlim=0.0, want_trace=False) -> LsqrResult:
+        """LSQR on the system as stored; if preconditioned, returns x = p*z, se = p*se_z."""
+        b = np.ascontiguousarray(b, dtype=np.float64)
+        assert b.shape == (self.m_tot,)
+        x = np.zeros(self.n)
+        se = np.zeros(self.n)
+        res = _Res()
+        trace = np.zeros((max(int(itnlim), 1), 5)) if want_trace else None
+        rc = self.lib.gsr_oracle_lsqr(self._sp, _ptr(b), int(itnlim), float(atol), float(btol),
+                                      float(conlim), _ptr(self.p), _ptr(x), _ptr(se),
+                                      C.addressof(res), _ptr(trace))
+        if rc != 0:
+            raise MemoryError("oracle lsqr allocation failed")
+        return LsqrResult(x, se, int(res.istop), int(res.itn), res.anorm, res.acond, res.rnorm,
+                          res.arnorm, res.xnorm, None if trace is None else trace[: res.itn])
+
+
+def norm(a) -> float:
+    """Eq. 4 of the paper (max-scaled Euclidean norm)."""
+    a = np.ascontiguousarray(a, dtype=np.float64).reshape(-1)
+    return float(_load().gsr_oracle_norm(_ptr(a), a.shape[0]))

@@ -1,0 +1,361 @@
+/*
+ * gsr_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, single-threaded FP64 CPU restatement of the hot path of the Gaia
+ * AVU-GSR solver (arXiv 2308.00778, /root/reference/PAPER.md): the two sparse
+ * products aprod1 / aprod2, the column preconditioning, the Eq. 4 norm and the
+ * LSQR iteration of Paige & Saunders that the paper runs.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / reference
+ * legs may build, load or call this file.  It shares no code, header, table or
+ * helper with paper_2308_00778_b200/ (the CUDA path) and neither includes the
+ * other.  Build: gcc -O2 -ffp-contract=off -shared -fPIC (no FMA contraction,
+ * no reordering: every sum below is evaluated in the order it is written).
+ *
+ * What pins each function (tests/test_oracle_pins.py, tests/golden/):
+ *   col mapping, aprod1, aprod2 : dense expansion + numpy matmul, structure
+ *                                 invariants of PAPER.md:78-80, adjoint identity,
+ *                                 a hand-worked fixture (tests/golden/hand_system.txt)
+ *   norm (Eq. 4)                : equals the Euclidean norm; overflow-safe case
+ *   precondition                : unit column norms, ||A'||_F^2 = #non-zero columns
+ *   lsqr                        : dense least squares (numpy lstsq), planted
+ *                                 solution, scipy.sparse.linalg.lsqr (same algorithm),
+ *                                 true residual / A^T r norms per iteration, istop cases
+ *   x_k, se (standard errors)   : closed form V_k (B_k^T B_k)^-1 V_k^T from a dense,
+ *                                 re-orthogonalised Golub-Kahan bidiagonalisation
+ *                                 (k <= 20), upper bound diag((A'^T A')^-1), scipy var
+ *
+ * Matrix definition (PAPER.md:78-80 and the index expressions
+ * of Algorithm 2).  Row i of A holds
+ * 24 stored coefficients V[i*24 + k], k = 0..23, in the section order
+ *   [ 5 astrometric | 12 attitude = 3 axes x 4 | 6 instrumental | 1 global ]
+ * and coefficient k sits in column
+ *   k <  5 : ia[i] + k                                   (ia[i] = 5*star(i))
+ *   k < 17 : 5*nStars + a*nDofAtt + iatt[i] + j          a=(k-5)/4, j=(k-5)%4
+ *   k < 23 : 5*nStars + 3*nDofAtt + ic[i*6 + (k-17)]
+ *   k = 23 : 5*nStars + 3*nDofAtt + nInstr
+ * Constraint rows are generic sparse rows appended below
+ * the observation rows, given as CSR (rowptr, col, val) with absolute columns.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define N_ASTRO 5
+#define N_AXES 3
+#define N_PAR_AXIS 4
+#define N_ATT (N_AXES * N_PAR_AXIS)
+#define N_INSTR 6
+#define N_GLOB 1
+#define N_PAR (N_ASTRO + N_ATT + N_INSTR + N_GLOB) /* 24 */
+
+typedef struct {
+    int64_t n_obs;      /* observation rows m                                  */
+    int64_t n_stars;    /* N_Stars                                             */
+    int64_t n_dof_att;  /* N_DFA, per axis                                     */
+    int64_t n_instr;    /* number of instrumental columns                      */
+    int64_t n_con;      /* constraint rows                                     */
+    double *V;          /* [n_obs*24] row-major A_d              */
+    const int64_t *ia;  /* [n_obs]   M_i astro part: 5*star, non-decreasing    */
+    const int64_t *iatt;/* [n_obs]   M_i attitude part: start s_i, axis 0      */
+    const int32_t *ic;  /* [n_obs*6] I_c instrumental columns                  */
+    const int64_t *con_rowptr; /* [n_con+1]                                    */
+    const int64_t *con_col;    /* [nnz] absolute columns                       */
+    double *con_val;           /* [nnz]                                        */
+} gsr_oracle_system;
+
+int64_t gsr_oracle_ncols(const gsr_oracle_system *S)
+{
+    return N_ASTRO * S->n_stars + N_AXES * S->n_dof_att + S->n_instr + N_GLOB;
+}
+
+/* Column of stored coefficient k of observation row i (see header). */
+int64_t gsr_oracle_col(const gsr_oracle_system *S, int64_t i, int k)
+{
+    const int64_t off_att = N_ASTRO * S->n_stars;
+    const int64_t off_instr = off_att + N_AXES * S->n_dof_att;
+    const int64_t off_glob = off_instr + S->n_instr;
+    if (k < N_ASTRO)
+        return S->ia[i] + k;
+    if (k < N_ASTRO + N_ATT) {
+        int a = (k - N_ASTRO) / N_PAR_AXIS, j = (k - N_ASTRO) % N_PAR_AXIS;
+        return off_att + (int64_t)a * S->n_dof_att + S->iatt[i] + j;
+    }
+    if (k < N_ASTRO + N_ATT + N_INSTR)
+        return off_instr + S->ic[i * N_INSTR + (k - N_ASTRO - N_ATT)];
+    return off_glob;
+}
+
+/*
+ * aprod mode 1, Eq. 2 "b += A x"; Algorithm 2 left column
+ * (PAPER.md:270-312): per row, sum the 24 products in k order, then
+ * b[i] = b[i] + sum.  Constraint rows follow ("Constraints
+ * computation", Alg. 2 o.29).  y has n_obs + n_con entries.  If abs_y != NULL it
+ * receives |y_in[i]| + sum_k |V x| (the bound used by the 1e-12 tolerance).
+ */
+void gsr_oracle_aprod1(const gsr_oracle_system *S, const double *x, double *y, double *abs_y)
+{
+    for (int64_t i = 0; i < S->n_obs; ++i) {
+        double sum = 0.0, asum = 0.0;
+        for (int k = 0; k < N_PAR; ++k) {
+            double t = S->V[i * N_PAR + k] * x[gsr_oracle_col(S, i, k)];
+            sum = sum + t;
+            asum = asum + fabs(t);
+        }
+        if (abs_y)
+            abs_y[i] = fabs(y[i]) + asum;
+        y[i] = y[i] + sum;
+    }
+    for (int64_t r = 0; r < S->n_con; ++r) {
+        double sum = 0.0, asum = 0.0;
+        for (int64_t q = S->con_rowptr[r]; q < S->con_rowptr[r + 1]; ++q) {
+            double t = S->con_val[q] * x[S->con_col[q]];
+            sum = sum + t;
+            asum = asum + fabs(t);
+        }
+        if (abs_y)
+            abs_y[S->n_obs + r] = fabs(y[S->n_obs + r]) + asum;
+        y[S->n_obs + r] = y[S->n_obs + r] + sum;
+    }
+}
+
+/*
+ * aprod mode 2, Eq. 3 "x += A^T b"; Algorithm 3 left column
+ * (PAPER.md:485-576): rows in order, the 24 coefficients of a row in k order,
+ * x[col] += V * y[i].  abs_x (optional) accumulates |x_in| + sum |V y|.
+ */
+void gsr_oracle_aprod2(const gsr_oracle_system *S, const double *y, double *x, double *abs_x)
+{
+    const int64_t n = gsr_oracle_ncols(S);
+    if (abs_x)
+        for (int64_t j = 0; j < n; ++j)
+            abs_x[j] = fabs(x[j]);
+    for (int64_t i = 0; i < S->n_obs; ++i) {
+        for (int k = 0; k < N_PAR; ++k) {
+            int64_t c = gsr_oracle_col(S, i, k);
+            double t = S->V[i * N_PAR + k] * y[i];
+            x[c] = x[c] + t;
+            if (abs_x)
+                abs_x[c] = abs_x[c] + fabs(t);
+        }
+    }
+    for (int64_t r = 0; r < S->n_con; ++r) {
+        for (int64_t q = S->con_rowptr[r]; q < S->con_rowptr[r + 1]; ++q) {
+            int64_t c = S->con_col[q];
+            double t = S->con_val[q] * y[S->n_obs + r];
+            x[c] = x[c] + t;
+            if (abs_x)
+                abs_x[c] = abs_x[c] + fabs(t);
+        }
+    }
+}
+
+/*
+ * Eq. 4: |a| = max(a) * sqrt( sum_i a_i^2 / max(a)^2 ), with
+ * max(a) = max_i |a_i|.  Returns 0 for the zero vector.
+ */
+double gsr_oracle_norm(const double *a, int64_t n)
+{
+    double mx = 0.0;
+    for (int64_t i = 0; i < n; ++i)
+        if (fabs(a[i]) > mx)
+            mx = fabs(a[i]);
+    if (mx == 0.0)
+        return 0.0;
+    double s = 0.0;
+    for (int64_t i = 0; i < n; ++i) {
+        double q = a[i] / mx;
+        s = s + q * q;
+    }
+    return mx * sqrt(s);
+}
+
+/*
+ * Column preconditioning (Alg. 1 l.2-3): "we
+ * normalized the parameters of each column by the norm of the column itself",
+ * the factors stored in p and the solution "re-multiplied by p" afterwards.
+ * Reading (R1-R4): nrm_j = sqrt(sum_i A_ij^2) over all rows including
+ * constraints, p_j = 1/nrm_j (1 if the column is empty), A_ij <- fl(A_ij * p_j)
+ * in place.
+ */
+void gsr_oracle_precondition(gsr_oracle_system *S, double *p)
+{
+    const int64_t n = gsr_oracle_ncols(S);
+    for (int64_t j = 0; j < n; ++j)
+        p[j] = 0.0;
+    for (int64_t i = 0; i < S->n_obs; ++i)
+        for (int k = 0; k < N_PAR; ++k) {
+            double v = S->V[i * N_PAR + k];
+            p[gsr_oracle_col(S, i, k)] += v * v;
+        }
+    for (int64_t r = 0; r < S->n_con; ++r)
+        for (int64_t q = S->con_rowptr[r]; q < S->con_rowptr[r + 1]; ++q)
+            p[S->con_col[q]] += S->con_val[q] * S->con_val[q];
+    for (int64_t j = 0; j < n; ++j)
+        p[j] = (p[j] > 0.0) ? 1.0 / sqrt(p[j]) : 1.0;
+    for (int64_t i = 0; i < S->n_obs; ++i)
+        for (int k = 0; k < N_PAR; ++k)
+            S->V[i * N_PAR + k] = S->V[i * N_PAR + k] * p[gsr_oracle_col(S, i, k)];
+    for (int64_t r = 0; r < S->n_con; ++r)
+        for (int64_t q = S->con_rowptr[r]; q < S->con_rowptr[r + 1]; ++q)
+            S->con_val[q] = S->con_val[q] * p[S->con_col[q]];
+}
+
+typedef struct {
+    int32_t istop;
+    int64_t itn;
+    double anorm, acond, rnorm, arnorm, xnorm;
+} gsr_oracle_result;
+
+/*
+ * LSQR (Paige & Saunders 1982, cited PAPER.md:34, 742-743; the loop is
+ * Alg. 1 l.17-26), damp = 0, on the system as it stands in S
+ * (already preconditioned or not).  Steps and notation follow SURVEY.md 8(c).3.
+ * b has n_obs+n_con entries and is not modified.  z (n) receives the solution of
+ * the system in S, var (n) the accumulated sum_k (w_k/rho_k)^2.  If p != NULL,
+ * x = p (.) z and se = p (.) se_z (Alg. 1 l.27) are written to
+ * x / se instead of z / se_z.  trace, if not NULL, receives 5 doubles per
+ * iteration: rnorm, arnorm, anorm, acond, xnorm.
+ */
+int gsr_oracle_lsqr(const gsr_oracle_system *S, const double *b, int64_t itnlim, double atol,
+                    double btol, double conlim, const double *p, double *x, double *se,
+                    gsr_oracle_result *R, double *trace)
+{
+    const int64_t n = gsr_oracle_ncols(S);
+    const int64_t m = S->n_obs + S->n_con;
+    double *u = (double *)malloc(sizeof(double) * (size_t)(m > 0 ? m : 1));
+    double *v = (double *)calloc((size_t)n, sizeof(double));
+    double *w = (double *)calloc((size_t)n, sizeof(double));
+    if (!u || !v || !w) {
+        free(u); free(v); free(w);
+        return -1;
+    }
+    int32_t istop = 0;
+    int64_t itn = 0;
+    double anorm = 0.0, acond = 0.0, ddnorm = 0.0, xxnorm = 0.0, xnorm = 0.0, z = 0.0;
+    double cs2 = -1.0, sn2 = 0.0, arnorm = 0.0;
+    const double ctol = (conlim > 0.0) ? 1.0 / conlim : 0.0;
+
+    /* step 1: x = 0, var = 0, u = b, beta = |u|, u /= beta, v = A^T u, alpha = |v|, v /= alpha, w = v */
+    for (int64_t j = 0; j < n; ++j) {
+        x[j] = 0.0;
+        se[j] = 0.0; /* holds var until the finish step */
+    }
+    memcpy(u, b, sizeof(double) * (size_t)m);
+    double alpha = 0.0;
+    double beta = gsr_oracle_norm(u, m);
+    if (beta > 0.0) {
+        for (int64_t i = 0; i < m; ++i)
+            u[i] = u[i] / beta;
+        gsr_oracle_aprod2(S, u, v, NULL); /* "initial solution" via aprod 2 */
+        alpha = gsr_oracle_norm(v, n);
+    }
+    if (alpha > 0.0) {
+        for (int64_t j = 0; j < n; ++j)
+            v[j] = v[j] / alpha;
+        memcpy(w, v, sizeof(double) * (size_t)n);
+    }
+    double rhobar = alpha, phibar = beta;
+    const double bnorm = beta;
+    double rnorm = beta;
+    arnorm = alpha * beta;
+
+    if (arnorm != 0.0) {
+        while (itn < itnlim) {
+            /* step 2: bidiagonalisation */
+            itn = itn + 1;
+            for (int64_t i = 0; i < m; ++i)
+                u[i] = -alpha * u[i];
+            gsr_oracle_aprod1(S, v, u, NULL);
+            beta = gsr_oracle_norm(u, m);
+            if (beta > 0.0) {
+                for (int64_t i = 0; i < m; ++i)
+                    u[i] = u[i] / beta;
+                anorm = sqrt(anorm * anorm + alpha * alpha + beta * beta);
+                for (int64_t j = 0; j < n; ++j)
+                    v[j] = -beta * v[j];
+                gsr_oracle_aprod2(S, u, v, NULL);
+                alpha = gsr_oracle_norm(v, n);
+                if (alpha > 0.0)
+                    for (int64_t j = 0; j < n; ++j)
+                        v[j] = v[j] / alpha;
+            }
+            /* step 3: plane rotation */
+            const double rho = sqrt(rhobar * rhobar + beta * beta);
+            const double cs = rhobar / rho;
+            const double sn = beta / rho;
+            const double theta = sn * alpha;
+            rhobar = -cs * alpha;
+            const double phi = cs * phibar;
+            phibar = sn * phibar;
+            const double tau = sn * phi;
+            /* step 4: update x, w, var */
+            const double t1 = phi / rho;
+            const double t2 = -theta / rho;
+            for (int64_t j = 0; j < n; ++j) {
+                const double dk = w[j] / rho;
+                x[j] = x[j] + t1 * w[j];
+                w[j] = v[j] + t2 * w[j];
+                se[j] = se[j] + dk * dk;
+                ddnorm = ddnorm + dk * dk;
+            }
+            /* step 5: norm of x */
+            const double delta = sn2 * rho;
+            const double gambar = -cs2 * rho;
+            const double rhs = phi - delta * z;
+            const double zbar = rhs / gambar;
+            xnorm = sqrt(xxnorm + zbar * zbar);
+            const double gamma = sqrt(gambar * gambar + theta * theta);
+            cs2 = gambar / gamma;
+            sn2 = theta / gamma;
+            z = rhs / gamma;
+            xxnorm = xxnorm + z * z;
+            /* step 6: estimates */
+            acond = anorm * sqrt(ddnorm);
+            rnorm = phibar;
+            arnorm = alpha * fabs(tau);
+            if (trace) {
+                double *t = trace + 5 * (itn - 1);
+                t[0] = rnorm; t[1] = arnorm; t[2] = anorm; t[3] = acond; t[4] = xnorm;
+            }
+            /* step 7: stopping tests, later assignments override earlier ones */
+            const double test1 = rnorm / bnorm;
+            const double test2 = (anorm * rnorm != 0.0) ? arnorm / (anorm * rnorm) : 0.0;
+            const double test3 = 1.0 / acond;
+            const double t1p = test1 / (1.0 + anorm * xnorm / bnorm);
+            const double rtol = btol + atol * anorm * xnorm / bnorm;
+            if (itn >= itnlim) istop = 7;
+            if (1.0 + test3 <= 1.0) istop = 6;
+            if (1.0 + test2 <= 1.0) istop = 5;
+            if (1.0 + t1p <= 1.0) istop = 4;
+            if (test3 <= ctol) istop = 3;
+            if (test2 <= atol) istop = 2;
+            if (test1 <= rtol) istop = 1;
+            if (istop != 0)
+                break;
+        }
+    }
+    /* step 8: standard errors, then un-scaling by p */
+    {
+        double s = rnorm;
+        if (m > n)
+            s = rnorm / sqrt((double)(m - n));
+        for (int64_t j = 0; j < n; ++j)
+            se[j] = sqrt(se[j]) * s;
+    }
+    if (p)
+        for (int64_t j = 0; j < n; ++j) {
+            x[j] = p[j] * x[j];
+            se[j] = p[j] * se[j];
+        }
+    R->istop = istop;
+    R->itn = itn;
+    R->anorm = anorm;
+    R->acond = acond;
+    R->rnorm = rnorm;
+    R->arnorm = arnorm;
+    R->xnorm = xnorm;
+    free(u); free(v); free(w);
+    return 0;
+}
