@@ -1,0 +1,178 @@
+/*
+ * gsr.h -- C ABI of libgsr.so: the LSQR hot path of the Gaia AVU-GSR solver
+ * (arXiv 2308.00778; citations are lines of /root/reference/PAPER.md) on one
+ * NVIDIA B200 (sm_100a), FP64.
+ *
+ * The system  A x = b  (Eq. 1-3).  A has n_obs observation rows
+ * and, below them, n_con constraint rows.  Every observation
+ * row stores N_par = 24 coefficients in the section order
+ *     [ 5 astrometric | 12 attitude = 3 axes x 4 | 6 instrumental | 1 global ]
+ * and the unknowns are ordered
+ *     [ astro: 5*n_stars | att axis0: n_dof_att | axis1 | axis2 | instr: n_instr | gamma ]
+ * so n = 5*n_stars + 3*n_dof_att + n_instr + 1.  Coefficient k of row i is in column
+ *     k <  5 : matrixIndexAstro[i] + k
+ *     k < 17 : 5*n_stars + a*n_dof_att + matrixIndexAtt[i] + j,  a=(k-5)/4, j=(k-5)%4
+ *     k < 23 : 5*n_stars + 3*n_dof_att + instrCol[6*i + (k-17)]
+ *     k = 23 : 5*n_stars + 3*n_dof_att + n_instr
+ * (index expressions of Algorithm 2).
+ *
+ * Conventions
+ *  - every call returns a gsr_status (0 = OK, negative = error); nothing throws;
+ *    gsr_last_error(h) gives a handle-owned, NUL-terminated description.
+ *  - "host or device" pointers are classified with cudaPointerGetAttributes;
+ *    "device" pointers must be device memory of the handle's device.
+ *  - the caller keeps ownership of every array it passes; the library copies.
+ *  - a handle is not thread-safe; all work is ordered on the handle's stream and
+ *    every call synchronises that stream before it returns.
+ *  - there is no CPU fallback: without a CUDA device gsr_create fails (GSR_ECUDA).
+ */
+#ifndef GSR_H
+#define GSR_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GSR_N_ASTRO 5
+#define GSR_N_ATT 12
+#define GSR_N_INSTR 6
+#define GSR_N_GLOB 1
+#define GSR_N_PAR 24
+
+typedef enum {
+    GSR_OK = 0,
+    GSR_EINVAL = -1, /* bad argument (NULL, negative size, unsupported section width) */
+    GSR_EINDEX = -2, /* an index array violates its contract; see gsr_bad_row()        */
+    GSR_ENOMEM = -3, /* device or host allocation failed                               */
+    GSR_ECUDA = -4,  /* CUDA runtime error (text in gsr_last_error)                    */
+    GSR_ESTATE = -5  /* call order: e.g. aprod before upload, precondition twice       */
+} gsr_status;
+
+/* Sizes of one system.  Section widths are fixed at 5/12/6/1
+ * (BASELINE north_star); the fields exist so that a mismatch is an error rather
+ * than a silent misread. */
+typedef struct {
+    int64_t n_obs;      /* observation rows m (>= 0)                                   */
+    int64_t n_stars;    /* N_Stars                                                     */
+    int64_t n_dof_att;  /* N_DFA, attitude degrees of freedom per axis (>= 4)          */
+    int64_t n_instr;    /* number of instrumental columns (>= 6)                       */
+    int64_t n_con;      /* constraint rows appended below the observations (>= 0)      */
+    int64_t n_con_nnz;  /* non-zeros of the constraint rows                            */
+    int32_t n_astro_par, n_att_par, n_instr_par, n_glob_par; /* must be 5, 12, 6, 1    */
+    int32_t device;     /* CUDA device ordinal                                         */
+    void *stream;       /* cudaStream_t to run on (e.g. torch's current stream); NULL = the
+                           library creates its own non-blocking stream                */
+} gsr_layout;
+
+typedef struct gsr_handle gsr_handle;
+
+/* Outputs of gsr_lsqr.  x and se: caller-allocated, n doubles each, host or
+ * device; se may be NULL. */
+typedef struct {
+    double *x;      /* solution of the original system (x = p (.) z, Alg. 1 l.27)      */
+    double *se;     /* standard errors ("variances"; Alg. 1 l.26-27)      */
+    int32_t istop;  /* Paige-Saunders stop code 0..7                                   */
+    int64_t itn;    /* iterations done                                                 */
+    double anorm, acond, rnorm, arnorm, xnorm; /* LSQR estimates (of the scaled system) */
+} gsr_result;
+
+/* Allocates the handle and all device storage for a system of these sizes.
+ * PAPER.md:94-104 (Alg. 1 l.4-12: device selection, cudaMalloc). */
+int32_t gsr_create(const gsr_layout *layout, gsr_handle **out);
+
+/* Frees everything.  NULL is allowed. */
+int32_t gsr_destroy(gsr_handle *h);
+
+const char *gsr_last_error(const gsr_handle *h);
+
+/* After GSR_EINDEX: first offending observation row (or -1). */
+int64_t gsr_bad_row(const gsr_handle *h);
+
+/* n = 5*n_stars + 3*n_dof_att + n_instr + 1 and m_tot = n_obs + n_con. */
+int64_t gsr_ncols(const gsr_handle *h);
+int64_t gsr_nrows(const gsr_handle *h);
+
+/* Copies the system to the device (A_d, M_i, I_c; Alg. 1 l.6-12).
+ *   values           f64 [n_obs*24] row-major, section order as above
+ *   matrixIndexAstro i64 [n_obs]   = 5*star(i), non-decreasing, in [0, 5*(n_stars-1)]
+ *   matrixIndexAtt   i64 [n_obs]   = s_i in [0, n_dof_att-4] (axis-0 relative)
+ *   instrCol         i32 [n_obs*6] in [0, n_instr)
+ *   b                f64 [n_obs+n_con] known terms
+ * All host or device.  Validates the index contracts on the device (GSR_EINDEX,
+ * gsr_bad_row) and derives the star row pointer.  Replaces any earlier upload and
+ * clears the preconditioned state. */
+int32_t gsr_upload(gsr_handle *h, const double *values, const int64_t *matrixIndexAstro,
+                   const int64_t *matrixIndexAtt, const int32_t *instrCol, const double *b);
+
+/* Chunked form of gsr_upload for systems generated piecewise on the device (the
+ * 116 GB "Large" config cannot exist twice in HBM): copies rows [row0, row0+nrows)
+ * of the four arrays and of b.  Call gsr_upload_finish() once every row is in; it
+ * validates and derives layouts exactly as gsr_upload does.  b_tail (n_con entries,
+ * may be NULL when n_con == 0) holds the known terms of the constraint rows. */
+int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double *values,
+                        const int64_t *matrixIndexAstro, const int64_t *matrixIndexAtt,
+                        const int32_t *instrCol, const double *b);
+int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail);
+
+/* Constraint rows as CSR with absolute column indices:
+ * rowptr i64 [n_con+1], col i64 [n_con_nnz] in [0, n), val f64 [n_con_nnz].
+ * Host or device.  Must precede gsr_precondition. */
+int32_t gsr_upload_constraints(gsr_handle *h, const int64_t *rowptr, const int64_t *col,
+                               const double *val);
+
+/* Derived layout, for bit-exact checks: i64 [n_stars+1], first row of each star.
+ * out: host or device. */
+int32_t gsr_get_star_rowptr(gsr_handle *h, int64_t *out);
+
+/* Column preconditioning (Alg. 1 l.2-3): p_j = 1/||A_:j||_2 over all
+ * rows including constraints (1 for an empty column), A_ij <- fl(A_ij * p_j) in
+ * place on the device.  A second call is GSR_ESTATE. */
+int32_t gsr_precondition(gsr_handle *h);
+
+/* p (n doubles; all 1 before gsr_precondition).  out: host or device. */
+int32_t gsr_get_colscale(gsr_handle *h, double *out);
+
+/* Device copy of the matrix values as they stand (scaled if preconditioned):
+ * out f64 [n_obs*24], host or device; con_val_out f64 [n_con_nnz] or NULL. */
+int32_t gsr_get_values(gsr_handle *h, double *out, double *con_val_out);
+
+/* aprod mode 1, Eq. 2, Algorithm 2:  y += A x  on the matrix as it
+ * stands on the device.  x: n doubles, y: n_obs+n_con doubles, both DEVICE. */
+int32_t gsr_aprod1(gsr_handle *h, const double *x, double *y);
+
+/* aprod mode 2, Eq. 3, Algorithm 3:  x += A^T y.  DEVICE pointers.
+ * The astrometric and global sections are summed in a fixed order (bit
+ * reproducible); attitude and instrumental sums use floating-point atomics and
+ * may differ in the last bits from run to run. */
+int32_t gsr_aprod2(gsr_handle *h, const double *y, double *x);
+
+/* LSQR of Paige & Saunders (Alg. 1 l.13-27) with damp = 0
+ * on the device matrix and the uploaded b; b is not modified.  Runs at most itnlim
+ * iterations; conlim <= 0 disables the condition-number test.  The whole iteration
+ * (both aprods, norms, rotations, vector updates, stop tests) runs on the device;
+ * the host only polls istop.  Writes x = p (.) z and se = p (.) se_z. */
+int32_t gsr_lsqr(gsr_handle *h, int64_t itnlim, double atol, double btol, double conlim,
+                 gsr_result *result);
+
+/* Per-iteration log of the last gsr_lsqr: up to max_itn rows of 5 doubles
+ * (rnorm, arnorm, anorm, acond, xnorm) to a HOST buffer; returns rows written in
+ * *n_written.  Only the last GSR_TRACE_CAP iterations are kept. */
+#define GSR_TRACE_CAP 4096
+int32_t gsr_get_trace(gsr_handle *h, double *out, int64_t max_itn, int64_t *n_written);
+
+/* Device time of the last gsr_lsqr's iteration loop in milliseconds (CUDA events on
+ * the handle's stream), and the number of kernels launched in it. */
+int32_t gsr_last_timing(gsr_handle *h, double *loop_ms, int64_t *kernel_launches);
+
+/* Timing hooks for bench.py: run `reps` back-to-back launches of the kernel group of
+ * one product (which = 1: aprod1 group, 2: aprod2 group) with the LSQR scalars set
+ * to 1, on internal u/v work vectors, and return the mean device time per group in
+ * milliseconds (CUDA events on the handle's stream). */
+int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_per_launch);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GSR_H */

@@ -1,0 +1,616 @@
+// gsr.cu -- host side of libgsr.so (C ABI declared in include/gsr.h).
+// Everything numeric runs in the kernels of gsr_kernels.cuh; this file owns the device
+// storage, validates uploads, orders the kernels on one stream and captures the LSQR
+// iteration in a CUDA graph.  No CPU arithmetic path exists.
+#include "gsr.h"
+#include "gsr_kernels.cuh"
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+using namespace gsr;
+
+struct gsr_handle {
+    gsr_layout L{};
+    int64_t n = 0, mTot = 0, nTiles = 0;
+    cudaStream_t stream = nullptr;
+    cudaStream_t userStream = nullptr;
+    int smCount = 148;
+    // system
+    double *V = nullptr, *b = nullptr, *conVal = nullptr, *p = nullptr;
+    int64_t *ia = nullptr, *iatt = nullptr, *rp = nullptr, *conRp = nullptr, *conCol = nullptr;
+    int32_t *ic = nullptr;
+    // work
+    double *u = nullptr, *v = nullptr, *w = nullptr, *z = nullptr, *var = nullptr;
+    double *carryFirst = nullptr, *carryLast = nullptr, *globPartial = nullptr;
+    double *sqPartialU = nullptr, *sqPartialV = nullptr, *ddPartial = nullptr;
+    double *coefOne = nullptr, *coefTime = nullptr, *trace = nullptr;
+    Scalars *S = nullptr;
+    Scalars *hostS = nullptr;           // pinned, 2 slots
+    unsigned long long *badDev = nullptr;
+    int gridA1 = 1, gridA2 = 1, gridVec = 1, gridCon = 1, gridFix = 1;
+    bool uploaded = false, conUploaded = false, preconditioned = false, workReady = false;
+    int64_t badRow = -1;
+    cudaGraphExec_t iterGraph = nullptr;
+    cudaEvent_t ev0 = nullptr, ev1 = nullptr, evSlot[2] = {nullptr, nullptr};
+    double loopMs = 0.0;
+    int64_t launches = 0, lastItn = 0;
+    char err[512] = {0};
+};
+
+namespace {
+
+int fail(gsr_handle *h, int code, const char *fmt, ...)
+{
+    if (h) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(h->err, sizeof(h->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define CK(call)                                                                          \
+    do {                                                                                  \
+        cudaError_t e_ = (call);                                                          \
+        if (e_ != cudaSuccess) {                                                          \
+            cudaGetLastError();                                                           \
+            return fail(h, e_ == cudaErrorMemoryAllocation ? GSR_ENOMEM : GSR_ECUDA,      \
+                        "%s:%d %s: %s", __FILE__, __LINE__, #call, cudaGetErrorString(e_)); \
+        }                                                                                 \
+    } while (0)
+
+template <class T>
+cudaError_t dalloc(T **p, int64_t count)
+{
+    *p = nullptr;
+    return cudaMalloc(reinterpret_cast<void **>(p), size_t(std::max<int64_t>(count, 1)) * sizeof(T));
+}
+
+MatView view(const gsr_handle *h)
+{
+    MatView A;
+    A.V = h->V; A.ia = h->ia; A.iatt = h->iatt; A.ic = h->ic; A.rp = h->rp;
+    A.m = h->L.n_obs; A.nStars = h->L.n_stars; A.nDof = h->L.n_dof_att; A.nInstr = h->L.n_instr;
+    A.offAtt = 5 * h->L.n_stars;
+    A.offInstr = A.offAtt + 3 * h->L.n_dof_att;
+    A.offGlob = A.offInstr + h->L.n_instr;
+    A.n = h->n;
+    A.conRp = h->conRp; A.conCol = h->conCol; A.conVal = h->conVal; A.nCon = h->L.n_con;
+    return A;
+}
+
+int gridFor(int64_t count, int perBlock, int cap)
+{
+    int64_t g = (count + perBlock - 1) / perBlock;
+    return int(std::max<int64_t>(1, std::min<int64_t>(g, cap)));
+}
+
+int enter(gsr_handle *h)
+{
+    CK(cudaSetDevice(h->L.device));
+    if (h->userStream) CK(cudaStreamSynchronize(h->userStream));
+    return GSR_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
+{
+    if (!out) return GSR_EINVAL;
+    *out = nullptr;
+    if (!L) return GSR_EINVAL;
+    gsr_handle *h = new (std::nothrow) gsr_handle;
+    if (!h) return GSR_ENOMEM;
+    *out = h;   // returned even on failure so that gsr_last_error works; caller destroys it
+    h->L = *L;
+    if (L->n_astro_par != GSR_N_ASTRO || L->n_att_par != GSR_N_ATT || L->n_instr_par != GSR_N_INSTR ||
+        L->n_glob_par != GSR_N_GLOB)
+        return fail(h, GSR_EINVAL, "section widths must be 5/12/6/1 (got %d/%d/%d/%d)", L->n_astro_par,
+                    L->n_att_par, L->n_instr_par, L->n_glob_par);
+    if (L->n_obs < 0 || L->n_stars < 1 || L->n_dof_att < 4 || L->n_instr < 6 || L->n_con < 0 ||
+        L->n_con_nnz < 0 || (L->n_con == 0 && L->n_con_nnz != 0))
+        return fail(h, GSR_EINVAL, "bad sizes");
+    h->n = 5 * L->n_stars + 3 * L->n_dof_att + L->n_instr + 1;
+    h->mTot = L->n_obs + L->n_con;
+    h->nTiles = (L->n_obs + TILE - 1) / TILE;
+    h->userStream = static_cast<cudaStream_t>(L->stream);
+    int ndev = 0;
+    CK(cudaGetDeviceCount(&ndev));
+    if (L->device < 0 || L->device >= ndev) return fail(h, GSR_EINVAL, "device %d of %d", L->device, ndev);
+    CK(cudaSetDevice(L->device));
+    CK(cudaDeviceGetAttribute(&h->smCount, cudaDevAttrMultiProcessorCount, L->device));
+    CK(cudaStreamCreateWithFlags(&h->stream, cudaStreamNonBlocking));
+    CK(cudaEventCreate(&h->ev0));
+    CK(cudaEventCreate(&h->ev1));
+    CK(cudaEventCreateWithFlags(&h->evSlot[0], cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&h->evSlot[1], cudaEventDisableTiming));
+
+    CK(cudaFuncSetAttribute(k_aprod1, cudaFuncAttributeMaxDynamicSharedMemorySize, int(APROD_SMEM)));
+    CK(cudaFuncSetAttribute(k_aprod2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(APROD_SMEM)));
+    CK(cudaFuncSetAttribute(k_aprod2<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(APROD_SMEM)));
+    int occ1 = 1, occ2 = 1;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, k_aprod1, THREADS, APROD_SMEM));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, k_aprod2<false>, THREADS, APROD_SMEM));
+    h->gridA1 = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ1, 1));
+    h->gridA2 = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ2, 1));
+    h->gridVec = gridFor(std::max(h->n, h->mTot), 256 * 4, h->smCount * 8);
+    h->gridCon = gridFor(L->n_con, 8, h->smCount * 8);
+    h->gridFix = int((L->n_stars + 255) / 256) + 1;
+
+    const int64_t m = L->n_obs;
+    CK(dalloc(&h->V, m * N_PAR));
+    CK(dalloc(&h->ia, m));
+    CK(dalloc(&h->iatt, m));
+    CK(dalloc(&h->ic, m * N_INSTR));
+    CK(dalloc(&h->b, h->mTot));
+    CK(dalloc(&h->rp, L->n_stars + 1));
+    CK(dalloc(&h->conRp, L->n_con + 1));
+    CK(dalloc(&h->conCol, L->n_con_nnz));
+    CK(dalloc(&h->conVal, L->n_con_nnz));
+    CK(dalloc(&h->p, h->n));
+    CK(dalloc(&h->carryFirst, h->nTiles * N_ASTRO));
+    CK(dalloc(&h->carryLast, h->nTiles * N_ASTRO));
+    CK(dalloc(&h->globPartial, h->gridA2));
+    CK(dalloc(&h->sqPartialU, h->gridA1 + h->gridCon));
+    CK(dalloc(&h->sqPartialV, h->gridVec));
+    CK(dalloc(&h->ddPartial, h->gridVec));
+    CK(dalloc(&h->coefOne, 2));
+    CK(dalloc(&h->coefTime, 2));
+    CK(dalloc(&h->trace, 5 * GSR_TRACE_CAP));
+    CK(dalloc(&h->S, 1));
+    CK(dalloc(&h->badDev, 1));
+    CK(cudaMallocHost(reinterpret_cast<void **>(&h->hostS), 2 * sizeof(Scalars)));
+    const double one[2] = {1.0, 1.0}, tm[2] = {0.5, 0.5};
+    CK(cudaMemcpy(h->coefOne, one, sizeof(one), cudaMemcpyHostToDevice));
+    CK(cudaMemcpy(h->coefTime, tm, sizeof(tm), cudaMemcpyHostToDevice));
+    CK(cudaMemset(h->conRp, 0, sizeof(int64_t) * size_t(L->n_con + 1)));
+    k_fill<<<h->gridVec, 256, 0, h->stream>>>(h->p, h->n, 1.0);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(h->stream));
+    return GSR_OK;
+}
+
+int32_t gsr_destroy(gsr_handle *h)
+{
+    if (!h) return GSR_OK;
+    cudaSetDevice(h->L.device);
+    if (h->stream) cudaStreamSynchronize(h->stream);
+    if (h->iterGraph) cudaGraphExecDestroy(h->iterGraph);
+    void *ptrs[] = {h->V, h->b, h->conVal, h->p, h->ia, h->iatt, h->rp, h->conRp, h->conCol, h->ic,
+                    h->u, h->v, h->w, h->z, h->var, h->carryFirst, h->carryLast, h->globPartial,
+                    h->sqPartialU, h->sqPartialV, h->ddPartial, h->coefOne, h->coefTime, h->trace,
+                    h->S, h->badDev};
+    for (void *q : ptrs)
+        if (q) cudaFree(q);
+    if (h->hostS) cudaFreeHost(h->hostS);
+    if (h->ev0) cudaEventDestroy(h->ev0);
+    if (h->ev1) cudaEventDestroy(h->ev1);
+    for (auto &e : h->evSlot)
+        if (e) cudaEventDestroy(e);
+    if (h->stream) cudaStreamDestroy(h->stream);
+    cudaGetLastError();
+    delete h;
+    return GSR_OK;
+}
+
+const char *gsr_last_error(const gsr_handle *h) { return h ? h->err : "null handle"; }
+int64_t gsr_bad_row(const gsr_handle *h) { return h ? h->badRow : -1; }
+int64_t gsr_ncols(const gsr_handle *h) { return h ? h->n : -1; }
+int64_t gsr_nrows(const gsr_handle *h) { return h ? h->mTot : -1; }
+
+int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double *values,
+                        const int64_t *ia, const int64_t *iatt, const int32_t *ic, const double *b)
+{
+    if (!h) return GSR_EINVAL;
+    if (row0 < 0 || nrows < 0 || row0 + nrows > h->L.n_obs) return fail(h, GSR_EINVAL, "row range");
+    if (nrows > 0 && (!values || !ia || !iatt || !ic || !b)) return fail(h, GSR_EINVAL, "null array");
+    int rc = enter(h);
+    if (rc) return rc;
+    h->uploaded = false;
+    h->preconditioned = false;
+    const size_t r = size_t(nrows);
+    CK(cudaMemcpyAsync(h->V + row0 * N_PAR, values, r * N_PAR * sizeof(double), cudaMemcpyDefault, h->stream));
+    CK(cudaMemcpyAsync(h->ia + row0, ia, r * sizeof(int64_t), cudaMemcpyDefault, h->stream));
+    CK(cudaMemcpyAsync(h->iatt + row0, iatt, r * sizeof(int64_t), cudaMemcpyDefault, h->stream));
+    CK(cudaMemcpyAsync(h->ic + row0 * N_INSTR, ic, r * N_INSTR * sizeof(int32_t), cudaMemcpyDefault, h->stream));
+    CK(cudaMemcpyAsync(h->b + row0, b, r * sizeof(double), cudaMemcpyDefault, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return GSR_OK;
+}
+
+int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail)
+{
+    if (!h) return GSR_EINVAL;
+    if (h->L.n_con > 0 && !b_tail) return fail(h, GSR_EINVAL, "b_tail is NULL but n_con > 0");
+    int rc = enter(h);
+    if (rc) return rc;
+    if (h->L.n_con > 0)
+        CK(cudaMemcpyAsync(h->b + h->L.n_obs, b_tail, size_t(h->L.n_con) * sizeof(double), cudaMemcpyDefault,
+                           h->stream));
+    const unsigned long long none = ~0ull;
+    CK(cudaMemcpyAsync(h->badDev, &none, sizeof(none), cudaMemcpyHostToDevice, h->stream));
+    MatView A = view(h);
+    k_validate<<<gridFor(A.m, 256, h->smCount * 16), 256, 0, h->stream>>>(A, h->badDev);
+    CK(cudaGetLastError());
+    unsigned long long bad = none;
+    CK(cudaMemcpyAsync(&bad, h->badDev, sizeof(bad), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    if (bad != none) {
+        h->badRow = int64_t(bad);
+        return fail(h, GSR_EINDEX, "index contract violated at observation row %lld", (long long)bad);
+    }
+    h->badRow = -1;
+    k_star_rowptr<<<int((h->L.n_stars + 1 + 255) / 256), 256, 0, h->stream>>>(h->ia, A.m, A.nStars, h->rp);
+    CK(cudaGetLastError());
+    k_fill<<<h->gridVec, 256, 0, h->stream>>>(h->p, h->n, 1.0);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(h->stream));
+    h->uploaded = true;
+    h->preconditioned = false;
+    return GSR_OK;
+}
+
+int32_t gsr_upload(gsr_handle *h, const double *values, const int64_t *ia, const int64_t *iatt,
+                   const int32_t *ic, const double *b)
+{
+    if (!h) return GSR_EINVAL;
+    if (!b && h->mTot > 0) return fail(h, GSR_EINVAL, "null array");
+    int rc = gsr_upload_rows(h, 0, h->L.n_obs, values, ia, iatt, ic, b);
+    if (rc) return rc;
+    return gsr_upload_finish(h, h->L.n_con > 0 ? b + h->L.n_obs : nullptr);
+}
+
+int32_t gsr_upload_constraints(gsr_handle *h, const int64_t *rowptr, const int64_t *col, const double *val)
+{
+    if (!h) return GSR_EINVAL;
+    if (h->L.n_con == 0) return fail(h, GSR_EINVAL, "layout has no constraint rows");
+    if (!rowptr || !col || !val) return fail(h, GSR_EINVAL, "null array");
+    if (h->preconditioned) return fail(h, GSR_ESTATE, "constraints must be uploaded before gsr_precondition");
+    int rc = enter(h);
+    if (rc) return rc;
+    const int64_t nnz = h->L.n_con_nnz;
+    CK(cudaMemcpyAsync(h->conRp, rowptr, size_t(h->L.n_con + 1) * sizeof(int64_t), cudaMemcpyDefault, h->stream));
+    CK(cudaMemcpyAsync(h->conCol, col, size_t(nnz) * sizeof(int64_t), cudaMemcpyDefault, h->stream));
+    CK(cudaMemcpyAsync(h->conVal, val, size_t(nnz) * sizeof(double), cudaMemcpyDefault, h->stream));
+    const unsigned long long none = ~0ull;
+    CK(cudaMemcpyAsync(h->badDev, &none, sizeof(none), cudaMemcpyHostToDevice, h->stream));
+    MatView A = view(h);
+    k_validate_con<<<gridFor(std::max(nnz, A.nCon + 1), 256, h->smCount * 16), 256, 0, h->stream>>>(A, nnz, h->badDev);
+    CK(cudaGetLastError());
+    unsigned long long bad = none;
+    CK(cudaMemcpyAsync(&bad, h->badDev, sizeof(bad), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    if (bad != none) {
+        h->badRow = int64_t(bad);
+        h->conUploaded = false;
+        return fail(h, GSR_EINDEX, "constraint CSR violated at entry %lld", (long long)bad);
+    }
+    h->conUploaded = true;
+    return GSR_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------
+// kernel groups
+// ---------------------------------------------------------------------------------------
+namespace {
+
+int readyCheck(gsr_handle *h)
+{
+    if (!h->uploaded) return fail(h, GSR_ESTATE, "no system uploaded");
+    if (h->L.n_con > 0 && !h->conUploaded) return fail(h, GSR_ESTATE, "constraint rows not uploaded");
+    return GSR_OK;
+}
+
+// y <- cy*y + cx*(A x); partials of sum y^2 go to sqPartial (or nowhere).  Returns #kernels.
+int enqueueAprod1(gsr_handle *h, const double *x, double *y, const double *coef, double *sqPartial,
+                  const int *done, int *nPartial)
+{
+    MatView A = view(h);
+    k_aprod1<<<h->gridA1, THREADS, APROD_SMEM, h->stream>>>(A, x, y, coef, sqPartial, done);
+    int nk = 1, np = h->gridA1;
+    if (A.nCon > 0) {
+        k_con_aprod1<<<h->gridCon, 256, 0, h->stream>>>(A, x, y, coef, sqPartial ? sqPartial + h->gridA1 : nullptr, done);
+        ++nk;
+        np += h->gridCon;
+    }
+    if (nPartial) *nPartial = np;
+    return nk;
+}
+
+// x <- cx*x + cy*(A^T y).  prescale: multiply the att/instr/gamma sections by cx first
+// (needed whenever cx != 1).  Returns #kernels.
+template <bool SQUARE>
+int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef, const int *done, bool prescale)
+{
+    MatView A = view(h);
+    int nk = 0;
+    if (prescale) {
+        k_scale<<<h->gridVec, 256, 0, h->stream>>>(x, A.offAtt, A.n, coef, done);
+        ++nk;
+    }
+    k_aprod2<SQUARE><<<h->gridA2, THREADS, APROD_SMEM, h->stream>>>(A, y, x, coef, h->carryFirst, h->carryLast,
+                                                                  h->globPartial, done);
+    k_astro_fixup<<<h->gridFix, 256, 0, h->stream>>>(A, x, coef, h->carryFirst, h->carryLast, h->globPartial,
+                                                     h->gridA2, done);
+    nk += 2;
+    if (A.nCon > 0) {
+        k_con_aprod2<SQUARE><<<h->gridCon, 256, 0, h->stream>>>(A, y, x, coef, done);
+        ++nk;
+    }
+    return nk;
+}
+
+int ensureWork(gsr_handle *h)
+{
+    if (h->workReady) return GSR_OK;
+    CK(dalloc(&h->u, h->mTot));
+    CK(dalloc(&h->v, h->n));
+    CK(dalloc(&h->w, h->n));
+    CK(dalloc(&h->z, h->n));
+    CK(dalloc(&h->var, h->n));
+    h->workReady = true;
+    return GSR_OK;
+}
+
+// One LSQR iteration enqueued on h->stream.  Returns #kernels.
+int enqueueIteration(gsr_handle *h)
+{
+    Scalars *S = h->S;
+    const int *done = &S->done;
+    int nk = 0, npU = 0;
+    nk += enqueueAprod1(h, h->v, h->u, &S->a1_cx, h->sqPartialU, done, &npU);
+    k_scalar<<<1, 256, 0, h->stream>>>(PH_AFTER_APROD1, S, h->sqPartialU, npU, nullptr, 0);
+    nk += enqueueAprod2<false>(h, h->u, h->v, &S->a2_cx, done, true);
+    k_sumsq<<<h->gridVec, 256, 0, h->stream>>>(h->v, h->n, h->sqPartialV, done);
+    k_scalar<<<1, 256, 0, h->stream>>>(PH_AFTER_APROD2, S, h->sqPartialV, h->gridVec, nullptr, 0);
+    k_update<<<h->gridVec, 256, 0, h->stream>>>(h->z, h->w, h->v, h->var, h->n, S, h->ddPartial);
+    k_scalar<<<1, 256, 0, h->stream>>>(PH_AFTER_UPDATE, S, h->ddPartial, h->gridVec, h->trace, GSR_TRACE_CAP);
+    return nk + 5;
+}
+
+}  // namespace
+
+extern "C" {
+
+int32_t gsr_get_star_rowptr(gsr_handle *h, int64_t *out)
+{
+    if (!h || !out) return GSR_EINVAL;
+    if (!h->uploaded) return fail(h, GSR_ESTATE, "no system uploaded");
+    int rc = enter(h);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(out, h->rp, size_t(h->L.n_stars + 1) * sizeof(int64_t), cudaMemcpyDefault, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return GSR_OK;
+}
+
+int32_t gsr_get_colscale(gsr_handle *h, double *out)
+{
+    if (!h || !out) return GSR_EINVAL;
+    int rc = enter(h);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(out, h->p, size_t(h->n) * sizeof(double), cudaMemcpyDefault, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return GSR_OK;
+}
+
+int32_t gsr_get_values(gsr_handle *h, double *out, double *con_val_out)
+{
+    if (!h || !out) return GSR_EINVAL;
+    if (!h->uploaded) return fail(h, GSR_ESTATE, "no system uploaded");
+    int rc = enter(h);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(out, h->V, size_t(h->L.n_obs) * N_PAR * sizeof(double), cudaMemcpyDefault, h->stream));
+    if (con_val_out && h->L.n_con_nnz > 0)
+        CK(cudaMemcpyAsync(con_val_out, h->conVal, size_t(h->L.n_con_nnz) * sizeof(double), cudaMemcpyDefault,
+                           h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return GSR_OK;
+}
+
+int32_t gsr_precondition(gsr_handle *h)
+{
+    if (!h) return GSR_EINVAL;
+    int rc = readyCheck(h);
+    if (rc) return rc;
+    if (h->preconditioned) return fail(h, GSR_ESTATE, "already preconditioned");
+    rc = enter(h);
+    if (rc) return rc;
+    MatView A = view(h);
+    // column sums of squares = aprod2 with squared coefficients and y == 1 (same kernels,
+    // same fixed order for the astro and gamma sections)
+    CK(cudaMemsetAsync(h->p, 0, size_t(h->n) * sizeof(double), h->stream));
+    enqueueAprod2<true>(h, nullptr, h->p, h->coefOne, nullptr, false);
+    CK(cudaGetLastError());
+    k_colscale<<<h->gridVec, 256, 0, h->stream>>>(h->p, h->n);
+    k_scale_values<<<gridFor(A.m * N_PAR, 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(A, h->p);
+    if (A.nCon > 0)
+        k_scale_con_values<<<gridFor(h->L.n_con_nnz, 256, h->smCount * 16), 256, 0, h->stream>>>(A, h->L.n_con_nnz, h->p);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(h->stream));
+    h->preconditioned = true;
+    return GSR_OK;
+}
+
+int32_t gsr_aprod1(gsr_handle *h, const double *x, double *y)
+{
+    if (!h || !x || !y) return GSR_EINVAL;
+    int rc = readyCheck(h);
+    if (rc) return rc;
+    rc = enter(h);
+    if (rc) return rc;
+    enqueueAprod1(h, x, y, h->coefOne, nullptr, nullptr, nullptr);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(h->stream));
+    return GSR_OK;
+}
+
+int32_t gsr_aprod2(gsr_handle *h, const double *y, double *x)
+{
+    if (!h || !x || !y) return GSR_EINVAL;
+    int rc = readyCheck(h);
+    if (rc) return rc;
+    rc = enter(h);
+    if (rc) return rc;
+    enqueueAprod2<false>(h, y, x, h->coefOne, nullptr, false);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(h->stream));
+    return GSR_OK;
+}
+
+int32_t gsr_lsqr(gsr_handle *h, int64_t itnlim, double atol, double btol, double conlim, gsr_result *R)
+{
+    if (!h || !R || !R->x) return GSR_EINVAL;
+    int rc = readyCheck(h);
+    if (rc) return rc;
+    rc = enter(h);
+    if (rc) return rc;
+    rc = ensureWork(h);
+    if (rc) return rc;
+    cudaStream_t st = h->stream;
+    Scalars init;
+    memset(&init, 0, sizeof(init));
+    init.atol = atol; init.btol = btol; init.ctol = conlim > 0.0 ? 1.0 / conlim : 0.0;
+    init.itnlim = itnlim;
+    CK(cudaMemcpyAsync(h->S, &init, sizeof(init), cudaMemcpyHostToDevice, st));
+    // step 1: u^ = b, beta = |b|; v^ = A^T u^/beta, alpha = |v^|; w = v; x = var = 0
+    CK(cudaMemcpyAsync(h->u, h->b, size_t(h->mTot) * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    CK(cudaMemsetAsync(h->v, 0, size_t(h->n) * sizeof(double), st));
+    CK(cudaMemsetAsync(h->z, 0, size_t(h->n) * sizeof(double), st));
+    CK(cudaMemsetAsync(h->var, 0, size_t(h->n) * sizeof(double), st));
+    k_sumsq<<<h->gridVec, 256, 0, st>>>(h->u, h->mTot, h->sqPartialV, nullptr);
+    k_scalar<<<1, 256, 0, st>>>(PH_INIT_BETA, h->S, h->sqPartialV, h->gridVec, nullptr, 0);
+    enqueueAprod2<false>(h, h->u, h->v, &h->S->a2_cx, nullptr, false);
+    k_sumsq<<<h->gridVec, 256, 0, st>>>(h->v, h->n, h->sqPartialV, nullptr);
+    k_scalar<<<1, 256, 0, st>>>(PH_INIT_ALPHA, h->S, h->sqPartialV, h->gridVec, nullptr, 0);
+    k_init_w<<<h->gridVec, 256, 0, st>>>(h->w, h->v, h->n, h->S);
+    CK(cudaGetLastError());
+
+    // the iteration as one CUDA graph; re-captured per solve because the
+    // work pointers and grids are fixed per handle, it is captured once and kept
+    int perIter = 0;
+    if (!h->iterGraph) {
+        cudaGraph_t g = nullptr;
+        CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+        perIter = enqueueIteration(h);
+        cudaError_t ec = cudaStreamEndCapture(st, &g);
+        if (ec != cudaSuccess) return fail(h, GSR_ECUDA, "graph capture: %s", cudaGetErrorString(ec));
+        ec = cudaGraphInstantiate(&h->iterGraph, g, 0);
+        cudaGraphDestroy(g);
+        if (ec != cudaSuccess) return fail(h, GSR_ECUDA, "graph instantiate: %s", cudaGetErrorString(ec));
+    }
+    perIter = 7 + (h->L.n_con > 0 ? 2 : 0) + 3;
+
+    // Loop control: the device decides (S->done); the host enqueues chunks of graph launches and
+    // polls the scalars of the previous chunk while the next one runs.
+    CK(cudaEventRecord(h->ev0, st));
+    int64_t launched = 0;
+    int slot = 0;
+    bool pending[2] = {false, false};
+    bool stop = false;
+    const int64_t chunk = h->L.n_obs > (int64_t(1) << 22) ? 4 : 32;
+    while (!stop && launched < itnlim) {
+        const int64_t c = std::min<int64_t>(chunk, itnlim - launched);
+        for (int64_t k = 0; k < c; ++k) CK(cudaGraphLaunch(h->iterGraph, st));
+        launched += c;
+        CK(cudaMemcpyAsync(&h->hostS[slot], h->S, sizeof(Scalars), cudaMemcpyDeviceToHost, st));
+        CK(cudaEventRecord(h->evSlot[slot], st));
+        pending[slot] = true;
+        const int prev = slot ^ 1;
+        if (pending[prev]) {
+            CK(cudaEventSynchronize(h->evSlot[prev]));
+            pending[prev] = false;
+            if (h->hostS[prev].done) stop = true;
+        }
+        slot ^= 1;
+    }
+    CK(cudaEventRecord(h->ev1, st));
+    CK(cudaStreamSynchronize(st));
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, h->ev0, h->ev1));
+    h->loopMs = ms;
+    h->launches = launched * perIter;
+
+    // finish (Alg. 1 l.27): x = p (.) z, se; staged in v / w when the outputs are host memory
+    k_finish<<<h->gridVec, 256, 0, st>>>(h->z, h->var, h->p, h->v, R->se ? h->w : nullptr, h->n, h->mTot, h->S);
+    CK(cudaGetLastError());
+    CK(cudaMemcpyAsync(R->x, h->v, size_t(h->n) * sizeof(double), cudaMemcpyDefault, st));
+    if (R->se) CK(cudaMemcpyAsync(R->se, h->w, size_t(h->n) * sizeof(double), cudaMemcpyDefault, st));
+    CK(cudaMemcpyAsync(&h->hostS[0], h->S, sizeof(Scalars), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    const Scalars &F = h->hostS[0];
+    R->istop = F.istop; R->itn = F.itn; R->anorm = F.anorm; R->acond = F.acond;
+    R->rnorm = F.rnorm; R->arnorm = F.arnorm; R->xnorm = F.xnorm;
+    h->lastItn = F.itn;
+    return GSR_OK;
+}
+
+int32_t gsr_get_trace(gsr_handle *h, double *out, int64_t max_itn, int64_t *n_written)
+{
+    if (!h || !out || !n_written) return GSR_EINVAL;
+    int rc = enter(h);
+    if (rc) return rc;
+    const int64_t have = std::min<int64_t>(h->lastItn, GSR_TRACE_CAP);
+    const int64_t cnt = std::min(have, max_itn);
+    const int64_t first = h->lastItn - cnt;   // iteration index (0-based) of the first row returned
+    for (int64_t k = 0; k < cnt; ++k)
+        CK(cudaMemcpy(out + 5 * k, h->trace + 5 * ((first + k) % GSR_TRACE_CAP), 5 * sizeof(double),
+                      cudaMemcpyDeviceToHost));
+    *n_written = cnt;
+    return GSR_OK;
+}
+
+int32_t gsr_last_timing(gsr_handle *h, double *loop_ms, int64_t *kernel_launches)
+{
+    if (!h) return GSR_EINVAL;
+    if (loop_ms) *loop_ms = h->loopMs;
+    if (kernel_launches) *kernel_launches = h->launches;
+    return GSR_OK;
+}
+
+int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_per_launch)
+{
+    if (!h || !ms_per_launch || reps < 1) return GSR_EINVAL;
+    if (which != 1 && which != 2 && which != 11 && which != 12) return fail(h, GSR_EINVAL, "which");
+    int rc = readyCheck(h);
+    if (rc) return rc;
+    rc = enter(h);
+    if (rc) return rc;
+    rc = ensureWork(h);
+    if (rc) return rc;
+    cudaStream_t st = h->stream;
+    MatView A = view(h);
+    // bounded operands: u = b, v = 1e-3; coefficients 0.5 keep repeated products finite
+    CK(cudaMemcpyAsync(h->u, h->b, size_t(h->mTot) * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    k_fill<<<h->gridVec, 256, 0, st>>>(h->v, h->n, 1e-3);
+    auto once = [&]() {
+        if (which == 1) enqueueAprod1(h, h->v, h->u, h->coefTime, h->sqPartialU, nullptr, nullptr);
+        else if (which == 2) enqueueAprod2<false>(h, h->u, h->v, h->coefTime, nullptr, true);
+        else if (which == 11)
+            k_aprod1<<<h->gridA1, THREADS, APROD_SMEM, st>>>(A, h->v, h->u, h->coefTime, h->sqPartialU, nullptr);
+        else
+            k_aprod2<false><<<h->gridA2, THREADS, APROD_SMEM, st>>>(A, h->u, h->v, h->coefTime, h->carryFirst,
+                                                                 h->carryLast, h->globPartial, nullptr);
+    };
+    once();   // warm-up
+    CK(cudaGetLastError());
+    CK(cudaEventRecord(h->ev0, st));
+    for (int r = 0; r < reps; ++r) once();
+    CK(cudaEventRecord(h->ev1, st));
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(st));
+    float ms = 0.f;
+    CK(cudaEventElapsedTime(&ms, h->ev0, h->ev1));
+    *ms_per_launch = double(ms) / reps;
+    return GSR_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,644 @@
+// gsr_kernels.cuh -- sm_100a kernels of the AVU-GSR LSQR hot path (arXiv 2308.00778).
+// Citations are lines of PAPER.md; the design is described in DESIGN.md.
+// No tensor cores: the path is two sparse products bound by HBM and by gather/scatter rate.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace gsr {
+
+constexpr int N_ASTRO = 5, N_ATT = 12, N_INSTR = 6, N_PAR = 24;
+constexpr int TILE = 32;          // rows per warp tile
+constexpr int ROW_PAD = 26;       // doubles per staged row in shared memory (208 B: LDS.128 conflict-free)
+constexpr int WARPS = 8;          // warps per CTA of the aprod kernels
+constexpr int THREADS = WARPS * 32;
+constexpr size_t APROD_SMEM = size_t(WARPS) * TILE * ROW_PAD * sizeof(double);
+
+// Device view of the uploaded system (A_d, M_i, I_c) in upload layout.
+struct MatView {
+    double *V;             // [m*24]
+    const int64_t *ia;     // [m] 5*star
+    const int64_t *iatt;   // [m] attitude start s_i (axis 0)
+    const int32_t *ic;     // [m*6]
+    const int64_t *rp;     // [nStars+1] derived star row pointer
+    int64_t m, nStars, nDof, nInstr;
+    int64_t offAtt, offInstr, offGlob, n;
+    // constraint rows (CSR, absolute columns)
+    const int64_t *conRp, *conCol;
+    double *conVal;
+    int64_t nCon;
+};
+
+// Scalars of the LSQR recurrences, resident in device memory.
+struct Scalars {
+    // coefficients read by the vector / aprod kernels
+    double a1_cx, a1_cy;   // aprod1:  u^ <- a1_cx * (A v^) + a1_cy * u^
+    double a2_cx, a2_cy;   // aprod2:  v^ <- a2_cx * v^ + a2_cy * (A^T u^)
+    double t1, t2, inv_rho, inv_alpha;
+    // recurrence state
+    double alpha, beta, rhobar, phibar, bnorm, anorm, acond, ddnorm, xxnorm, xnorm, z, cs2, sn2;
+    double rnorm, arnorm;
+    double atol, btol, ctol;
+    long long itn, itnlim;
+    int istop;
+    int done;              // 1: loop body is a no-op (stopped, or trivial system)
+};
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Deterministic block sum (fixed tree); result valid in thread 0.  red: >= 32 doubles of smem.
+__device__ __forceinline__ double block_sum(double v, double *red)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    v = warp_sum(v);
+    __syncthreads();
+    if (lane == 0) red[w] = v;
+    __syncthreads();
+    double r = 0.0;
+    if (w == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        r = lane < nw ? red[lane] : 0.0;
+        r = warp_sum(r);
+    }
+    return r;
+}
+
+// Coalesced load of one warp tile (nrows x 192 B, contiguous in global memory) with 16-byte
+// vector loads, staged row-padded into shared memory so that each lane can then read its own
+// row with conflict-free LDS.128 ("coalesced, vectorised 16-byte loads of
+// each row's 192-byte value block").
+__device__ __forceinline__ void stage_tile(double *sm, const double *gV, int nrows, int lane)
+{
+    const double2 *g = reinterpret_cast<const double2 *>(gV);
+    const int nchunk = nrows * 12;
+    double2 r[12];
+#pragma unroll
+    for (int t = 0; t < 12; ++t) {
+        const int c = t * 32 + lane;
+        if (c < nchunk) r[t] = __ldcs(g + c);
+    }
+#pragma unroll
+    for (int t = 0; t < 12; ++t) {
+        const int c = t * 32 + lane;
+        if (c < nchunk) {
+            const int row = c / 12, q = c - row * 12;
+            *reinterpret_cast<double2 *>(sm + row * ROW_PAD + 2 * q) = r[t];
+        }
+    }
+}
+
+__device__ __forceinline__ void read_row(const double *sm, int lane, double (&v)[N_PAR])
+{
+    const double2 *s = reinterpret_cast<const double2 *>(sm + lane * ROW_PAD);
+#pragma unroll
+    for (int q = 0; q < 12; ++q) {
+        const double2 t = s[q];
+        v[2 * q] = t.x;
+        v[2 * q + 1] = t.y;
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// aprod mode 1 (Eq. 2; Algorithm 2):  y <- cy*y + cx*(A x), one pass over A,
+// all four sections in one kernel, plus the per-CTA partial of sum y^2 (Eq. 4's norm, fused:
+// SURVEY a3).  coef = {cx, cy} in device memory.  Row i <-> one lane; a warp owns 32
+// consecutive rows, a CTA 256.
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(THREADS, 2)
+k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
+         const double *__restrict__ coef, double *__restrict__ sqPartial, const int *done)
+{
+    extern __shared__ double2 smem2[];
+    __shared__ double red[32];
+    if (done && *done) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double *sm = reinterpret_cast<double *>(smem2) + warp * TILE * ROW_PAD;
+    const double cx = coef[0], cy = coef[1];
+    const int64_t nTiles = (A.m + TILE - 1) / TILE;
+    const double *xAtt = x + A.offAtt, *xIns = x + A.offInstr;
+    const double xg = __ldg(x + A.offGlob);
+    double sq = 0.0;
+    for (int64_t tile = int64_t(blockIdx.x) * WARPS + warp; tile < nTiles;
+         tile += int64_t(gridDim.x) * WARPS) {
+        const int64_t r0 = tile * TILE;
+        const int nrows = int(min(int64_t(TILE), A.m - r0));
+        stage_tile(sm, A.V + r0 * N_PAR, nrows, lane);
+        __syncwarp();
+        if (lane < nrows) {
+            const int64_t i = r0 + lane;
+            double v[N_PAR];
+            read_row(sm, lane, v);
+            const double *xa = x + A.ia[i];
+            const double *xt = xAtt + A.iatt[i];
+            const int2 *icp = reinterpret_cast<const int2 *>(A.ic) + i * 3;
+            const int2 c0 = __ldcs(icp), c1 = __ldcs(icp + 1), c2 = __ldcs(icp + 2);
+            double sum = 0.0;
+#pragma unroll
+            for (int k = 0; k < N_ASTRO; ++k) sum = fma(v[k], __ldg(xa + k), sum);
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    sum = fma(v[5 + 4 * a + j], __ldg(xt + a * A.nDof + j), sum);
+            sum = fma(v[17], __ldg(xIns + c0.x), sum);
+            sum = fma(v[18], __ldg(xIns + c0.y), sum);
+            sum = fma(v[19], __ldg(xIns + c1.x), sum);
+            sum = fma(v[20], __ldg(xIns + c1.y), sum);
+            sum = fma(v[21], __ldg(xIns + c2.x), sum);
+            sum = fma(v[22], __ldg(xIns + c2.y), sum);
+            sum = fma(v[23], xg, sum);
+            const double yi = fma(cy, y[i], cx * sum);
+            y[i] = yi;
+            sq = fma(yi, yi, sq);
+        }
+        __syncwarp();
+    }
+    const double b = block_sum(sq, red);
+    if (threadIdx.x == 0 && sqPartial) sqPartial[blockIdx.x] = b;
+}
+
+// ---------------------------------------------------------------------------------------
+// aprod mode 2 (Eq. 3; Algorithm 3):  x <- cx*x + cy*(A^T y), one pass over A.
+//   astro (Alg. 3 c.1-9; the paper uses atomicAdd): rows are sorted by star,
+//     so each warp tile does a segmented inclusive scan over its 32 rows; a star whose rows lie
+//     inside the tile is stored directly (single writer, no atomics); a star cut by a tile edge
+//     leaves its partial in carryFirst/carryLast[tile] and k_astro_fixup adds the partials in
+//     tile order -> bit-reproducible.
+//   attitude and instrumental: RED.ADD.F64 to x, whose
+//     att/instr/glob sections were pre-scaled by cx (k_scale).
+//   gamma ("globSum1/globSum2"): warp -> CTA partial in fixed order, finished
+//     by k_astro_fixup's extra block.
+// SQUARE: terms are V^2 (y == 1): the column sums of squares of the preconditioner.
+// coef = {cx, cy} in device memory.
+// ---------------------------------------------------------------------------------------
+template <bool SQUARE>
+__global__ void __launch_bounds__(THREADS, 2)
+k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
+         const double *__restrict__ coef, double *__restrict__ carryFirst,
+         double *__restrict__ carryLast, double *__restrict__ globPartial, const int *done)
+{
+    extern __shared__ double2 smem2[];
+    __shared__ double red[32];
+    if (done && *done) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double *sm = reinterpret_cast<double *>(smem2) + warp * TILE * ROW_PAD;
+    const double cx = coef[0], cy = coef[1];
+    const int64_t nTiles = (A.m + TILE - 1) / TILE;
+    double *xAtt = x + A.offAtt, *xIns = x + A.offInstr;
+    double gsum = 0.0;
+    for (int64_t tile = int64_t(blockIdx.x) * WARPS + warp; tile < nTiles;
+         tile += int64_t(gridDim.x) * WARPS) {
+        const int64_t r0 = tile * TILE;
+        const int nrows = int(min(int64_t(TILE), A.m - r0));
+        stage_tile(sm, A.V + r0 * N_PAR, nrows, lane);
+        __syncwarp();
+        const bool valid = lane < nrows;
+        const int64_t i = r0 + (valid ? lane : nrows - 1);
+        double v[N_PAR];
+        read_row(sm, valid ? lane : nrows - 1, v);
+        const int64_t ia = A.ia[i];
+        double yv = 0.0;
+        if (valid) yv = SQUARE ? 1.0 : cy * y[i];
+#pragma unroll
+        for (int k = 0; k < N_PAR; ++k) v[k] = SQUARE ? v[k] * v[k] * yv : v[k] * yv;
+
+        // ---- attitude + instrumental scatter (valid lanes only; invalid lanes hold zeros)
+        if (valid) {
+            double *xt = xAtt + A.iatt[i];
+            const int2 *icp = reinterpret_cast<const int2 *>(A.ic) + i * 3;
+            const int2 c0 = __ldcs(icp), c1 = __ldcs(icp + 1), c2 = __ldcs(icp + 2);
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) atomicAdd(xt + a * A.nDof + j, v[5 + 4 * a + j]);
+            atomicAdd(xIns + c0.x, v[17]);
+            atomicAdd(xIns + c0.y, v[18]);
+            atomicAdd(xIns + c1.x, v[19]);
+            atomicAdd(xIns + c1.y, v[20]);
+            atomicAdd(xIns + c2.x, v[21]);
+            atomicAdd(xIns + c2.y, v[22]);
+        }
+        // ---- gamma: fixed-order warp sum, accumulated per warp over its tiles
+        gsum += warp_sum(v[23]);
+
+        // ---- astro: segmented scan by star over the tile's rows
+        const int64_t iaPrev = __shfl_up_sync(0xffffffffu, ia, 1);
+        const int64_t iaNext = __shfl_down_sync(0xffffffffu, ia, 1);
+        const bool head = (lane == 0) || (ia != iaPrev);
+        const bool tail = valid && ((lane == nrows - 1) || (ia != iaNext));
+        const unsigned heads = __ballot_sync(0xffffffffu, head);
+        const int segStart = 31 - __clz(heads & (0xffffffffu >> (31 - lane)));
+        const int dist = lane - segStart;
+        double s[N_ASTRO];
+#pragma unroll
+        for (int k = 0; k < N_ASTRO; ++k) s[k] = v[k];
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+#pragma unroll
+            for (int k = 0; k < N_ASTRO; ++k) {
+                const double t = __shfl_up_sync(0xffffffffu, s[k], d);
+                if (dist >= d) s[k] += t;
+            }
+        }
+        if (tail) {
+            bool cut = false;
+            if (segStart == 0 && r0 > 0) cut = (A.ia[r0 - 1] == ia);
+            if (lane == nrows - 1 && r0 + nrows < A.m) cut = cut || (A.ia[r0 + nrows] == ia);
+            if (!cut) {
+                double *xa = x + ia;
+#pragma unroll
+                for (int k = 0; k < N_ASTRO; ++k) xa[k] = fma(cx, xa[k], s[k]);
+            } else {
+                double *c = (segStart == 0 ? carryFirst : carryLast) + tile * N_ASTRO;
+#pragma unroll
+                for (int k = 0; k < N_ASTRO; ++k) c[k] = s[k];
+            }
+        }
+        __syncwarp();
+    }
+    // CTA partial of gamma in fixed order (lane 0 of each warp holds its running sum)
+    __syncthreads();
+    if (lane == 0) red[warp] = gsum;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double g = 0.0;
+        for (int w = 0; w < WARPS; ++w) g += red[w];
+        globPartial[blockIdx.x] = g;
+    }
+}
+
+// Finishes the astro section (stars cut by tile edges, stars without rows) and gamma.
+// One thread per star; the last block sums the gamma partials.  Deterministic.
+__global__ void __launch_bounds__(256)
+k_astro_fixup(MatView A, double *__restrict__ x, const double *__restrict__ coef,
+              const double *__restrict__ carryFirst, const double *__restrict__ carryLast,
+              const double *__restrict__ globPartial, int nGlobPartial, const int *done)
+{
+    __shared__ double red[32];
+    if (done && *done) return;
+    const double cx = coef[0];
+    if (blockIdx.x == gridDim.x - 1) {
+        double g = 0.0;
+        for (int p = threadIdx.x; p < nGlobPartial; p += blockDim.x) g += globPartial[p];
+        g = block_sum(g, red);
+        if (threadIdx.x == 0) x[A.offGlob] += g;   // section already scaled by cx
+        return;
+    }
+    const int64_t s = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (s >= A.nStars) return;
+    const int64_t r0 = A.rp[s], r1 = A.rp[s + 1];
+    double *xa = x + s * N_ASTRO;
+    if (r0 == r1) {
+#pragma unroll
+        for (int k = 0; k < N_ASTRO; ++k) xa[k] *= cx;
+        return;
+    }
+    const int64_t t0 = r0 / TILE, t1 = (r1 - 1) / TILE;
+    if (t0 == t1) return;   // stored by k_aprod2
+    double acc[N_ASTRO] = {0, 0, 0, 0, 0};
+    for (int64_t t = t0; t <= t1; ++t) {
+        const double *c = ((t == t0 && r0 != t * TILE) ? carryLast : carryFirst) + t * N_ASTRO;
+#pragma unroll
+        for (int k = 0; k < N_ASTRO; ++k) acc[k] += c[k];
+    }
+#pragma unroll
+    for (int k = 0; k < N_ASTRO; ++k) xa[k] = fma(cx, xa[k], acc[k]);
+}
+
+// x[lo..hi) *= coef[0]  (att + instr + gamma sections before the scatter of aprod2)
+__global__ void k_scale(double *__restrict__ x, int64_t lo, int64_t hi,
+                        const double *__restrict__ coef, const int *done)
+{
+    if (done && *done) return;
+    const double c = coef[0];
+    for (int64_t j = lo + int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < hi;
+         j += int64_t(gridDim.x) * blockDim.x)
+        x[j] *= c;
+}
+
+// ---------------------------------------------------------------------------------------
+// Constraint rows ("Constraints kernels"): CSR tail below the
+// observation rows.  aprod1: one warp per row; aprod2: one thread per non-zero (RED).
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_con_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
+             const double *__restrict__ coef, double *__restrict__ sqPartial, const int *done)
+{
+    __shared__ double red[32];
+    if (done && *done) return;
+    const int lane = threadIdx.x & 31;
+    const double cx = coef[0], cy = coef[1];
+    double sq = 0.0;
+    for (int64_t r = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) >> 5; r < A.nCon;
+         r += (int64_t(gridDim.x) * blockDim.x) >> 5) {
+        double sum = 0.0;
+        for (int64_t q = A.conRp[r] + lane; q < A.conRp[r + 1]; q += 32)
+            sum = fma(A.conVal[q], __ldg(x + A.conCol[q]), sum);
+        sum = warp_sum(sum);
+        if (lane == 0) {
+            const double yi = fma(cy, y[A.m + r], cx * sum);
+            y[A.m + r] = yi;
+            sq = fma(yi, yi, sq);
+        }
+    }
+    const double b = block_sum(sq, red);
+    if (threadIdx.x == 0 && sqPartial) sqPartial[blockIdx.x] = b;
+}
+
+template <bool SQUARE>
+__global__ void __launch_bounds__(256)
+k_con_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
+             const double *__restrict__ coef, const int *done)
+{
+    if (done && *done) return;
+    const double cy = coef[1];
+    const int lane = threadIdx.x & 31;
+    for (int64_t r = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) >> 5; r < A.nCon;
+         r += (int64_t(gridDim.x) * blockDim.x) >> 5) {
+        const double yv = SQUARE ? 1.0 : cy * y[A.m + r];
+        for (int64_t q = A.conRp[r] + lane; q < A.conRp[r + 1]; q += 32) {
+            const double v = A.conVal[q];
+            atomicAdd(x + A.conCol[q], SQUARE ? v * v : v * yv);
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// LSQR vector kernels (not described as ported in the paper).
+// ---------------------------------------------------------------------------------------
+// partial[b] = sum over this CTA's grid-stride elements of a[j]^2 (Eq. 4 norm, PAPER.md:226,
+// in its unscaled form; fixed summation order for a fixed grid).
+__global__ void __launch_bounds__(256)
+k_sumsq(const double *__restrict__ a, int64_t n, double *__restrict__ partial, const int *done)
+{
+    __shared__ double red[32];
+    if (done && *done) return;
+    double s = 0.0;
+    for (int64_t j = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < n;
+         j += int64_t(gridDim.x) * blockDim.x) {
+        const double t = a[j];
+        s = fma(t, t, s);
+    }
+    s = block_sum(s, red);
+    if (threadIdx.x == 0) partial[blockIdx.x] = s;
+}
+
+// Step 4 of LSQR: dk = w/rho; x += t1*w; w = v + t2*w; var += dk^2;
+// ddnorm += |dk|^2, with v = v^ * inv_alpha (lazy normalisation of v).
+__global__ void __launch_bounds__(256)
+k_update(double *__restrict__ x, double *__restrict__ w, const double *__restrict__ vhat,
+         double *__restrict__ var, int64_t n, const Scalars *__restrict__ S,
+         double *__restrict__ ddPartial)
+{
+    __shared__ double red[32];
+    if (S->done) return;
+    const double t1 = S->t1, t2 = S->t2, ir = S->inv_rho, ia = S->inv_alpha;
+    double dd = 0.0;
+    for (int64_t j = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < n;
+         j += int64_t(gridDim.x) * blockDim.x) {
+        const double wj = w[j];
+        const double dk = wj * ir;
+        x[j] = fma(t1, wj, x[j]);
+        w[j] = fma(t2, wj, vhat[j] * ia);
+        var[j] = fma(dk, dk, var[j]);
+        dd = fma(dk, dk, dd);
+    }
+    dd = block_sum(dd, red);
+    if (threadIdx.x == 0) ddPartial[blockIdx.x] = dd;
+}
+
+// w = v^ * inv_alpha (start of LSQR: w = v)
+__global__ void k_init_w(double *__restrict__ w, const double *__restrict__ vhat, int64_t n,
+                         const Scalars *__restrict__ S)
+{
+    const double ia = S->inv_alpha;
+    for (int64_t j = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < n;
+         j += int64_t(gridDim.x) * blockDim.x)
+        w[j] = vhat[j] * ia;
+}
+
+// Alg. 1 l.27: x = p (.) z, se = p (.) sqrt(var) * rnorm / sqrt(m - n).
+__global__ void k_finish(const double *__restrict__ z, const double *__restrict__ var,
+                         const double *__restrict__ p, double *__restrict__ xOut,
+                         double *__restrict__ seOut, int64_t n, int64_t mTot,
+                         const Scalars *__restrict__ S)
+{
+    double s = S->rnorm;
+    if (mTot > n) s = s / sqrt(double(mTot - n));
+    for (int64_t j = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < n;
+         j += int64_t(gridDim.x) * blockDim.x) {
+        xOut[j] = p[j] * z[j];
+        if (seOut) seOut[j] = p[j] * (sqrt(var[j]) * s);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// Scalar recurrences and stop tests (Paige & Saunders 1982, cited
+// PAPER.md:34, 742-743), one CTA; the partial sums are reduced in a fixed order first.
+// ---------------------------------------------------------------------------------------
+__device__ __forceinline__ double reduce_partials(const double *p, int n, double *red)
+{
+    double s = 0.0;
+    for (int j = threadIdx.x; j < n; j += blockDim.x) s += p[j];
+    s = block_sum(s, red);
+    __shared__ double bc;
+    if (threadIdx.x == 0) bc = s;
+    __syncthreads();
+    return bc;
+}
+
+enum { PH_INIT_BETA = 0, PH_INIT_ALPHA = 1, PH_AFTER_APROD1 = 2, PH_AFTER_APROD2 = 3, PH_AFTER_UPDATE = 4 };
+
+__global__ void __launch_bounds__(256)
+k_scalar(int phase, Scalars *S, const double *partial, int nPartial, double *trace, int traceCap)
+{
+    __shared__ double red[32];
+    if (phase >= PH_AFTER_APROD1 && S->done) return;
+    const double sum = reduce_partials(partial, nPartial, red);
+    if (threadIdx.x != 0) return;
+    if (phase == PH_INIT_BETA) {
+        // step 1: beta = |b|, u = b/beta (lazy: u^ = b, scale kept in beta)
+        const double beta = sqrt(sum);
+        S->beta = beta; S->bnorm = beta; S->rnorm = beta; S->phibar = beta;
+        S->a2_cx = 1.0; S->a2_cy = beta > 0.0 ? 1.0 / beta : 0.0;
+        S->anorm = 0; S->acond = 0; S->ddnorm = 0; S->xxnorm = 0; S->xnorm = 0; S->z = 0;
+        S->cs2 = -1.0; S->sn2 = 0.0; S->arnorm = 0; S->itn = 0; S->istop = 0; S->done = 0;
+        S->alpha = 0;
+    } else if (phase == PH_INIT_ALPHA) {
+        // v = A^T u, alpha = |v|, v /= alpha (lazy), w = v
+        const double alpha = sqrt(sum);
+        S->alpha = alpha; S->rhobar = alpha;
+        S->inv_alpha = alpha > 0.0 ? 1.0 / alpha : 0.0;
+        S->arnorm = alpha * S->beta;
+        if (S->arnorm == 0.0) S->done = 1;         // x = 0 is the solution: istop 0, itn 0
+        if (S->itnlim <= 0) S->done = 1;
+        S->a1_cx = S->inv_alpha;
+        S->a1_cy = S->beta > 0.0 ? -alpha / S->beta : 0.0;
+    } else if (phase == PH_AFTER_APROD1) {
+        // step 2 first half: beta = |A v - alpha u|, anorm; coefficients of v <- A^T u - beta v
+        const double beta = sqrt(sum), alpha = S->alpha;
+        S->beta = beta;
+        if (beta > 0.0) {
+            S->anorm = sqrt(S->anorm * S->anorm + alpha * alpha + beta * beta);
+            S->a2_cy = 1.0 / beta;
+            S->a2_cx = -beta * S->inv_alpha;       // v = v^/alpha
+        } else {
+            S->a2_cy = 0.0; S->a2_cx = 1.0;
+        }
+    } else if (phase == PH_AFTER_APROD2) {
+        // step 2 second half + step 3 (plane rotation) + coefficients of step 4
+        const double beta = S->beta;
+        double alpha = sqrt(sum);
+        if (!(beta > 0.0)) alpha = S->alpha;       // aprod2 was skipped: v, alpha unchanged
+        S->alpha = alpha;
+        S->inv_alpha = alpha > 0.0 ? 1.0 / alpha : 0.0;
+        const double rhobar = S->rhobar, phibar = S->phibar;
+        const double rho = sqrt(rhobar * rhobar + beta * beta);
+        const double cs = rhobar / rho, sn = beta / rho;
+        const double theta = sn * alpha;
+        S->rhobar = -cs * alpha;
+        const double phi = cs * phibar;
+        S->phibar = sn * phibar;
+        const double tau = sn * phi;
+        S->t1 = phi / rho; S->t2 = -theta / rho; S->inv_rho = 1.0 / rho;
+        // step 5: norm of x
+        const double delta = S->sn2 * rho, gambar = -S->cs2 * rho;
+        const double rhs = phi - delta * S->z;
+        const double zbar = rhs / gambar;
+        S->xnorm = sqrt(S->xxnorm + zbar * zbar);
+        const double gamma = sqrt(gambar * gambar + theta * theta);
+        S->cs2 = gambar / gamma; S->sn2 = theta / gamma;
+        S->z = rhs / gamma;
+        S->xxnorm = S->xxnorm + S->z * S->z;
+        S->rnorm = S->phibar;
+        S->arnorm = alpha * fabs(tau);
+    } else {  // PH_AFTER_UPDATE: steps 6-7
+        S->ddnorm = S->ddnorm + sum;
+        S->itn = S->itn + 1;
+        const double anorm = S->anorm, rnorm = S->rnorm, arnorm = S->arnorm, xnorm = S->xnorm;
+        const double bnorm = S->bnorm;
+        S->acond = anorm * sqrt(S->ddnorm);
+        if (trace) {
+            double *t = trace + 5 * ((S->itn - 1) % traceCap);
+            t[0] = rnorm; t[1] = arnorm; t[2] = anorm; t[3] = S->acond; t[4] = xnorm;
+        }
+        const double test1 = rnorm / bnorm;
+        const double test2 = (anorm * rnorm != 0.0) ? arnorm / (anorm * rnorm) : 0.0;
+        const double test3 = 1.0 / S->acond;
+        const double t1p = test1 / (1.0 + anorm * xnorm / bnorm);
+        const double rtol = S->btol + S->atol * anorm * xnorm / bnorm;
+        int istop = 0;
+        if (S->itn >= S->itnlim) istop = 7;
+        if (1.0 + test3 <= 1.0) istop = 6;
+        if (1.0 + test2 <= 1.0) istop = 5;
+        if (1.0 + t1p <= 1.0) istop = 4;
+        if (test3 <= S->ctol) istop = 3;
+        if (test2 <= S->atol) istop = 2;
+        if (test1 <= rtol) istop = 1;
+        S->istop = istop;
+        if (istop) S->done = 1;
+        // coefficients of the next aprod1:  u^ <- (1/alpha) A v^ - (alpha/beta) u^
+        S->a1_cx = S->inv_alpha;
+        S->a1_cy = S->beta > 0.0 ? -S->alpha / S->beta : 0.0;
+    }
+}
+
+// ---------------------------------------------------------------------------------------
+// Setup kernels: validation, star row pointer, preconditioner.
+// ---------------------------------------------------------------------------------------
+__global__ void k_validate(MatView A, unsigned long long *badRow)
+{
+    for (int64_t i = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; i < A.m;
+         i += int64_t(gridDim.x) * blockDim.x) {
+        const int64_t ia = A.ia[i], s = A.iatt[i];
+        bool bad = ia < 0 || ia > 5 * (A.nStars - 1) || (ia % 5) != 0;
+        if (i > 0) bad = bad || A.ia[i - 1] > ia;
+        bad = bad || s < 0 || s > A.nDof - 4;
+#pragma unroll
+        for (int j = 0; j < N_INSTR; ++j) {
+            const int32_t c = A.ic[i * N_INSTR + j];
+            bad = bad || c < 0 || c >= A.nInstr;
+        }
+        if (bad) atomicMin(badRow, (unsigned long long)i);
+    }
+}
+
+// rp[s] = first row i with ia[i] >= 5*s  (rows sorted by star), s = 0..nStars
+__global__ void k_star_rowptr(const int64_t *__restrict__ ia, int64_t m, int64_t nStars,
+                              int64_t *__restrict__ rp)
+{
+    const int64_t s = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (s > nStars) return;
+    const int64_t key = 5 * s;
+    int64_t lo = 0, hi = m;
+    while (lo < hi) {
+        const int64_t mid = (lo + hi) >> 1;
+        if (ia[mid] < key) lo = mid + 1; else hi = mid;
+    }
+    rp[s] = lo;
+}
+
+__global__ void k_validate_con(MatView A, int64_t nnz, unsigned long long *badRow)
+{
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < nnz;
+         q += int64_t(gridDim.x) * blockDim.x) {
+        const int64_t c = A.conCol[q];
+        if (c < 0 || c >= A.n) atomicMin(badRow, (unsigned long long)q);
+    }
+    for (int64_t r = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; r <= A.nCon;
+         r += int64_t(gridDim.x) * blockDim.x) {
+        const int64_t a = A.conRp[r];
+        bool bad = a < 0 || a > nnz || (r == 0 && a != 0) || (r == A.nCon && a != nnz);
+        if (r > 0) bad = bad || A.conRp[r - 1] > a;
+        if (bad) atomicMin(badRow, (unsigned long long)r);
+    }
+}
+
+// p_j = 1/sqrt(colsq_j), or 1 for an empty column (readings R1-R2)
+__global__ void k_colscale(double *__restrict__ p, int64_t n)
+{
+    for (int64_t j = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < n;
+         j += int64_t(gridDim.x) * blockDim.x) {
+        const double s = p[j];
+        p[j] = s > 0.0 ? 1.0 / sqrt(s) : 1.0;
+    }
+}
+
+// A_ij <- fl(A_ij * p_j) in place ("Normalization of A by p", Alg. 1 l.3).
+// One thread per stored coefficient (coalesced over A_d).
+__global__ void k_scale_values(MatView A, const double *__restrict__ p)
+{
+    const int64_t total = A.m * N_PAR;
+    for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < total;
+         e += int64_t(gridDim.x) * blockDim.x) {
+        const int64_t i = e / N_PAR;
+        const int k = int(e - i * N_PAR);
+        int64_t c;
+        if (k < N_ASTRO) c = A.ia[i] + k;
+        else if (k < N_ASTRO + N_ATT) c = A.offAtt + ((k - N_ASTRO) >> 2) * A.nDof + A.iatt[i] + ((k - N_ASTRO) & 3);
+        else if (k < N_PAR - 1) c = A.offInstr + A.ic[i * N_INSTR + (k - N_ASTRO - N_ATT)];
+        else c = A.offGlob;
+        A.V[e] = A.V[e] * p[c];
+    }
+}
+
+__global__ void k_scale_con_values(MatView A, int64_t nnz, const double *__restrict__ p)
+{
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < nnz;
+         q += int64_t(gridDim.x) * blockDim.x)
+        A.conVal[q] = A.conVal[q] * p[A.conCol[q]];
+}
+
+__global__ void k_fill(double *__restrict__ a, int64_t n, double v)
+{
+    for (int64_t j = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < n;
+         j += int64_t(gridDim.x) * blockDim.x)
+        a[j] = v;
+}
+
+}  // namespace gsr
