@@ -442,7 +442,7 @@ int32_t gsr_precondition(gsr_handle *h)
 
 int32_t gsr_aprod1(gsr_handle *h, const double *x, double *y)
 {
-    if (!h || !x || !y) return GSR_EINVAL;
+    if (!h || !x || (!y && h->mTot > 0)) return GSR_EINVAL;
     int rc = readyCheck(h);
     if (rc) return rc;
     rc = enter(h);
@@ -455,7 +455,7 @@ int32_t gsr_aprod1(gsr_handle *h, const double *x, double *y)
 
 int32_t gsr_aprod2(gsr_handle *h, const double *y, double *x)
 {
-    if (!h || !x || !y) return GSR_EINVAL;
+    if (!h || !x || (!y && h->mTot > 0)) return GSR_EINVAL;
     int rc = readyCheck(h);
     if (rc) return rc;
     rc = enter(h);

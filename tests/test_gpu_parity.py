@@ -1,0 +1,300 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Tolerances (BASELINE north_star): index/layout arrays bit-exact; every aprod output element within
+1e-12 * sum|terms|; LSQR x after a fixed iteration count within 1e-9 relative L2, same istop,
+itn within +-2.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from helpers import make_b, np_inputs, oracle_system
+from paper_2308_00778_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+APROD_TOL = 1e-12
+X_TOL = 1e-9
+
+
+def gsr_mod():
+    from paper_2308_00778_b200 import gsr
+    return gsr
+
+
+def dev(a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def make_gpu(S, d, b, upload_constraints=True):
+    gsr = gsr_mod()
+    G = gsr.Gsr(S.m, S.n_stars, S.n_dof_att, S.n_instr, S.n_con, len(S.con_col))
+    G.gsr_upload(np.ascontiguousarray(d["values"]), np.ascontiguousarray(d["matrixIndexAstro"]),
+                 np.ascontiguousarray(d["matrixIndexAtt"]), np.ascontiguousarray(d["instrCol"]), b)
+    if S.n_con and upload_constraints:
+        G.gsr_upload_constraints(S.con_rowptr, S.con_col, S.con_val)
+    return G
+
+
+def subset(d, keep):
+    """Keep the rows of a generated system selected by the boolean mask `keep`."""
+    out = dict(d)
+    for k in ("values", "matrixIndexAstro", "matrixIndexAtt", "instrCol", "noise"):
+        out[k] = np.ascontiguousarray(d[k][keep])
+    return out
+
+
+def check_aprods(S, G, seed=0):
+    rng = np.random.default_rng(seed)
+    x = rng.standard_normal(S.n)
+    y = rng.standard_normal(S.m_tot)
+    y1 = G.gsr_aprod1(dev(x), dev(y)).cpu().numpy()
+    y1o, ab = S.aprod1(x, y, want_abs=True)
+    assert np.all(np.abs(y1 - y1o) <= APROD_TOL * ab + 1e-300), np.max(np.abs(y1 - y1o) / (ab + 1e-300))
+    x2 = G.gsr_aprod2(dev(y), dev(x)).cpu().numpy()
+    x2o, ab2 = S.aprod2(y, x, want_abs=True)
+    assert np.all(np.abs(x2 - x2o) <= APROD_TOL * ab2 + 1e-300), np.max(np.abs(x2 - x2o) / (ab2 + 1e-300))
+    return x, y
+
+
+CASES = {
+    "mini": dict(cfg=synth.mini(seed=1)),
+    "mini_con": dict(cfg=synth.mini(seed=2, n_stars=40, obs=9, n_dof_att=30, n_instr=16, n_con=5, con_nnz=20)),
+    "ragged_tail": dict(cfg=synth.mini(seed=3, n_stars=37, obs=23, n_dof_att=64, n_instr=10)),        # 851 rows
+    "one_row_stars": dict(cfg=synth.mini(seed=4, n_stars=300, obs=1, n_dof_att=40, n_instr=9)),       # every tile full of heads
+    "one_star": dict(cfg=synth.mini(seed=5, n_stars=1, obs=1000, n_dof_att=200, n_instr=6)),          # one segment over 32 tiles
+    "tiny_rows": dict(cfg=synth.mini(seed=6, n_stars=3, obs=5, n_dof_att=4, n_instr=6)),              # m < 32, N_DFA = 4
+    "powerlaw": dict(cfg=synth.SynthConfig("pl", 400, 300, 50, obs_powerlaw=(2.0, 1, 200),
+                                           att_bursts=(5, 1e-2, 0.9), instr_zipf=1.1, seed=7)),
+}
+
+
+@pytest.mark.parametrize("name", list(CASES))
+def test_aprod_parity_and_layout(name):
+    cfg = CASES[name]["cfg"]
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    with make_gpu(S, d, b) as G:
+        assert G.n == S.n and G.m_tot == S.m_tot
+        rp = G.gsr_get_star_rowptr().cpu().numpy()
+        assert np.array_equal(rp, d["rowptr"])                                   # generator's own
+        assert np.array_equal(rp, np.searchsorted(S.ia, 5 * np.arange(S.n_stars + 1), side="left"))
+        check_aprods(S, G)
+
+
+def test_stars_without_rows_and_empty_system():
+    cfg = synth.mini(seed=8, n_stars=50, obs=20, n_dof_att=30, n_instr=8)
+    d = np_inputs(cfg)
+    star = d["matrixIndexAstro"] // 5
+    keep = ~np.isin(star, [0, 7, 8, 9, 30, 49])      # first, a run, one in the middle, last
+    ds = subset(d, keep)
+    S = oracle.OracleSystem(cfg.n_stars, cfg.n_dof_att, cfg.n_instr, ds["values"], ds["matrixIndexAstro"],
+                            ds["matrixIndexAtt"], ds["instrCol"])
+    b = S.aprod1(d["x_true"], ds["noise"])
+    with make_gpu(S, ds, b) as G:
+        rp = G.gsr_get_star_rowptr().cpu().numpy()
+        assert np.array_equal(rp, np.searchsorted(S.ia, 5 * np.arange(S.n_stars + 1), side="left"))
+        check_aprods(S, G)
+        G.gsr_precondition()
+        p = G.gsr_get_colscale().cpu().numpy()
+        po = S.precondition()
+        assert np.all(p[po == 1.0] == 1.0)           # empty columns: p = 1 (reading R2)
+        np.testing.assert_allclose(p, po, rtol=1e-14, atol=0)
+    # m = 0
+    gsr = gsr_mod()
+    e = np.zeros((0, 24))
+    with gsr.Gsr(0, 4, 8, 8) as G:
+        G.gsr_upload(e, np.zeros(0, np.int64), np.zeros(0, np.int64), np.zeros((0, 6), np.int32), np.zeros(0))
+        x = torch.ones(G.n, dtype=torch.float64, device="cuda")
+        y = torch.zeros(0, dtype=torch.float64, device="cuda")
+        G.gsr_aprod2(y, x)
+        assert torch.all(x == 1.0)
+        r = G.gsr_lsqr(5, 0.0, 0.0)
+        assert r.istop == 0 and r.itn == 0 and torch.all(r.x == 0)
+
+
+def test_tiny_config_aprod_parity():
+    cfg = synth.tiny()
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    with make_gpu(S, d, b) as G:
+        check_aprods(S, G)
+
+
+def test_astro_and_gamma_are_bit_reproducible():
+    cfg = synth.tiny()
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    rng = np.random.default_rng(5)
+    y = dev(rng.standard_normal(S.m))
+    with make_gpu(S, d, b) as G:
+        outs = []
+        for _ in range(3):
+            x = torch.zeros(S.n, dtype=torch.float64, device="cuda")
+            outs.append(G.gsr_aprod2(y, x).cpu().numpy())
+        na = 5 * cfg.n_stars
+        for o in outs[1:]:
+            assert np.array_equal(o[:na], outs[0][:na])
+            assert o[-1] == outs[0][-1]
+
+
+@pytest.mark.parametrize("name", ["mini_con", "ragged_tail", "powerlaw"])
+def test_precondition_parity(name):
+    cfg = CASES[name]["cfg"]
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    with make_gpu(S, d, b) as G:
+        G.gsr_precondition()
+        p = G.gsr_get_colscale().cpu().numpy()
+        po = S.precondition()
+        np.testing.assert_allclose(p, po, rtol=1e-14, atol=0)
+        V, cv = G.gsr_get_values()
+        # A' = fl(A * p): with p equal to ~1 ulp the stored values agree to a few ulp
+        np.testing.assert_allclose(V.cpu().numpy(), S.V, rtol=4e-15, atol=0)
+        if S.n_con:
+            np.testing.assert_allclose(cv.cpu().numpy(), S.con_val, rtol=4e-15, atol=0)
+        with pytest.raises(gsr_mod().GsrError) as e:
+            G.gsr_precondition()
+        assert e.value.code == gsr_mod().GSR_ESTATE
+        check_aprods_scaled(S, G)
+
+
+def check_aprods_scaled(S, G):
+    """aprods on the preconditioned matrices: the two stored matrices differ by rounding of p,
+    so the bound gets the 4e-15 relative slack of the stored values on top of 1e-12."""
+    rng = np.random.default_rng(1)
+    x = rng.standard_normal(S.n)
+    y = rng.standard_normal(S.m_tot)
+    y1 = G.gsr_aprod1(dev(x), dev(y)).cpu().numpy()
+    y1o, ab = S.aprod1(x, y, want_abs=True)
+    assert np.all(np.abs(y1 - y1o) <= (APROD_TOL + 4e-15) * ab)
+    x2 = G.gsr_aprod2(dev(y), dev(x)).cpu().numpy()
+    x2o, ab2 = S.aprod2(y, x, want_abs=True)
+    assert np.all(np.abs(x2 - x2o) <= (APROD_TOL + 4e-15) * ab2)
+
+
+def lsqr_both(cfg, itnlim, atol, btol, conlim=0.0, precond=True, noise=True):
+    S, d = oracle_system(cfg)
+    if not noise:
+        d["noise"] = np.zeros_like(d["noise"])
+    b = make_b(S, d)
+    G = make_gpu(S, d, b)
+    if precond:
+        G.gsr_precondition()
+        S.precondition()
+    r = G.gsr_lsqr(itnlim, atol, btol, conlim)
+    ro = S.lsqr(b, itnlim, atol, btol, conlim, want_trace=True)
+    return S, d, G, r, ro
+
+
+def rel(a, b):
+    return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
+
+
+@pytest.mark.parametrize("name,itn", [("mini", 30), ("mini_con", 25), ("ragged_tail", 40), ("powerlaw", 40)])
+def test_lsqr_fixed_iterations_small(name, itn):
+    S, d, G, r, ro = lsqr_both(CASES[name]["cfg"], itn, 0.0, 0.0)
+    with G:
+        assert (r.istop, r.itn) == (ro.istop, ro.itn) == (7, itn)
+        assert rel(r.x.cpu().numpy(), ro.x) <= X_TOL
+        assert rel(r.se.cpu().numpy(), ro.se) <= 1e-8
+        for a, bb in ((r.rnorm, ro.rnorm), (r.anorm, ro.anorm), (r.acond, ro.acond), (r.xnorm, ro.xnorm)):
+            assert abs(a - bb) <= 1e-9 * abs(bb)
+        assert abs(r.arnorm - ro.arnorm) <= 1e-9 * ro.anorm * ro.rnorm + 1e-9 * abs(ro.arnorm)
+        tr = G.gsr_get_trace()
+        assert tr.shape == (itn, 5)
+        np.testing.assert_allclose(tr[:, 0], ro.trace[:, 0], rtol=1e-9)
+        np.testing.assert_allclose(tr[:, 2], ro.trace[:, 2], rtol=1e-9)
+
+
+def test_lsqr_tiny_config_100_iterations():
+    """BASELINE configs[0]: 100 iterations on the preconditioned Tiny system."""
+    S, d, G, r, ro = lsqr_both(synth.tiny(), 100, 0.0, 0.0)
+    with G:
+        assert (r.istop, r.itn) == (ro.istop, ro.itn) == (7, 100)
+        assert rel(r.x.cpu().numpy(), ro.x) <= X_TOL
+        assert rel(r.se.cpu().numpy(), ro.se) <= 1e-8
+        assert rel(r.x.cpu().numpy(), d["x_true"]) <= 1e-2
+
+
+def test_lsqr_stop_tests_match():
+    # atol = btol = 1e-14 (BASELINE Tiny): same istop, itn within +-2
+    S, d, G, r, ro = lsqr_both(synth.tiny(), 400, 1e-14, 1e-14)
+    with G:
+        assert r.istop == ro.istop and r.istop != 7
+        assert abs(r.itn - ro.itn) <= 2, (r.itn, ro.itn)
+        assert rel(r.x.cpu().numpy(), ro.x) <= 1e-8
+    # loose tolerances stop early on test 2; conlim test 3; consistent system test 1
+    for kw in (dict(atol=1e-6, btol=1e-6), dict(atol=0.0, btol=0.0, conlim=5.0),
+               dict(atol=1e-10, btol=1e-10, noise=False)):
+        noise = kw.pop("noise", True)
+        S, d, G, r, ro = lsqr_both(CASES["ragged_tail"]["cfg"], 300, kw.get("atol"), kw.get("btol"),
+                                   kw.get("conlim", 0.0), noise=noise)
+        with G:
+            assert r.istop == ro.istop and r.istop in (1, 2, 3), (kw, r.istop, ro.istop)
+            assert abs(r.itn - ro.itn) <= 2
+
+
+def test_lsqr_unpreconditioned_and_host_output():
+    cfg = CASES["mini"]["cfg"]
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    with make_gpu(S, d, b) as G:
+        r = G.gsr_lsqr(20, 0.0, 0.0, host_out=True)
+        ro = S.lsqr(b, 20, 0.0, 0.0)
+        assert not r.x.is_cuda
+        assert rel(r.x.numpy(), ro.x) <= X_TOL
+        # a second solve on the same handle reuses the captured graph and gives the same answer
+        r2 = G.gsr_lsqr(20, 0.0, 0.0)
+        assert rel(r2.x.cpu().numpy(), ro.x) <= X_TOL
+        assert r2.kernel_launches > 0 and r2.loop_ms > 0
+
+
+def test_b_zero_gives_istop0():
+    cfg = CASES["mini"]["cfg"]
+    S, d = oracle_system(cfg)
+    with make_gpu(S, d, np.zeros(S.m_tot)) as G:
+        r = G.gsr_lsqr(10, 1e-10, 1e-10)
+        assert r.istop == 0 and r.itn == 0 and torch.all(r.x == 0)
+
+
+def test_index_validation():
+    gsr = gsr_mod()
+    cfg = CASES["mini"]["cfg"]
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    for key, row, val in (("matrixIndexAstro", 17, 3), ("matrixIndexAtt", 40, cfg.n_dof_att - 3),
+                          ("instrCol", 100, cfg.n_instr), ("matrixIndexAstro", 5, 5 * cfg.n_stars)):
+        bad = {k: np.array(v, copy=True) for k, v in d.items()}
+        if key == "instrCol":
+            bad[key][row, 2] = val
+        else:
+            bad[key][row] = val
+        G = gsr.Gsr(S.m, S.n_stars, S.n_dof_att, S.n_instr)
+        with G:
+            with pytest.raises(gsr.GsrError) as e:
+                G.gsr_upload(bad["values"], bad["matrixIndexAstro"], bad["matrixIndexAtt"], bad["instrCol"], b)
+            assert e.value.code == gsr.GSR_EINDEX
+            assert G.gsr_bad_row() in (row, row + 1)
+            with pytest.raises(gsr.GsrError) as e2:     # nothing usable was uploaded
+                G.gsr_precondition()
+            assert e2.value.code == gsr.GSR_ESTATE
+    with pytest.raises(gsr.GsrError) as e:
+        gsr.Gsr(10, 2, 3, 8)                             # N_DFA < 4
+    assert e.value.code == gsr.GSR_EINVAL
+
+
+def test_chunked_device_upload_equals_whole_upload():
+    cfg = CASES["ragged_tail"]["cfg"]
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    gsr = gsr_mod()
+    with gsr.Gsr(S.m, S.n_stars, S.n_dof_att, S.n_instr) as G:
+        step = 300
+        for r0 in range(0, S.m, step):
+            r1 = min(r0 + step, S.m)
+            G.gsr_upload_rows(r0, r1 - r0, dev(d["values"][r0:r1]), dev(d["matrixIndexAstro"][r0:r1]),
+                              dev(d["matrixIndexAtt"][r0:r1]), dev(d["instrCol"][r0:r1]), dev(b[r0:r1]))
+        G.gsr_upload_finish()
+        check_aprods(S, G)
