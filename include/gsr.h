@@ -116,6 +116,9 @@ int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double
                         const int32_t *instrCol, const double *b);
 int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail);
 
+/* Replaces the known terms b (n_obs+n_con doubles, host or device) of an uploaded system. */
+int32_t gsr_set_b(gsr_handle *h, const double *b);
+
 /* Constraint rows as CSR with absolute column indices:
  * rowptr i64 [n_con+1], col i64 [n_con_nnz] in [0, n), val f64 [n_con_nnz].
  * Host or device.  Must precede gsr_precondition. */

@@ -267,6 +267,17 @@ int32_t gsr_upload(gsr_handle *h, const double *values, const int64_t *ia, const
     return gsr_upload_finish(h, h->L.n_con > 0 ? b + h->L.n_obs : nullptr);
 }
 
+int32_t gsr_set_b(gsr_handle *h, const double *b)
+{
+    if (!h || (!b && h->mTot > 0)) return GSR_EINVAL;
+    if (!h->uploaded) return fail(h, GSR_ESTATE, "no system uploaded");
+    int rc = enter(h);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(h->b, b, size_t(h->mTot) * sizeof(double), cudaMemcpyDefault, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    return GSR_OK;
+}
+
 int32_t gsr_upload_constraints(gsr_handle *h, const int64_t *rowptr, const int64_t *col, const double *val)
 {
     if (!h) return GSR_EINVAL;

@@ -22,7 +22,7 @@ TRACE_CAP = 4096
 # every symbol include/gsr.h declares (tests check that the library exports each one)
 SYMBOLS = [
     "gsr_create", "gsr_destroy", "gsr_last_error", "gsr_bad_row", "gsr_ncols", "gsr_nrows",
-    "gsr_upload", "gsr_upload_rows", "gsr_upload_finish", "gsr_upload_constraints",
+    "gsr_upload", "gsr_upload_rows", "gsr_upload_finish", "gsr_upload_constraints", "gsr_set_b",
     "gsr_get_star_rowptr", "gsr_precondition", "gsr_get_colscale", "gsr_get_values",
     "gsr_aprod1", "gsr_aprod2", "gsr_lsqr", "gsr_get_trace", "gsr_last_timing", "gsr_time_aprod",
 ]
@@ -71,6 +71,7 @@ def load_library():
         "gsr_upload_rows": (I32, [P, I64, I64, P, P, P, P, P]),
         "gsr_upload_finish": (I32, [P, P]),
         "gsr_upload_constraints": (I32, [P, P, P, P]),
+        "gsr_set_b": (I32, [P, P]),
         "gsr_get_star_rowptr": (I32, [P, P]),
         "gsr_precondition": (I32, [P]),
         "gsr_get_colscale": (I32, [P, P]),
@@ -189,6 +190,9 @@ class Gsr:
     def gsr_upload_constraints(self, rowptr, col, val):
         self._ck(self.lib.gsr_upload_constraints(self._h, _ptr(rowptr, torch.int64, "rowptr"),
                                                  _ptr(col, torch.int64, "col"), _ptr(val, torch.float64, "val")))
+
+    def gsr_set_b(self, b):
+        self._ck(self.lib.gsr_set_b(self._h, _ptr(b, torch.float64, "b")))
 
     def gsr_bad_row(self):
         return int(self.lib.gsr_bad_row(self._h))

@@ -65,7 +65,11 @@ CASES = {
     "one_row_stars": dict(cfg=synth.mini(seed=4, n_stars=300, obs=1, n_dof_att=40, n_instr=9)),       # every tile full of heads
     "one_star": dict(cfg=synth.mini(seed=5, n_stars=1, obs=1000, n_dof_att=200, n_instr=6)),          # one segment over 32 tiles
     "tiny_rows": dict(cfg=synth.mini(seed=6, n_stars=3, obs=5, n_dof_att=4, n_instr=6)),              # m < 32, N_DFA = 4
-    "powerlaw": dict(cfg=synth.SynthConfig("pl", 400, 300, 50, obs_powerlaw=(2.0, 1, 200),
+    # Skewed-like: power-law rows per star, bursty attitude times, Zipf instrument columns.
+    # kmin = 1 (many stars cut to 1-2 rows; rank deficient, aprod parity only) and kmin = 8 (well posed).
+    "powerlaw_short": dict(cfg=synth.SynthConfig("pl1", 400, 300, 50, obs_powerlaw=(2.0, 1, 200),
+                                                 att_bursts=(5, 1e-2, 0.9), instr_zipf=1.1, seed=7)),
+    "powerlaw": dict(cfg=synth.SynthConfig("pl8", 400, 300, 50, obs_powerlaw=(2.0, 8, 200),
                                            att_bursts=(5, 1e-2, 0.9), instr_zipf=1.1, seed=7)),
 }
 
