@@ -93,7 +93,9 @@ int gridFor(int64_t count, int perBlock, int cap)
 int enter(gsr_handle *h)
 {
     CK(cudaSetDevice(h->L.device));
-    if (h->userStream) CK(cudaStreamSynchronize(h->userStream));
+    // work the caller queued (e.g. torch kernels that produced the arguments) must be complete
+    // before the library's own stream touches them; a NULL handle is the legacy default stream
+    CK(cudaStreamSynchronize(h->userStream));
     return GSR_OK;
 }
 
