@@ -218,14 +218,25 @@ def main_ours(args):
     peak, peak_src = peaks()
     ms1 = G.gsr_time_aprod(11, args.kernel_reps)
     ms2 = G.gsr_time_aprod(12, args.kernel_reps)
+    try:
+        ms2a = G.gsr_time_aprod(13, args.kernel_reps)      # time-ordered attitude kernel, if in use
+    except gsr.GsrError:
+        ms2a = None
     ms1g = G.gsr_time_aprod(1, args.kernel_reps)
     ms2g = G.gsr_time_aprod(2, args.kernel_reps)
     gb1 = ROW_BYTES_APROD1 * m / 1e9
     gb2 = (ROW_BYTES_APROD2 * m + 8 * G.n) / 1e9
+    # per-kernel algorithmic bytes: with the attitude section on its own
+    # time-ordered copy the main aprod2 kernel needs 96 B of non-attitude values + 32 B indices + 8 B y
+    # per row, the attitude kernel 96 B values + 4 B start + 4 B permutation + 8 B y
+    gb2_main = (136 * m + 8 * G.n) / 1e9 if ms2a is not None else gb2
     k = {"k_aprod1": {"ms": ms1, "alg_gb": gb1, "gbs": gb1 / (ms1 * 1e-3)},
-         "k_aprod2": {"ms": ms2, "alg_gb": gb2, "gbs": gb2 / (ms2 * 1e-3)},
+         "k_aprod2": {"ms": ms2, "alg_gb": gb2_main, "gbs": gb2_main / (ms2 * 1e-3)},
          "aprod1_group_ms": ms1g, "aprod2_group_ms": ms2g}
-    dom = "k_aprod2" if ms2 >= ms1 else "k_aprod1"
+    if ms2a is not None:
+        gb2a = 112 * m / 1e9
+        k["k_aprod2_att"] = {"ms": ms2a, "alg_gb": gb2a, "gbs": gb2a / (ms2a * 1e-3)}
+    dom = max((n for n in k if n.startswith("k_")), key=lambda n: k[n]["ms"])
     roofline = {"bound": "hbm", "kernel": dom, "achieved": k[dom]["gbs"], "peak": peak, "unit": "GB/s",
                 "frac": k[dom]["gbs"] / peak, "traffic": None, "peak_source": peak_src,
                 "aprod1_plus_aprod2_gbs": (gb1 + gb2) / ((ms1g + ms2g) * 1e-3),

@@ -169,10 +169,12 @@ int32_t gsr_get_trace(gsr_handle *h, double *out, int64_t max_itn, int64_t *n_wr
  * the handle's stream), and the number of kernels launched in it. */
 int32_t gsr_last_timing(gsr_handle *h, double *loop_ms, int64_t *kernel_launches);
 
-/* Timing hooks for bench.py: run `reps` back-to-back launches of the kernel group of
- * one product (which = 1: aprod1 group, 2: aprod2 group) with the LSQR scalars set
- * to 1, on internal u/v work vectors, and return the mean device time per group in
- * milliseconds (CUDA events on the handle's stream). */
+/* Timing hook for bench.py: run `reps` back-to-back launches of one product's kernels with the
+ * LSQR coefficients set to 0.5 (bounded operands) on the internal u/v work vectors, after one
+ * warm-up launch, and return the mean device time per launch in milliseconds (CUDA events on the
+ * handle's stream).  which = 1: whole aprod1 group; 2: whole aprod2 group (pre-scale, attitude
+ * kernel, main kernel, fix-up, constraints); 11: k_aprod1 alone; 12: k_aprod2 (main) alone;
+ * 13: k_aprod2_att alone (GSR_ESTATE if the handle has no time-ordered attitude copy). */
 int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_per_launch);
 
 #ifdef __cplusplus

@@ -5,6 +5,8 @@
 #include "gsr.h"
 #include "gsr_kernels.cuh"
 
+#include <cub/device/device_radix_sort.cuh>
+
 #include <algorithm>
 #include <cstdarg>
 #include <cstdio>
@@ -28,6 +30,12 @@ struct gsr_handle {
     double *carryFirst = nullptr, *carryLast = nullptr, *globPartial = nullptr;
     double *sqPartialU = nullptr, *sqPartialV = nullptr, *ddPartial = nullptr;
     double *coefOne = nullptr, *coefTime = nullptr, *trace = nullptr;
+    // time-ordered attitude copy (aprod2 "bucketed scatter") and instrument replicas
+    double *attT = nullptr, *insRep = nullptr;
+    int32_t *sT = nullptr;
+    uint32_t *permT = nullptr;
+    int nRep = 1, gridAtt = 1, perIter = 0;
+    bool useAttT = false;
     Scalars *S = nullptr;
     Scalars *hostS = nullptr;           // pinned, 2 slots
     unsigned long long *badDev = nullptr;
@@ -81,6 +89,8 @@ MatView view(const gsr_handle *h)
     A.offGlob = A.offInstr + h->L.n_instr;
     A.n = h->n;
     A.conRp = h->conRp; A.conCol = h->conCol; A.conVal = h->conVal; A.nCon = h->L.n_con;
+    A.attT = h->useAttT ? h->attT : nullptr; A.sT = h->sT; A.permT = h->permT;
+    A.insRep = h->insRep; A.nRep = h->nRep;
     return A;
 }
 
@@ -96,6 +106,45 @@ int enter(gsr_handle *h)
     // work the caller queued (e.g. torch kernels that produced the arguments) must be complete
     // before the library's own stream touches them; a NULL handle is the legacy default stream
     CK(cudaStreamSynchronize(h->userStream));
+    return GSR_OK;
+}
+
+// Time order of the attitude section (setup): stable radix sort of the rows by
+// attitude start (cub, a library primitive used once per upload, not on the per-iteration path),
+// then a gather of the 12 attitude coefficients of every row into column-major attT.
+int buildAttT(gsr_handle *h)
+{
+    if (!h->useAttT) return GSR_OK;
+    const int64_t m = h->L.n_obs;
+    MatView A = view(h);
+    int32_t *keyIn = nullptr;
+    uint32_t *valIn = nullptr;
+    void *tmp = nullptr;
+    size_t tmpBytes = 0;
+    int endBit = 1;
+    while (endBit < 31 && (int64_t(1) << endBit) < h->L.n_dof_att) ++endBit;
+    cudaError_t e = cub::DeviceRadixSort::SortPairs(nullptr, tmpBytes, keyIn, h->sT, valIn, h->permT, m, 0,
+                                                    endBit, h->stream);
+    if (e == cudaSuccess) e = dalloc(&keyIn, m);
+    if (e == cudaSuccess) e = dalloc(&valIn, m);
+    if (e == cudaSuccess) e = cudaMalloc(&tmp, std::max<size_t>(tmpBytes, 16));
+    if (e == cudaSuccess) {
+        k_sort_keys<<<gridFor(m, 256, h->smCount * 16), 256, 0, h->stream>>>(h->iatt, m, keyIn, valIn);
+        e = cub::DeviceRadixSort::SortPairs(tmp, tmpBytes, keyIn, h->sT, valIn, h->permT, m, 0, endBit, h->stream);
+    }
+    if (e == cudaSuccess) {
+        k_gather_att<<<gridFor(m, 256, h->smCount * 16), 256, 0, h->stream>>>(A);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (keyIn) cudaFree(keyIn);
+    if (valIn) cudaFree(valIn);
+    if (tmp) cudaFree(tmp);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        return fail(h, e == cudaErrorMemoryAllocation ? GSR_ENOMEM : GSR_ECUDA, "time-ordered attitude copy: %s",
+                    cudaGetErrorString(e));
+    }
     return GSR_OK;
 }
 
@@ -135,16 +184,21 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(cudaEventCreateWithFlags(&h->evSlot[1], cudaEventDisableTiming));
 
     CK(cudaFuncSetAttribute(k_aprod1, cudaFuncAttributeMaxDynamicSharedMemorySize, int(APROD_SMEM)));
-    CK(cudaFuncSetAttribute(k_aprod2<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(APROD_SMEM)));
-    CK(cudaFuncSetAttribute(k_aprod2<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(APROD_SMEM)));
+    CK(cudaFuncSetAttribute(k_aprod2<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(APROD_SMEM)));
+    CK(cudaFuncSetAttribute(k_aprod2<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(APROD_SMEM)));
+    CK(cudaFuncSetAttribute(k_aprod2<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(APROD_SMEM)));
     int occ1 = 1, occ2 = 1;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, k_aprod1, THREADS, APROD_SMEM));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, k_aprod2<false>, THREADS, APROD_SMEM));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, k_aprod2<false, true>, THREADS, APROD_SMEM));
     h->gridA1 = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ1, 1));
     h->gridA2 = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ2, 1));
     h->gridVec = gridFor(std::max(h->n, h->mTot), 256 * 4, h->smCount * 8);
     h->gridCon = gridFor(L->n_con, 8, h->smCount * 8);
-    h->gridFix = int((L->n_stars + 255) / 256) + 1;
+    // fix-up grid: one thread per star, then one per instrument column (replica fold), then gamma
+    h->gridFix = int((L->n_stars + 255) / 256) + int((L->n_instr + 255) / 256) + 1;
+    h->gridAtt = gridFor(h->nTiles, 8, h->smCount * 8);
+    // instrument replicas: spread the REDs of aprod2 over >= ~512k distinct addresses
+    h->nRep = int(std::max<int64_t>(1, std::min<int64_t>(128, (524288 + L->n_instr - 1) / L->n_instr)));
 
     const int64_t m = L->n_obs;
     CK(dalloc(&h->V, m * N_PAR));
@@ -168,6 +222,32 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(dalloc(&h->trace, 5 * GSR_TRACE_CAP));
     CK(dalloc(&h->S, 1));
     CK(dalloc(&h->badDev, 1));
+    CK(dalloc(&h->insRep, int64_t(h->nRep) * L->n_instr));
+    CK(dalloc(&h->u, h->mTot));
+    CK(dalloc(&h->v, h->n));
+    CK(dalloc(&h->w, h->n));
+    CK(dalloc(&h->z, h->n));
+    CK(dalloc(&h->var, h->n));
+    h->workReady = true;
+    {   // the time-ordered attitude copy costs 104 B/row (+ 12 B/row of sort scratch at upload): take it
+        // only if it fits beside everything else with 2 GB to spare (the 116 GB Large config does not)
+        size_t freeB = 0, totB = 0;
+        CK(cudaMemGetInfo(&freeB, &totB));
+        const size_t need = size_t(m) * (N_ATT * 8 + 4 + 4) + size_t(m) * 12 + (size_t(64) << 20);
+        if (m > 0 && m < (int64_t(1) << 32) && L->n_dof_att < (int64_t(1) << 31) &&
+            freeB > need + (size_t(2) << 30)) {
+            bool ok = dalloc(&h->attT, m * N_ATT) == cudaSuccess && dalloc(&h->sT, m) == cudaSuccess &&
+                      dalloc(&h->permT, m) == cudaSuccess;
+            if (!ok) {
+                cudaGetLastError();
+                if (h->attT) cudaFree(h->attT);
+                if (h->sT) cudaFree(h->sT);
+                if (h->permT) cudaFree(h->permT);
+                h->attT = nullptr; h->sT = nullptr; h->permT = nullptr;
+            }
+            h->useAttT = ok;
+        }
+    }
     CK(cudaMallocHost(reinterpret_cast<void **>(&h->hostS), 2 * sizeof(Scalars)));
     const double one[2] = {1.0, 1.0}, tm[2] = {0.5, 0.5};
     CK(cudaMemcpy(h->coefOne, one, sizeof(one), cudaMemcpyHostToDevice));
@@ -188,7 +268,7 @@ int32_t gsr_destroy(gsr_handle *h)
     void *ptrs[] = {h->V, h->b, h->conVal, h->p, h->ia, h->iatt, h->rp, h->conRp, h->conCol, h->ic,
                     h->u, h->v, h->w, h->z, h->var, h->carryFirst, h->carryLast, h->globPartial,
                     h->sqPartialU, h->sqPartialV, h->ddPartial, h->coefOne, h->coefTime, h->trace,
-                    h->S, h->badDev};
+                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (h->hostS) cudaFreeHost(h->hostS);
@@ -254,6 +334,8 @@ int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail)
     k_fill<<<h->gridVec, 256, 0, h->stream>>>(h->p, h->n, 1.0);
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(h->stream));
+    int rcT = buildAttT(h);
+    if (rcT) return rcT;
     h->uploaded = true;
     h->preconditioned = false;
     return GSR_OK;
@@ -345,13 +427,21 @@ template <bool SQUARE>
 int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef, const int *done, bool prescale)
 {
     MatView A = view(h);
-    int nk = 0;
-    if (prescale) {
-        k_scale<<<h->gridVec, 256, 0, h->stream>>>(x, A.offAtt, A.n, coef, done);
+    int nk = 1;
+    k_pre_aprod2<<<h->gridVec, 256, 0, h->stream>>>(x, A.offAtt, A.n, coef, h->insRep, int64_t(h->nRep) * A.nInstr,
+                                                    prescale ? 1 : 0, done);
+    // attitude section: segmented reduction on the time-ordered copy when there is one; the
+    // preconditioner pass (SQUARE) and the low-memory fallback scatter it with REDs in k_aprod2
+    const bool attRed = SQUARE || !h->useAttT;
+    if (attRed) {
+        k_aprod2<SQUARE, true><<<h->gridA2, THREADS, APROD_SMEM, h->stream>>>(A, y, x, coef, h->carryFirst,
+                                                                            h->carryLast, h->globPartial, done);
+    } else {
+        k_aprod2_att<false><<<h->gridAtt, 256, 0, h->stream>>>(A, y, x, coef, done);
+        k_aprod2<false, false><<<h->gridA2, THREADS, APROD_SMEM, h->stream>>>(A, y, x, coef, h->carryFirst,
+                                                                            h->carryLast, h->globPartial, done);
         ++nk;
     }
-    k_aprod2<SQUARE><<<h->gridA2, THREADS, APROD_SMEM, h->stream>>>(A, y, x, coef, h->carryFirst, h->carryLast,
-                                                                  h->globPartial, done);
     k_astro_fixup<<<h->gridFix, 256, 0, h->stream>>>(A, x, coef, h->carryFirst, h->carryLast, h->globPartial,
                                                      h->gridA2, done);
     nk += 2;
@@ -364,7 +454,7 @@ int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef,
 
 int ensureWork(gsr_handle *h)
 {
-    if (h->workReady) return GSR_OK;
+    if (h->workReady) return GSR_OK;   // allocated by gsr_create
     CK(dalloc(&h->u, h->mTot));
     CK(dalloc(&h->v, h->n));
     CK(dalloc(&h->w, h->n));
@@ -447,6 +537,8 @@ int32_t gsr_precondition(gsr_handle *h)
     k_scale_values<<<gridFor(A.m * N_PAR, 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(A, h->p);
     if (A.nCon > 0)
         k_scale_con_values<<<gridFor(h->L.n_con_nnz, 256, h->smCount * 16), 256, 0, h->stream>>>(A, h->L.n_con_nnz, h->p);
+    if (h->useAttT)   // the time-ordered copy follows the scaled coefficients
+        k_gather_att<<<gridFor(A.m, 256, h->smCount * 16), 256, 0, h->stream>>>(A);
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(h->stream));
     h->preconditioned = true;
@@ -513,14 +605,14 @@ int32_t gsr_lsqr(gsr_handle *h, int64_t itnlim, double atol, double btol, double
     if (!h->iterGraph) {
         cudaGraph_t g = nullptr;
         CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
-        perIter = enqueueIteration(h);
+        h->perIter = enqueueIteration(h);
         cudaError_t ec = cudaStreamEndCapture(st, &g);
         if (ec != cudaSuccess) return fail(h, GSR_ECUDA, "graph capture: %s", cudaGetErrorString(ec));
         ec = cudaGraphInstantiate(&h->iterGraph, g, 0);
         cudaGraphDestroy(g);
         if (ec != cudaSuccess) return fail(h, GSR_ECUDA, "graph instantiate: %s", cudaGetErrorString(ec));
     }
-    perIter = 7 + (h->L.n_con > 0 ? 2 : 0) + 3;
+    perIter = h->perIter;
 
     // Loop control: the device decides (S->done); the host enqueues chunks of graph launches and
     // polls the scalars of the previous chunk while the next one runs.
@@ -592,7 +684,8 @@ int32_t gsr_last_timing(gsr_handle *h, double *loop_ms, int64_t *kernel_launches
 int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_per_launch)
 {
     if (!h || !ms_per_launch || reps < 1) return GSR_EINVAL;
-    if (which != 1 && which != 2 && which != 11 && which != 12) return fail(h, GSR_EINVAL, "which");
+    if (which != 1 && which != 2 && which != 11 && which != 12 && which != 13) return fail(h, GSR_EINVAL, "which");
+    if (which == 13 && !h->useAttT) return fail(h, GSR_ESTATE, "no time-ordered attitude copy on this handle");
     int rc = readyCheck(h);
     if (rc) return rc;
     rc = enter(h);
@@ -609,9 +702,14 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
         else if (which == 2) enqueueAprod2<false>(h, h->u, h->v, h->coefTime, nullptr, true);
         else if (which == 11)
             k_aprod1<<<h->gridA1, THREADS, APROD_SMEM, st>>>(A, h->v, h->u, h->coefTime, h->sqPartialU, nullptr);
+        else if (which == 13)
+            k_aprod2_att<false><<<h->gridAtt, 256, 0, st>>>(A, h->u, h->v, h->coefTime, nullptr);
+        else if (h->useAttT)
+            k_aprod2<false, false><<<h->gridA2, THREADS, APROD_SMEM, st>>>(A, h->u, h->v, h->coefTime, h->carryFirst,
+                                                                        h->carryLast, h->globPartial, nullptr);
         else
-            k_aprod2<false><<<h->gridA2, THREADS, APROD_SMEM, st>>>(A, h->u, h->v, h->coefTime, h->carryFirst,
-                                                                 h->carryLast, h->globPartial, nullptr);
+            k_aprod2<false, true><<<h->gridA2, THREADS, APROD_SMEM, st>>>(A, h->u, h->v, h->coefTime, h->carryFirst,
+                                                                       h->carryLast, h->globPartial, nullptr);
     };
     once();   // warm-up
     CK(cudaGetLastError());

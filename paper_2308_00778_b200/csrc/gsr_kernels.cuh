@@ -27,6 +27,14 @@ struct MatView {
     const int64_t *conRp, *conCol;
     double *conVal;
     int64_t nCon;
+    // time-ordered attitude copy (built at upload when memory allows; nullptr otherwise):
+    // attT[k*m + t] = V[permT[t]*24 + 5 + k], rows t sorted by attitude start sT[t] (stable)
+    double *attT;
+    const int32_t *sT;
+    const uint32_t *permT;
+    // replicated accumulators of the instrumental section for aprod2: insRep[r*nInstr + c]
+    double *insRep;
+    int nRep;
 };
 
 // Scalars of the LSQR recurrences, resident in device memory.
@@ -72,6 +80,7 @@ __device__ __forceinline__ double block_sum(double v, double *red)
 // vector loads, staged row-padded into shared memory so that each lane can then read its own
 // row with conflict-free LDS.128 ("coalesced, vectorised 16-byte loads of
 // each row's 192-byte value block").
+template <bool SKIP_ATT = false>
 __device__ __forceinline__ void stage_tile(double *sm, const double *gV, int nrows, int lane)
 {
     const double2 *g = reinterpret_cast<const double2 *>(gV);
@@ -80,15 +89,16 @@ __device__ __forceinline__ void stage_tile(double *sm, const double *gV, int nro
 #pragma unroll
     for (int t = 0; t < 12; ++t) {
         const int c = t * 32 + lane;
-        if (c < nchunk) r[t] = __ldcs(g + c);
+        const int q = c % 12;
+        // 16-byte chunks 4..7 of a row (bytes 64..127) hold attitude coefficients only
+        if (c < nchunk && !(SKIP_ATT && q >= 4 && q < 8)) r[t] = __ldcs(g + c);
     }
 #pragma unroll
     for (int t = 0; t < 12; ++t) {
         const int c = t * 32 + lane;
-        if (c < nchunk) {
-            const int row = c / 12, q = c - row * 12;
+        const int row = c / 12, q = c - row * 12;
+        if (c < nchunk && !(SKIP_ATT && q >= 4 && q < 8))
             *reinterpret_cast<double2 *>(sm + row * ROW_PAD + 2 * q) = r[t];
-        }
     }
 }
 
@@ -176,7 +186,10 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
 // SQUARE: terms are V^2 (y == 1): the column sums of squares of the preconditioner.
 // coef = {cx, cy} in device memory.
 // ---------------------------------------------------------------------------------------
-template <bool SQUARE>
+// ATT_RED: scatter the attitude section here with REDs (fallback / preconditioner pass); when false
+// the attitude section is done by k_aprod2_att on the time-ordered copy and the chunks of A that
+// hold only attitude coefficients are not even loaded.
+template <bool SQUARE, bool ATT_RED>
 __global__ void __launch_bounds__(THREADS, 2)
 k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
          const double *__restrict__ coef, double *__restrict__ carryFirst,
@@ -189,13 +202,16 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
     double *sm = reinterpret_cast<double *>(smem2) + warp * TILE * ROW_PAD;
     const double cx = coef[0], cy = coef[1];
     const int64_t nTiles = (A.m + TILE - 1) / TILE;
-    double *xAtt = x + A.offAtt, *xIns = x + A.offInstr;
+    double *xAtt = x + A.offAtt;
+    // instrumental REDs go to one of nRep replicas of the section (spreads the L2 atomic traffic
+    // over nRep times more lines); k_astro_fixup folds the replicas into x in a fixed order
+    double *xIns = A.insRep + int64_t((blockIdx.x * WARPS + warp) % A.nRep) * A.nInstr;
     double gsum = 0.0;
     for (int64_t tile = int64_t(blockIdx.x) * WARPS + warp; tile < nTiles;
          tile += int64_t(gridDim.x) * WARPS) {
         const int64_t r0 = tile * TILE;
         const int nrows = int(min(int64_t(TILE), A.m - r0));
-        stage_tile(sm, A.V + r0 * N_PAR, nrows, lane);
+        stage_tile<!ATT_RED>(sm, A.V + r0 * N_PAR, nrows, lane);
         __syncwarp();
         const bool valid = lane < nrows;
         const int64_t i = r0 + (valid ? lane : nrows - 1);
@@ -209,13 +225,15 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
 
         // ---- attitude + instrumental scatter (valid lanes only; invalid lanes hold zeros)
         if (valid) {
-            double *xt = xAtt + A.iatt[i];
             const int2 *icp = reinterpret_cast<const int2 *>(A.ic) + i * 3;
             const int2 c0 = __ldcs(icp), c1 = __ldcs(icp + 1), c2 = __ldcs(icp + 2);
+            if (ATT_RED) {
+                double *xt = xAtt + A.iatt[i];
 #pragma unroll
-            for (int a = 0; a < 3; ++a)
+                for (int a = 0; a < 3; ++a)
 #pragma unroll
-                for (int j = 0; j < 4; ++j) atomicAdd(xt + a * A.nDof + j, v[5 + 4 * a + j]);
+                    for (int j = 0; j < 4; ++j) atomicAdd(xt + a * A.nDof + j, v[5 + 4 * a + j]);
+            }
             atomicAdd(xIns + c0.x, v[17]);
             atomicAdd(xIns + c0.y, v[18]);
             atomicAdd(xIns + c1.x, v[19]);
@@ -282,11 +300,22 @@ k_astro_fixup(MatView A, double *__restrict__ x, const double *__restrict__ coef
     __shared__ double red[32];
     if (done && *done) return;
     const double cx = coef[0];
+    const int starBlocks = int((A.nStars + blockDim.x - 1) / blockDim.x);
     if (blockIdx.x == gridDim.x - 1) {
         double g = 0.0;
         for (int p = threadIdx.x; p < nGlobPartial; p += blockDim.x) g += globPartial[p];
         g = block_sum(g, red);
         if (threadIdx.x == 0) x[A.offGlob] += g;   // section already scaled by cx
+        return;
+    }
+    if (blockIdx.x >= starBlocks) {
+        // fold the instrument replicas (replica order fixed) into the pre-scaled section
+        const int64_t c = int64_t(blockIdx.x - starBlocks) * blockDim.x + threadIdx.x;
+        if (c < A.nInstr) {
+            double t = 0.0;
+            for (int r = 0; r < A.nRep; ++r) t += A.insRep[int64_t(r) * A.nInstr + c];
+            x[A.offInstr + c] += t;
+        }
         return;
     }
     const int64_t s = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
@@ -310,15 +339,110 @@ k_astro_fixup(MatView A, double *__restrict__ x, const double *__restrict__ coef
     for (int k = 0; k < N_ASTRO; ++k) xa[k] = fma(cx, xa[k], acc[k]);
 }
 
-// x[lo..hi) *= coef[0]  (att + instr + gamma sections before the scatter of aprod2)
-__global__ void k_scale(double *__restrict__ x, int64_t lo, int64_t hi,
-                        const double *__restrict__ coef, const int *done)
+// Before the scatter of aprod2: x[lo..hi) *= coef[0] (att + instr + gamma sections, only when
+// prescale) and the instrument replicas are zeroed.
+__global__ void k_pre_aprod2(double *__restrict__ x, int64_t lo, int64_t hi,
+                             const double *__restrict__ coef, double *__restrict__ rep,
+                             int64_t nRepTotal, int prescale, const int *done)
 {
     if (done && *done) return;
-    const double c = coef[0];
-    for (int64_t j = lo + int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < hi;
-         j += int64_t(gridDim.x) * blockDim.x)
-        x[j] *= c;
+    const int64_t tid = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+    const int64_t nth = int64_t(gridDim.x) * blockDim.x;
+    if (prescale) {
+        const double c = coef[0];
+        for (int64_t j = lo + tid; j < hi; j += nth) x[j] *= c;
+    }
+    for (int64_t j = tid; j < nRepTotal; j += nth) rep[j] = 0.0;
+}
+
+// ---------------------------------------------------------------------------------------
+// aprod2, attitude section on the time-ordered copy ("bucketed scatter", north_star; the
+// paper's kernels use one atomicAdd per coefficient, Alg. 3).  Rows t are
+// sorted by attitude start s, so the 32 rows of a warp tile share very few distinct s: a
+// segmented scan by s over the tile leaves one sum per (s, axis, j) and only those are added to x
+// (RED), instead of 12 REDs per row.  y is gathered through permT (one 8-byte gather per row).
+// ---------------------------------------------------------------------------------------
+template <bool SQUARE>
+__global__ void __launch_bounds__(256)
+k_aprod2_att(MatView A, const double *__restrict__ y, double *__restrict__ x,
+             const double *__restrict__ coef, const int *done)
+{
+    if (done && *done) return;
+    const int lane = threadIdx.x & 31;
+    const double cy = coef[1];
+    double *xAtt = x + A.offAtt;
+    const int64_t nTiles = (A.m + TILE - 1) / TILE;
+    const int64_t warpId = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) >> 5;
+    const int64_t nWarps = (int64_t(gridDim.x) * blockDim.x) >> 5;
+    for (int64_t tile = warpId; tile < nTiles; tile += nWarps) {
+        const int64_t t0 = tile * TILE;
+        const int nrows = int(min(int64_t(TILE), A.m - t0));
+        const bool valid = lane < nrows;
+        const int64_t t = t0 + (valid ? lane : nrows - 1);
+        const int32_t sv = __ldcs(A.sT + t);
+        double yv = 0.0;
+        if (valid) yv = SQUARE ? 1.0 : cy * __ldg(y + __ldcs(A.permT + t));
+        double v[N_ATT];
+#pragma unroll
+        for (int k = 0; k < N_ATT; ++k) {
+            const double a = __ldcs(A.attT + int64_t(k) * A.m + t);
+            v[k] = SQUARE ? a * a * yv : a * yv;
+        }
+        const int32_t sPrev = __shfl_up_sync(0xffffffffu, sv, 1);
+        const int32_t sNext = __shfl_down_sync(0xffffffffu, sv, 1);
+        const bool head = (lane == 0) || (sv != sPrev);
+        const bool tail = valid && ((lane == nrows - 1) || (sv != sNext));
+        const unsigned heads = __ballot_sync(0xffffffffu, head);
+        if (heads == 1u) {
+            // one s in the whole tile (the common case): plain warp sums, lanes 0..11 add one each
+            double mine = 0.0;
+#pragma unroll
+            for (int k = 0; k < N_ATT; ++k) {
+                const double t2 = warp_sum(v[k]);
+                if (lane == k) mine = t2;
+            }
+            if (lane < N_ATT) atomicAdd(xAtt + int64_t(lane >> 2) * A.nDof + sv + (lane & 3), mine);
+        } else {
+            const int segStart = 31 - __clz(heads & (0xffffffffu >> (31 - lane)));
+            const int dist = lane - segStart;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+#pragma unroll
+                for (int k = 0; k < N_ATT; ++k) {
+                    const double t2 = __shfl_up_sync(0xffffffffu, v[k], d);
+                    if (dist >= d) v[k] += t2;
+                }
+            }
+            if (tail) {
+#pragma unroll
+                for (int a = 0; a < 3; ++a)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) atomicAdd(xAtt + a * A.nDof + sv + j, v[4 * a + j]);
+            }
+        }
+    }
+}
+
+// attT[k*m + t] = V[permT[t]*24 + 5 + k]  (re-run after the values are scaled by p)
+__global__ void k_gather_att(MatView A)
+{
+    for (int64_t t = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; t < A.m;
+         t += int64_t(gridDim.x) * blockDim.x) {
+        const double *row = A.V + int64_t(A.permT[t]) * N_PAR + N_ASTRO;
+#pragma unroll
+        for (int k = 0; k < N_ATT; ++k) A.attT[int64_t(k) * A.m + t] = row[k];
+    }
+}
+
+// keys / values of the time sort: key = attitude start (int32), value = row
+__global__ void k_sort_keys(const int64_t *__restrict__ iatt, int64_t m, int32_t *__restrict__ key,
+                            uint32_t *__restrict__ val)
+{
+    for (int64_t i = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; i < m;
+         i += int64_t(gridDim.x) * blockDim.x) {
+        key[i] = int32_t(iatt[i]);
+        val[i] = uint32_t(i);
+    }
 }
 
 // ---------------------------------------------------------------------------------------
