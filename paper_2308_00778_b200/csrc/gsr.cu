@@ -39,7 +39,10 @@ struct gsr_handle {
     Scalars *S = nullptr;
     Scalars *hostS = nullptr;           // pinned, 2 slots
     unsigned long long *badDev = nullptr;
-    int gridA1 = 1, gridA2 = 1, gridVec = 1, gridCon = 1, gridFix = 1;
+    // upload staging (host sources are copied here piecewise, then written tile-transposed)
+    double *stageV = nullptr;
+    int32_t *stageC = nullptr;
+    int gridA1 = 1, gridA2 = 1, gridA2m = 1, gridVec = 1, gridCon = 1, gridFix = 1;
     bool uploaded = false, conUploaded = false, preconditioned = false, workReady = false;
     int64_t badRow = -1;
     cudaGraphExec_t iterGraph = nullptr;
@@ -109,13 +112,27 @@ int enter(gsr_handle *h)
     return GSR_OK;
 }
 
-// Time order of the attitude section (setup): stable radix sort of the rows by
-// attitude start (cub, a library primitive used once per upload, not on the per-iteration path),
-// then a gather of the 12 attitude coefficients of every row into column-major attT.
+constexpr int64_t STAGE_ROWS = int64_t(1) << 20;   // rows per staging piece (192 MB + 24 MB)
+
+bool isDevicePtr(const void *p)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+// Time order of the attitude section (setup).  Rows are cut into blocks of
+// 2^ATT_BLOCK_BITS consecutive rows (star order); inside a block they are stably sorted by attitude
+// start (cub radix sort, a library primitive used once per upload, not on the per-iteration path).
+// A block's slice of y (16 MB) then stays in L2 while k_aprod2_att gathers it through permT.  The 12
+// attitude coefficients of every row are gathered into column-major attT.
 int buildAttT(gsr_handle *h)
 {
     if (!h->useAttT) return GSR_OK;
-    const int64_t m = h->L.n_obs;
+    const int64_t m = h->L.n_obs, blk = int64_t(1) << ATT_BLOCK_BITS;
     MatView A = view(h);
     int32_t *keyIn = nullptr;
     uint32_t *valIn = nullptr;
@@ -123,14 +140,17 @@ int buildAttT(gsr_handle *h)
     size_t tmpBytes = 0;
     int endBit = 1;
     while (endBit < 31 && (int64_t(1) << endBit) < h->L.n_dof_att) ++endBit;
-    cudaError_t e = cub::DeviceRadixSort::SortPairs(nullptr, tmpBytes, keyIn, h->sT, valIn, h->permT, m, 0,
+    const int64_t cap = std::min(m, blk);
+    cudaError_t e = cub::DeviceRadixSort::SortPairs(nullptr, tmpBytes, keyIn, h->sT, valIn, h->permT, cap, 0,
                                                     endBit, h->stream);
-    if (e == cudaSuccess) e = dalloc(&keyIn, m);
-    if (e == cudaSuccess) e = dalloc(&valIn, m);
+    if (e == cudaSuccess) e = dalloc(&keyIn, cap);
+    if (e == cudaSuccess) e = dalloc(&valIn, cap);
     if (e == cudaSuccess) e = cudaMalloc(&tmp, std::max<size_t>(tmpBytes, 16));
-    if (e == cudaSuccess) {
-        k_sort_keys<<<gridFor(m, 256, h->smCount * 16), 256, 0, h->stream>>>(h->iatt, m, keyIn, valIn);
-        e = cub::DeviceRadixSort::SortPairs(tmp, tmpBytes, keyIn, h->sT, valIn, h->permT, m, 0, endBit, h->stream);
+    for (int64_t i0 = 0; e == cudaSuccess && i0 < m; i0 += blk) {
+        const int64_t cnt = std::min(blk, m - i0);
+        k_sort_keys<<<gridFor(cnt, 256, h->smCount * 16), 256, 0, h->stream>>>(h->iatt, i0, cnt, keyIn, valIn);
+        e = cub::DeviceRadixSort::SortPairs(tmp, tmpBytes, keyIn, h->sT + i0, valIn, h->permT + i0, cnt, 0, endBit,
+                                            h->stream);
     }
     if (e == cudaSuccess) {
         k_gather_att<<<gridFor(m, 256, h->smCount * 16), 256, 0, h->stream>>>(A);
@@ -183,15 +203,13 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(cudaEventCreateWithFlags(&h->evSlot[0], cudaEventDisableTiming));
     CK(cudaEventCreateWithFlags(&h->evSlot[1], cudaEventDisableTiming));
 
-    CK(cudaFuncSetAttribute(k_aprod1, cudaFuncAttributeMaxDynamicSharedMemorySize, int(APROD_SMEM)));
-    CK(cudaFuncSetAttribute(k_aprod2<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(APROD_SMEM)));
-    CK(cudaFuncSetAttribute(k_aprod2<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(APROD_SMEM)));
-    CK(cudaFuncSetAttribute(k_aprod2<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, int(APROD_SMEM)));
-    int occ1 = 1, occ2 = 1;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, k_aprod1, THREADS, APROD_SMEM));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, k_aprod2<false, true>, THREADS, APROD_SMEM));
+    int occ1 = 1, occ2 = 1, occ2m = 1;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, k_aprod1, THREADS, 0));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, k_aprod2<false, true>, THREADS, 0));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2m, k_aprod2<false, false>, THREADS, 0));
     h->gridA1 = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ1, 1));
     h->gridA2 = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ2, 1));
+    h->gridA2m = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ2m, 1));   // main kernel without attitude
     h->gridVec = gridFor(std::max(h->n, h->mTot), 256 * 4, h->smCount * 8);
     h->gridCon = gridFor(L->n_con, 8, h->smCount * 8);
     // fix-up grid: one thread per star, then one per instrument column (replica fold), then gamma
@@ -201,10 +219,15 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     h->nRep = int(std::max<int64_t>(1, std::min<int64_t>(128, (524288 + L->n_instr - 1) / L->n_instr)));
 
     const int64_t m = L->n_obs;
-    CK(dalloc(&h->V, m * N_PAR));
+    // coefficients and instrument columns are stored tile-transposed and padded to whole tiles
+    CK(dalloc(&h->V, h->nTiles * TILE * N_PAR));
     CK(dalloc(&h->ia, m));
     CK(dalloc(&h->iatt, m));
-    CK(dalloc(&h->ic, m * N_INSTR));
+    CK(dalloc(&h->ic, h->nTiles * TILE * N_INSTR));
+    if (h->nTiles > 0) {   // zero the padding rows of the last tile
+        CK(cudaMemset(h->V + (h->nTiles - 1) * TILE * N_PAR, 0, sizeof(double) * TILE * N_PAR));
+        CK(cudaMemset(h->ic + (h->nTiles - 1) * TILE * N_INSTR, 0, sizeof(int32_t) * TILE * N_INSTR));
+    }
     CK(dalloc(&h->b, h->mTot));
     CK(dalloc(&h->rp, L->n_stars + 1));
     CK(dalloc(&h->conRp, L->n_con + 1));
@@ -213,7 +236,7 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(dalloc(&h->p, h->n));
     CK(dalloc(&h->carryFirst, h->nTiles * N_ASTRO));
     CK(dalloc(&h->carryLast, h->nTiles * N_ASTRO));
-    CK(dalloc(&h->globPartial, h->gridA2));
+    CK(dalloc(&h->globPartial, std::max(h->gridA2, h->gridA2m)));
     CK(dalloc(&h->sqPartialU, h->gridA1 + h->gridCon));
     CK(dalloc(&h->sqPartialV, h->gridVec));
     CK(dalloc(&h->ddPartial, h->gridVec));
@@ -268,7 +291,7 @@ int32_t gsr_destroy(gsr_handle *h)
     void *ptrs[] = {h->V, h->b, h->conVal, h->p, h->ia, h->iatt, h->rp, h->conRp, h->conCol, h->ic,
                     h->u, h->v, h->w, h->z, h->var, h->carryFirst, h->carryLast, h->globPartial,
                     h->sqPartialU, h->sqPartialV, h->ddPartial, h->coefOne, h->coefTime, h->trace,
-                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT};
+                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (h->hostS) cudaFreeHost(h->hostS);
@@ -298,11 +321,33 @@ int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double
     h->uploaded = false;
     h->preconditioned = false;
     const size_t r = size_t(nrows);
-    CK(cudaMemcpyAsync(h->V + row0 * N_PAR, values, r * N_PAR * sizeof(double), cudaMemcpyDefault, h->stream));
     CK(cudaMemcpyAsync(h->ia + row0, ia, r * sizeof(int64_t), cudaMemcpyDefault, h->stream));
     CK(cudaMemcpyAsync(h->iatt + row0, iatt, r * sizeof(int64_t), cudaMemcpyDefault, h->stream));
-    CK(cudaMemcpyAsync(h->ic + row0 * N_INSTR, ic, r * N_INSTR * sizeof(int32_t), cudaMemcpyDefault, h->stream));
     CK(cudaMemcpyAsync(h->b + row0, b, r * sizeof(double), cudaMemcpyDefault, h->stream));
+    // values and instrCol: row-major in the caller's memory -> tile-transposed on the device.
+    // Device sources are read in place; host sources go through a bounded staging buffer.
+    MatView A = view(h);
+    const bool devV = nrows > 0 && isDevicePtr(values), devC = nrows > 0 && isDevicePtr(ic);
+    if (nrows > 0 && (!devV || !devC) && !h->stageV) {
+        CK(dalloc(&h->stageV, STAGE_ROWS * N_PAR));
+        CK(dalloc(&h->stageC, STAGE_ROWS * N_INSTR));
+    }
+    for (int64_t q0 = 0; q0 < nrows; q0 += STAGE_ROWS) {
+        const int64_t cnt = std::min(STAGE_ROWS, nrows - q0);
+        const double *srcV = values + q0 * N_PAR;
+        const int32_t *srcC = ic + q0 * N_INSTR;
+        if (!devV) {
+            CK(cudaMemcpyAsync(h->stageV, srcV, size_t(cnt) * N_PAR * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+            srcV = h->stageV;
+        }
+        if (!devC) {
+            CK(cudaMemcpyAsync(h->stageC, srcC, size_t(cnt) * N_INSTR * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
+            srcC = h->stageC;
+        }
+        k_ingest_rows<<<gridFor(cnt * (N_PAR + N_INSTR), 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(
+            A, h->ic, row0 + q0, cnt, srcV, srcC);
+        CK(cudaGetLastError());
+    }
     CK(cudaStreamSynchronize(h->stream));
     return GSR_OK;
 }
@@ -410,7 +455,7 @@ int enqueueAprod1(gsr_handle *h, const double *x, double *y, const double *coef,
                   const int *done, int *nPartial)
 {
     MatView A = view(h);
-    k_aprod1<<<h->gridA1, THREADS, APROD_SMEM, h->stream>>>(A, x, y, coef, sqPartial, done);
+    k_aprod1<<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sqPartial, done);
     int nk = 1, np = h->gridA1;
     if (A.nCon > 0) {
         k_con_aprod1<<<h->gridCon, 256, 0, h->stream>>>(A, x, y, coef, sqPartial ? sqPartial + h->gridA1 : nullptr, done);
@@ -434,16 +479,16 @@ int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef,
     // preconditioner pass (SQUARE) and the low-memory fallback scatter it with REDs in k_aprod2
     const bool attRed = SQUARE || !h->useAttT;
     if (attRed) {
-        k_aprod2<SQUARE, true><<<h->gridA2, THREADS, APROD_SMEM, h->stream>>>(A, y, x, coef, h->carryFirst,
+        k_aprod2<SQUARE, true><<<h->gridA2, THREADS, 0, h->stream>>>(A, y, x, coef, h->carryFirst,
                                                                             h->carryLast, h->globPartial, done);
     } else {
         k_aprod2_att<false><<<h->gridAtt, 256, 0, h->stream>>>(A, y, x, coef, done);
-        k_aprod2<false, false><<<h->gridA2, THREADS, APROD_SMEM, h->stream>>>(A, y, x, coef, h->carryFirst,
-                                                                            h->carryLast, h->globPartial, done);
+        k_aprod2<false, false><<<h->gridA2m, THREADS, 0, h->stream>>>(A, y, x, coef, h->carryFirst,
+                                                                             h->carryLast, h->globPartial, done);
         ++nk;
     }
     k_astro_fixup<<<h->gridFix, 256, 0, h->stream>>>(A, x, coef, h->carryFirst, h->carryLast, h->globPartial,
-                                                     h->gridA2, done);
+                                                     attRed ? h->gridA2 : h->gridA2m, done);
     nk += 2;
     if (A.nCon > 0) {
         k_con_aprod2<SQUARE><<<h->gridCon, 256, 0, h->stream>>>(A, y, x, coef, done);
@@ -511,7 +556,24 @@ int32_t gsr_get_values(gsr_handle *h, double *out, double *con_val_out)
     if (!h->uploaded) return fail(h, GSR_ESTATE, "no system uploaded");
     int rc = enter(h);
     if (rc) return rc;
-    CK(cudaMemcpyAsync(out, h->V, size_t(h->L.n_obs) * N_PAR * sizeof(double), cudaMemcpyDefault, h->stream));
+    {   // the device keeps the coefficients tile-transposed: export the row-major view piecewise
+        MatView A = view(h);
+        const int64_t m = h->L.n_obs;
+        const bool devOut = isDevicePtr(out);
+        if (m > 0 && !devOut && !h->stageV) {
+            CK(dalloc(&h->stageV, STAGE_ROWS * N_PAR));
+            CK(dalloc(&h->stageC, STAGE_ROWS * N_INSTR));
+        }
+        for (int64_t q0 = 0; q0 < m; q0 += STAGE_ROWS) {
+            const int64_t cnt = std::min(STAGE_ROWS, m - q0);
+            double *dst = devOut ? out + q0 * N_PAR : h->stageV;
+            k_export_rows<<<gridFor(cnt * N_PAR, 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(A, q0, cnt, dst);
+            CK(cudaGetLastError());
+            if (!devOut)
+                CK(cudaMemcpyAsync(out + q0 * N_PAR, h->stageV, size_t(cnt) * N_PAR * sizeof(double),
+                                   cudaMemcpyDeviceToHost, h->stream));
+        }
+    }
     if (con_val_out && h->L.n_con_nnz > 0)
         CK(cudaMemcpyAsync(con_val_out, h->conVal, size_t(h->L.n_con_nnz) * sizeof(double), cudaMemcpyDefault,
                            h->stream));
@@ -534,7 +596,7 @@ int32_t gsr_precondition(gsr_handle *h)
     enqueueAprod2<true>(h, nullptr, h->p, h->coefOne, nullptr, false);
     CK(cudaGetLastError());
     k_colscale<<<h->gridVec, 256, 0, h->stream>>>(h->p, h->n);
-    k_scale_values<<<gridFor(A.m * N_PAR, 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(A, h->p);
+    k_scale_values<<<gridFor(h->nTiles * TILE * N_PAR, 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(A, h->p);
     if (A.nCon > 0)
         k_scale_con_values<<<gridFor(h->L.n_con_nnz, 256, h->smCount * 16), 256, 0, h->stream>>>(A, h->L.n_con_nnz, h->p);
     if (h->useAttT)   // the time-ordered copy follows the scaled coefficients
@@ -701,14 +763,14 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
         if (which == 1) enqueueAprod1(h, h->v, h->u, h->coefTime, h->sqPartialU, nullptr, nullptr);
         else if (which == 2) enqueueAprod2<false>(h, h->u, h->v, h->coefTime, nullptr, true);
         else if (which == 11)
-            k_aprod1<<<h->gridA1, THREADS, APROD_SMEM, st>>>(A, h->v, h->u, h->coefTime, h->sqPartialU, nullptr);
+            k_aprod1<<<h->gridA1, THREADS, 0, st>>>(A, h->v, h->u, h->coefTime, h->sqPartialU, nullptr);
         else if (which == 13)
             k_aprod2_att<false><<<h->gridAtt, 256, 0, st>>>(A, h->u, h->v, h->coefTime, nullptr);
         else if (h->useAttT)
-            k_aprod2<false, false><<<h->gridA2, THREADS, APROD_SMEM, st>>>(A, h->u, h->v, h->coefTime, h->carryFirst,
+            k_aprod2<false, false><<<h->gridA2m, THREADS, 0, st>>>(A, h->u, h->v, h->coefTime, h->carryFirst,
                                                                         h->carryLast, h->globPartial, nullptr);
         else
-            k_aprod2<false, true><<<h->gridA2, THREADS, APROD_SMEM, st>>>(A, h->u, h->v, h->coefTime, h->carryFirst,
+            k_aprod2<false, true><<<h->gridA2, THREADS, 0, st>>>(A, h->u, h->v, h->coefTime, h->carryFirst,
                                                                        h->carryLast, h->globPartial, nullptr);
     };
     once();   // warm-up

@@ -9,17 +9,24 @@ namespace gsr {
 
 constexpr int N_ASTRO = 5, N_ATT = 12, N_INSTR = 6, N_PAR = 24;
 constexpr int TILE = 32;          // rows per warp tile
-constexpr int ROW_PAD = 26;       // doubles per staged row in shared memory (208 B: LDS.128 conflict-free)
 constexpr int WARPS = 8;          // warps per CTA of the aprod kernels
 constexpr int THREADS = WARPS * 32;
-constexpr size_t APROD_SMEM = size_t(WARPS) * TILE * ROW_PAD * sizeof(double);
+constexpr int ATT_BLOCK_BITS = 21;   // rows per block of the time-ordered attitude copy (2^21)
+
+// Device layout of the coefficients ("tile-transposed"): the 32 rows of a warp tile are stored
+// coefficient-major, V[(tile*24 + k)*32 + lane], so that lane <-> row reads each of its 24
+// coefficients with one coalesced 8-byte load per warp instruction (256 B, two lines) and no
+// shared-memory transposition.  instrCol likewise: ic[(tile*6 + j)*32 + lane].  Storage is padded
+// to whole tiles (zero coefficients, column 0).  The upload format stays row-major.
+__host__ __device__ __forceinline__ int64_t vpos(int64_t i, int k) { return ((i >> 5) * N_PAR + k) * TILE + (i & 31); }
+__host__ __device__ __forceinline__ int64_t cpos(int64_t i, int j) { return ((i >> 5) * N_INSTR + j) * TILE + (i & 31); }
 
 // Device view of the uploaded system (A_d, M_i, I_c) in upload layout.
 struct MatView {
-    double *V;             // [m*24]
+    double *V;             // [nTiles*24*32] tile-transposed, see vpos()
     const int64_t *ia;     // [m] 5*star
     const int64_t *iatt;   // [m] attitude start s_i (axis 0)
-    const int32_t *ic;     // [m*6]
+    const int32_t *ic;     // [nTiles*6*32] tile-transposed, see cpos()
     const int64_t *rp;     // [nStars+1] derived star row pointer
     int64_t m, nStars, nDof, nInstr;
     int64_t offAtt, offInstr, offGlob, n;
@@ -76,40 +83,16 @@ __device__ __forceinline__ double block_sum(double v, double *red)
     return r;
 }
 
-// Coalesced load of one warp tile (nrows x 192 B, contiguous in global memory) with 16-byte
-// vector loads, staged row-padded into shared memory so that each lane can then read its own
-// row with conflict-free LDS.128 ("coalesced, vectorised 16-byte loads of
-// each row's 192-byte value block").
-template <bool SKIP_ATT = false>
-__device__ __forceinline__ void stage_tile(double *sm, const double *gV, int nrows, int lane)
+// The 24 coefficients of row (tile, lane): coalesced streaming loads.  ATT: load the attitude
+// coefficients too (k = 5..16).
+template <bool ATT>
+__device__ __forceinline__ void load_row(const double *__restrict__ V, int64_t tile, int lane, double (&v)[N_PAR])
 {
-    const double2 *g = reinterpret_cast<const double2 *>(gV);
-    const int nchunk = nrows * 12;
-    double2 r[12];
+    const double *g = V + tile * (N_PAR * TILE) + lane;
 #pragma unroll
-    for (int t = 0; t < 12; ++t) {
-        const int c = t * 32 + lane;
-        const int q = c % 12;
-        // 16-byte chunks 4..7 of a row (bytes 64..127) hold attitude coefficients only
-        if (c < nchunk && !(SKIP_ATT && q >= 4 && q < 8)) r[t] = __ldcs(g + c);
-    }
-#pragma unroll
-    for (int t = 0; t < 12; ++t) {
-        const int c = t * 32 + lane;
-        const int row = c / 12, q = c - row * 12;
-        if (c < nchunk && !(SKIP_ATT && q >= 4 && q < 8))
-            *reinterpret_cast<double2 *>(sm + row * ROW_PAD + 2 * q) = r[t];
-    }
-}
-
-__device__ __forceinline__ void read_row(const double *sm, int lane, double (&v)[N_PAR])
-{
-    const double2 *s = reinterpret_cast<const double2 *>(sm + lane * ROW_PAD);
-#pragma unroll
-    for (int q = 0; q < 12; ++q) {
-        const double2 t = s[q];
-        v[2 * q] = t.x;
-        v[2 * q + 1] = t.y;
+    for (int q = 0; q < N_PAR; ++q) {
+        if (ATT || q < N_ASTRO || q >= N_ASTRO + N_ATT) v[q] = __ldcs(g + q * TILE);
+        else v[q] = 0.0;
     }
 }
 
@@ -123,11 +106,9 @@ __global__ void __launch_bounds__(THREADS, 2)
 k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
          const double *__restrict__ coef, double *__restrict__ sqPartial, const int *done)
 {
-    extern __shared__ double2 smem2[];
     __shared__ double red[32];
     if (done && *done) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double *sm = reinterpret_cast<double *>(smem2) + warp * TILE * ROW_PAD;
     const double cx = coef[0], cy = coef[1];
     const int64_t nTiles = (A.m + TILE - 1) / TILE;
     const double *xAtt = x + A.offAtt, *xIns = x + A.offInstr;
@@ -137,16 +118,16 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
          tile += int64_t(gridDim.x) * WARPS) {
         const int64_t r0 = tile * TILE;
         const int nrows = int(min(int64_t(TILE), A.m - r0));
-        stage_tile(sm, A.V + r0 * N_PAR, nrows, lane);
-        __syncwarp();
         if (lane < nrows) {
             const int64_t i = r0 + lane;
             double v[N_PAR];
-            read_row(sm, lane, v);
-            const double *xa = x + A.ia[i];
-            const double *xt = xAtt + A.iatt[i];
-            const int2 *icp = reinterpret_cast<const int2 *>(A.ic) + i * 3;
-            const int2 c0 = __ldcs(icp), c1 = __ldcs(icp + 1), c2 = __ldcs(icp + 2);
+            load_row<true>(A.V, tile, lane, v);
+            const double *xa = x + __ldcs(A.ia + i);
+            const double *xt = xAtt + __ldcs(A.iatt + i);
+            const int32_t *icp = A.ic + tile * (N_INSTR * TILE) + lane;
+            int32_t c[N_INSTR];
+#pragma unroll
+            for (int j = 0; j < N_INSTR; ++j) c[j] = __ldcs(icp + j * TILE);
             double sum = 0.0;
 #pragma unroll
             for (int k = 0; k < N_ASTRO; ++k) sum = fma(v[k], __ldg(xa + k), sum);
@@ -155,18 +136,13 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
 #pragma unroll
                 for (int j = 0; j < 4; ++j)
                     sum = fma(v[5 + 4 * a + j], __ldg(xt + a * A.nDof + j), sum);
-            sum = fma(v[17], __ldg(xIns + c0.x), sum);
-            sum = fma(v[18], __ldg(xIns + c0.y), sum);
-            sum = fma(v[19], __ldg(xIns + c1.x), sum);
-            sum = fma(v[20], __ldg(xIns + c1.y), sum);
-            sum = fma(v[21], __ldg(xIns + c2.x), sum);
-            sum = fma(v[22], __ldg(xIns + c2.y), sum);
+#pragma unroll
+            for (int j = 0; j < N_INSTR; ++j) sum = fma(v[17 + j], __ldg(xIns + c[j]), sum);
             sum = fma(v[23], xg, sum);
             const double yi = fma(cy, y[i], cx * sum);
             y[i] = yi;
             sq = fma(yi, yi, sq);
         }
-        __syncwarp();
     }
     const double b = block_sum(sq, red);
     if (threadIdx.x == 0 && sqPartial) sqPartial[blockIdx.x] = b;
@@ -195,11 +171,9 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
          const double *__restrict__ coef, double *__restrict__ carryFirst,
          double *__restrict__ carryLast, double *__restrict__ globPartial, const int *done)
 {
-    extern __shared__ double2 smem2[];
     __shared__ double red[32];
     if (done && *done) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double *sm = reinterpret_cast<double *>(smem2) + warp * TILE * ROW_PAD;
     const double cx = coef[0], cy = coef[1];
     const int64_t nTiles = (A.m + TILE - 1) / TILE;
     double *xAtt = x + A.offAtt;
@@ -211,13 +185,15 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
          tile += int64_t(gridDim.x) * WARPS) {
         const int64_t r0 = tile * TILE;
         const int nrows = int(min(int64_t(TILE), A.m - r0));
-        stage_tile<!ATT_RED>(sm, A.V + r0 * N_PAR, nrows, lane);
-        __syncwarp();
         const bool valid = lane < nrows;
         const int64_t i = r0 + (valid ? lane : nrows - 1);
         double v[N_PAR];
-        read_row(sm, valid ? lane : nrows - 1, v);
-        const int64_t ia = A.ia[i];
+        load_row<ATT_RED>(A.V, tile, valid ? lane : nrows - 1, v);
+        const int64_t ia = __ldcs(A.ia + i);
+        // astro index of the rows just before and just after the tile (-1: none), fetched with the
+        // tile's other loads instead of after the scan
+        const int64_t iaBefore = r0 > 0 ? __ldg(A.ia + r0 - 1) : int64_t(-1);
+        const int64_t iaAfter = r0 + nrows < A.m ? __ldg(A.ia + r0 + nrows) : int64_t(-1);
         double yv = 0.0;
         if (valid) yv = SQUARE ? 1.0 : cy * y[i];
 #pragma unroll
@@ -225,8 +201,10 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
 
         // ---- attitude + instrumental scatter (valid lanes only; invalid lanes hold zeros)
         if (valid) {
-            const int2 *icp = reinterpret_cast<const int2 *>(A.ic) + i * 3;
-            const int2 c0 = __ldcs(icp), c1 = __ldcs(icp + 1), c2 = __ldcs(icp + 2);
+            const int32_t *icp = A.ic + tile * (N_INSTR * TILE) + lane;
+            int32_t c[N_INSTR];
+#pragma unroll
+            for (int j = 0; j < N_INSTR; ++j) c[j] = __ldcs(icp + j * TILE);
             if (ATT_RED) {
                 double *xt = xAtt + A.iatt[i];
 #pragma unroll
@@ -234,12 +212,8 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
 #pragma unroll
                     for (int j = 0; j < 4; ++j) atomicAdd(xt + a * A.nDof + j, v[5 + 4 * a + j]);
             }
-            atomicAdd(xIns + c0.x, v[17]);
-            atomicAdd(xIns + c0.y, v[18]);
-            atomicAdd(xIns + c1.x, v[19]);
-            atomicAdd(xIns + c1.y, v[20]);
-            atomicAdd(xIns + c2.x, v[21]);
-            atomicAdd(xIns + c2.y, v[22]);
+#pragma unroll
+            for (int j = 0; j < N_INSTR; ++j) atomicAdd(xIns + c[j], v[17 + j]);
         }
         // ---- gamma: fixed-order warp sum, accumulated per warp over its tiles
         gsum += warp_sum(v[23]);
@@ -265,8 +239,8 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         }
         if (tail) {
             bool cut = false;
-            if (segStart == 0 && r0 > 0) cut = (A.ia[r0 - 1] == ia);
-            if (lane == nrows - 1 && r0 + nrows < A.m) cut = cut || (A.ia[r0 + nrows] == ia);
+            if (segStart == 0) cut = (iaBefore == ia);
+            if (lane == nrows - 1) cut = cut || (iaAfter == ia);
             if (!cut) {
                 double *xa = x + ia;
 #pragma unroll
@@ -277,7 +251,6 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
                 for (int k = 0; k < N_ASTRO; ++k) c[k] = s[k];
             }
         }
-        __syncwarp();
     }
     // CTA partial of gamma in fixed order (lane 0 of each warp holds its running sum)
     __syncthreads();
@@ -428,20 +401,20 @@ __global__ void k_gather_att(MatView A)
 {
     for (int64_t t = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; t < A.m;
          t += int64_t(gridDim.x) * blockDim.x) {
-        const double *row = A.V + int64_t(A.permT[t]) * N_PAR + N_ASTRO;
+        const int64_t i = A.permT[t];
 #pragma unroll
-        for (int k = 0; k < N_ATT; ++k) A.attT[int64_t(k) * A.m + t] = row[k];
+        for (int k = 0; k < N_ATT; ++k) A.attT[int64_t(k) * A.m + t] = A.V[vpos(i, N_ASTRO + k)];
     }
 }
 
-// keys / values of the time sort: key = attitude start (int32), value = row
-__global__ void k_sort_keys(const int64_t *__restrict__ iatt, int64_t m, int32_t *__restrict__ key,
+// keys / values of the time sort of rows [i0, i0+cnt): key = attitude start (int32), value = row
+__global__ void k_sort_keys(const int64_t *__restrict__ iatt, int64_t i0, int64_t cnt, int32_t *__restrict__ key,
                             uint32_t *__restrict__ val)
 {
-    for (int64_t i = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; i < m;
-         i += int64_t(gridDim.x) * blockDim.x) {
-        key[i] = int32_t(iatt[i]);
-        val[i] = uint32_t(i);
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < cnt;
+         q += int64_t(gridDim.x) * blockDim.x) {
+        key[q] = int32_t(iatt[i0 + q]);
+        val[q] = uint32_t(i0 + q);
     }
 }
 
@@ -685,7 +658,7 @@ __global__ void k_validate(MatView A, unsigned long long *badRow)
         bad = bad || s < 0 || s > A.nDof - 4;
 #pragma unroll
         for (int j = 0; j < N_INSTR; ++j) {
-            const int32_t c = A.ic[i * N_INSTR + j];
+            const int32_t c = A.ic[cpos(i, j)];
             bad = bad || c < 0 || c >= A.nInstr;
         }
         if (bad) atomicMin(badRow, (unsigned long long)i);
@@ -737,15 +710,19 @@ __global__ void k_colscale(double *__restrict__ p, int64_t n)
 // One thread per stored coefficient (coalesced over A_d).
 __global__ void k_scale_values(MatView A, const double *__restrict__ p)
 {
-    const int64_t total = A.m * N_PAR;
+    const int64_t total = ((A.m + TILE - 1) / TILE) * (N_PAR * TILE);
     for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < total;
          e += int64_t(gridDim.x) * blockDim.x) {
-        const int64_t i = e / N_PAR;
-        const int k = int(e - i * N_PAR);
+        // e = (tile*24 + k)*32 + lane
+        const int64_t tk = e >> 5;
+        const int64_t tile = tk / N_PAR;
+        const int k = int(tk - tile * N_PAR);
+        const int64_t i = tile * TILE + (e & 31);
+        if (i >= A.m) continue;
         int64_t c;
         if (k < N_ASTRO) c = A.ia[i] + k;
         else if (k < N_ASTRO + N_ATT) c = A.offAtt + ((k - N_ASTRO) >> 2) * A.nDof + A.iatt[i] + ((k - N_ASTRO) & 3);
-        else if (k < N_PAR - 1) c = A.offInstr + A.ic[i * N_INSTR + (k - N_ASTRO - N_ATT)];
+        else if (k < N_PAR - 1) c = A.offInstr + A.ic[cpos(i, k - N_ASTRO - N_ATT)];
         else c = A.offGlob;
         A.V[e] = A.V[e] * p[c];
     }
@@ -756,6 +733,36 @@ __global__ void k_scale_con_values(MatView A, int64_t nnz, const double *__restr
     for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < nnz;
          q += int64_t(gridDim.x) * blockDim.x)
         A.conVal[q] = A.conVal[q] * p[A.conCol[q]];
+}
+
+// Upload (Alg. 1 l.6-12): rows [row0, row0+cnt) arrive row-major (A_d, I_c as the paper
+// stores them) and are written tile-transposed.  One thread per stored element; the
+// reads are coalesced, the writes hit 32 lines per warp but only once per upload.
+__global__ void k_ingest_rows(MatView A, int32_t *__restrict__ icDev, int64_t row0, int64_t cnt,
+                              const double *__restrict__ values, const int32_t *__restrict__ ic)
+{
+    const int64_t nV = cnt * N_PAR, nC = cnt * N_INSTR;
+    for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < nV + nC;
+         e += int64_t(gridDim.x) * blockDim.x) {
+        if (e < nV) {
+            const int64_t r = e / N_PAR;
+            A.V[vpos(row0 + r, int(e - r * N_PAR))] = values[e];
+        } else {
+            const int64_t f = e - nV, r = f / N_INSTR;
+            icDev[cpos(row0 + r, int(f - r * N_INSTR))] = ic[f];
+        }
+    }
+}
+
+// out[(i - row0)*24 + k] = V(i, k) for rows [row0, row0+cnt): the row-major view for gsr_get_values.
+__global__ void k_export_rows(MatView A, int64_t row0, int64_t cnt, double *__restrict__ out)
+{
+    const int64_t nV = cnt * N_PAR;
+    for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < nV;
+         e += int64_t(gridDim.x) * blockDim.x) {
+        const int64_t r = e / N_PAR;
+        out[e] = A.V[vpos(row0 + r, int(e - r * N_PAR))];
+    }
 }
 
 __global__ void k_fill(double *__restrict__ a, int64_t n, double v)
