@@ -34,7 +34,7 @@ struct gsr_handle {
     double *attT = nullptr, *insRep = nullptr;
     int32_t *sT = nullptr;
     uint32_t *permT = nullptr;
-    int nRep = 1, gridAtt = 1, perIter = 0;
+    int nRep = 1, gridAtt = 1, perIter = 0, nInsSm = 0;
     bool useAttT = false;
     Scalars *S = nullptr;
     Scalars *hostS = nullptr;           // pinned, 2 slots
@@ -93,7 +93,7 @@ MatView view(const gsr_handle *h)
     A.n = h->n;
     A.conRp = h->conRp; A.conCol = h->conCol; A.conVal = h->conVal; A.nCon = h->L.n_con;
     A.attT = h->useAttT ? h->attT : nullptr; A.sT = h->sT; A.permT = h->permT;
-    A.insRep = h->insRep; A.nRep = h->nRep;
+    A.insRep = h->insRep; A.nRep = h->nRep; A.nInsSm = h->nInsSm;
     return A;
 }
 
@@ -206,15 +206,25 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     int occ1 = 1, occ2 = 1, occ2m = 1;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, k_aprod1, THREADS, 0));
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, k_aprod2<false, true>, THREADS, 0));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2m, k_aprod2<false, false>, THREADS, 0));
+    occ2m = 1;
     h->gridA1 = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ1, 1));
     h->gridA2 = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ2, 1));
-    h->gridA2m = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ2m, 1));   // main kernel without attitude
+    {   // main kernel without attitude: one CTA per SM with a private shared-memory table for the first
+        // nInsSm instrument columns (as many as fit beside the static shared memory)
+        int maxSm = 0;
+        CK(cudaDeviceGetAttribute(&maxSm, cudaDevAttrMaxSharedMemoryPerBlockOptin, L->device));
+        const int64_t fit = (int64_t(maxSm) - 1024) / int64_t(sizeof(double));
+        h->nInsSm = int(std::max<int64_t>(0, std::min<int64_t>(L->n_instr, fit)));
+        CK(cudaFuncSetAttribute(k_aprod2<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                int(h->nInsSm * sizeof(double))));
+        h->gridA2m = gridFor(h->nTiles, PRIV_THREADS / 32, h->smCount);
+        (void)occ2m;
+    }
     h->gridVec = gridFor(std::max(h->n, h->mTot), 256 * 4, h->smCount * 8);
     h->gridCon = gridFor(L->n_con, 8, h->smCount * 8);
     // fix-up grid: one thread per star, then one per instrument column (replica fold), then gamma
     h->gridFix = int((L->n_stars + 255) / 256) + int((L->n_instr + 255) / 256) + 1;
-    h->gridAtt = gridFor(h->nTiles, 8, h->smCount * 8);
+    h->gridAtt = gridFor(h->nTiles, 8, h->smCount * 4);
     // instrument replicas: spread the REDs of aprod2 over >= ~512k distinct addresses
     h->nRep = int(std::max<int64_t>(1, std::min<int64_t>(128, (524288 + L->n_instr - 1) / L->n_instr)));
 
@@ -483,7 +493,7 @@ int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef,
                                                                             h->carryLast, h->globPartial, done);
     } else {
         k_aprod2_att<false><<<h->gridAtt, 256, 0, h->stream>>>(A, y, x, coef, done);
-        k_aprod2<false, false><<<h->gridA2m, THREADS, 0, h->stream>>>(A, y, x, coef, h->carryFirst,
+        k_aprod2<false, false, true><<<h->gridA2m, PRIV_THREADS, size_t(h->nInsSm) * sizeof(double), h->stream>>>(A, y, x, coef, h->carryFirst,
                                                                              h->carryLast, h->globPartial, done);
         ++nk;
     }
@@ -767,7 +777,7 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
         else if (which == 13)
             k_aprod2_att<false><<<h->gridAtt, 256, 0, st>>>(A, h->u, h->v, h->coefTime, nullptr);
         else if (h->useAttT)
-            k_aprod2<false, false><<<h->gridA2m, THREADS, 0, st>>>(A, h->u, h->v, h->coefTime, h->carryFirst,
+            k_aprod2<false, false, true><<<h->gridA2m, PRIV_THREADS, size_t(h->nInsSm) * sizeof(double), st>>>(A, h->u, h->v, h->coefTime, h->carryFirst,
                                                                         h->carryLast, h->globPartial, nullptr);
         else
             k_aprod2<false, true><<<h->gridA2, THREADS, 0, st>>>(A, h->u, h->v, h->coefTime, h->carryFirst,

@@ -42,6 +42,7 @@ struct MatView {
     // replicated accumulators of the instrumental section for aprod2: insRep[r*nInstr + c]
     double *insRep;
     int nRep;
+    int nInsSm;            // instrument columns [0, nInsSm) accumulate in shared memory (k_aprod2<.., PRIV>)
 };
 
 // Scalars of the LSQR recurrences, resident in device memory.
@@ -165,24 +166,36 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
 // ATT_RED: scatter the attitude section here with REDs (fallback / preconditioner pass); when false
 // the attitude section is done by k_aprod2_att on the time-ordered copy and the chunks of A that
 // hold only attitude coefficients are not even loaded.
-template <bool SQUARE, bool ATT_RED>
-__global__ void __launch_bounds__(THREADS, 2)
+// PRIV ("shared-memory histogram plus global atomics", north_star): the CTA keeps private accumulators
+// for the instrument columns [0, nInsSm) in shared memory (ATOMS, no L2 traffic) and only the other
+// columns are added with REDs; the private table is flushed with one RED per touched column at the end.
+// One CTA of PRIV_THREADS per SM (the table takes most of the shared memory).
+constexpr int PRIV_THREADS = 512;
+template <bool SQUARE, bool ATT_RED, bool PRIV = false>
+__global__ void __launch_bounds__(PRIV ? PRIV_THREADS : THREADS, PRIV ? 1 : 2)
 k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
          const double *__restrict__ coef, double *__restrict__ carryFirst,
          double *__restrict__ carryLast, double *__restrict__ globPartial, const int *done)
 {
     __shared__ double red[32];
+    extern __shared__ double sIns[];   // PRIV: nInsSm private instrument accumulators
     if (done && *done) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int nWarpsCta = PRIV ? PRIV_THREADS / 32 : WARPS;
     const double cx = coef[0], cy = coef[1];
     const int64_t nTiles = (A.m + TILE - 1) / TILE;
     double *xAtt = x + A.offAtt;
     // instrumental REDs go to one of nRep replicas of the section (spreads the L2 atomic traffic
     // over nRep times more lines); k_astro_fixup folds the replicas into x in a fixed order
-    double *xIns = A.insRep + int64_t((blockIdx.x * WARPS + warp) % A.nRep) * A.nInstr;
+    double *xIns = A.insRep + int64_t((blockIdx.x * nWarpsCta + warp) % A.nRep) * A.nInstr;
+    const int32_t nSm = PRIV ? A.nInsSm : 0;
+    if (PRIV) {
+        for (int c = threadIdx.x; c < nSm; c += PRIV_THREADS) sIns[c] = 0.0;
+        __syncthreads();
+    }
     double gsum = 0.0;
-    for (int64_t tile = int64_t(blockIdx.x) * WARPS + warp; tile < nTiles;
-         tile += int64_t(gridDim.x) * WARPS) {
+    for (int64_t tile = int64_t(blockIdx.x) * nWarpsCta + warp; tile < nTiles;
+         tile += int64_t(gridDim.x) * nWarpsCta) {
         const int64_t r0 = tile * TILE;
         const int nrows = int(min(int64_t(TILE), A.m - r0));
         const bool valid = lane < nrows;
@@ -213,7 +226,10 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
                     for (int j = 0; j < 4; ++j) atomicAdd(xt + a * A.nDof + j, v[5 + 4 * a + j]);
             }
 #pragma unroll
-            for (int j = 0; j < N_INSTR; ++j) atomicAdd(xIns + c[j], v[17 + j]);
+            for (int j = 0; j < N_INSTR; ++j) {
+                if (PRIV && c[j] < nSm) atomicAdd(sIns + c[j], v[17 + j]);
+                else atomicAdd(xIns + c[j], v[17 + j]);
+            }
         }
         // ---- gamma: fixed-order warp sum, accumulated per warp over its tiles
         gsum += warp_sum(v[23]);
@@ -258,8 +274,14 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
     __syncthreads();
     if (threadIdx.x == 0) {
         double g = 0.0;
-        for (int w = 0; w < WARPS; ++w) g += red[w];
+        for (int w = 0; w < nWarpsCta; ++w) g += red[w];
         globPartial[blockIdx.x] = g;
+    }
+    if (PRIV) {   // flush the private table (the barrier above ordered the ATOMS before these reads)
+        for (int c = threadIdx.x; c < nSm; c += PRIV_THREADS) {
+            const double t = sIns[c];
+            if (t != 0.0) atomicAdd(xIns + c, t);
+        }
     }
 }
 
@@ -353,6 +375,11 @@ k_aprod2_att(MatView A, const double *__restrict__ y, double *__restrict__ x,
         const bool valid = lane < nrows;
         const int64_t t = t0 + (valid ? lane : nrows - 1);
         const int32_t sv = __ldcs(A.sT + t);
+        // The gathers below land anywhere in this block's slice of y.  Pull the NEXT block's slice
+        // into L2 linearly while this block is processed (one 32-byte sector per 4 rows): first touches
+        // that arrive together are not merged by L2 and would each go to DRAM (measured).
+        if (!SQUARE && (lane & 3) == 0 && t + (int64_t(1) << ATT_BLOCK_BITS) < A.m)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(y + t + (int64_t(1) << ATT_BLOCK_BITS)));
         double yv = 0.0;
         if (valid) yv = SQUARE ? 1.0 : cy * __ldg(y + __ldcs(A.permT + t));
         double v[N_ATT];
@@ -378,8 +405,10 @@ k_aprod2_att(MatView A, const double *__restrict__ y, double *__restrict__ x,
         } else {
             const int segStart = 31 - __clz(heads & (0xffffffffu >> (31 - lane)));
             const int dist = lane - segStart;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
+            // scan steps only up to the longest segment of this tile (segments are short when the
+            // block holds few rows per attitude start)
+            const int maxDist = __reduce_max_sync(0xffffffffu, dist);
+            for (int d = 1; d <= maxDist; d <<= 1) {
 #pragma unroll
                 for (int k = 0; k < N_ATT; ++k) {
                     const double t2 = __shfl_up_sync(0xffffffffu, v[k], d);
