@@ -43,7 +43,7 @@ def parse():
     ap.add_argument("--workload", default="medium")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--kernel-reps", type=int, default=5)
+    ap.add_argument("--kernel-reps", type=int, default=20)
     return ap.parse_args()
 
 
@@ -102,7 +102,7 @@ def build_on_device(cfg, G, dev, torch, synth):
     rp = synth.star_rowptr(cfg, dev)
     m = int(rp[-1])
     step = 20_000 if cfg.obs_per_star > 0 else 50_000
-    noise = torch.empty(m, dtype=torch.float64, device=dev)
+    noise = torch.zeros(m + cfg.n_con, dtype=torch.float64, device=dev)   # constraint rows: b_c = A_c x_true
     for s0 in range(0, cfg.n_stars, step):
         s1 = min(s0 + step, cfg.n_stars)
         part = synth.generate_rows(cfg, s0, s1, dev, rp)
@@ -112,7 +112,9 @@ def build_on_device(cfg, G, dev, torch, synth):
                           part["matrixIndexAtt"].contiguous(), part["instrCol"].contiguous(),
                           part["noise"].contiguous())
         del part
-    G.gsr_upload_finish()
+    G.gsr_upload_finish(noise[m:].contiguous() if cfg.n_con else None)
+    if cfg.n_con:
+        G.gsr_upload_constraints(*synth.constraints(cfg, dev))
     xt = synth.x_true(cfg, dev)
     G.gsr_aprod1(xt, noise)             # noise <- noise + A x_true
     G.gsr_set_b(noise)
@@ -191,7 +193,7 @@ def main_ours(args):
     cfg = workload_cfg(args.workload)
     rp = synth.star_rowptr(cfg)
     m = int(rp[-1])
-    G = gsr.Gsr(m, cfg.n_stars, cfg.n_dof_att, cfg.n_instr, device=local)
+    G = gsr.Gsr(m, cfg.n_stars, cfg.n_dof_att, cfg.n_instr, cfg.n_con, cfg.n_con * cfg.con_nnz, device=local)
     t_gen = time.perf_counter()
     build_on_device(cfg, G, dev, torch, synth)
     G.gsr_precondition()
@@ -237,8 +239,16 @@ def main_ours(args):
         gb2a = 112 * m / 1e9
         k["k_aprod2_att"] = {"ms": ms2a, "alg_gb": gb2a, "gbs": gb2a / (ms2a * 1e-3)}
     dom = max((n for n in k if n.startswith("k_")), key=lambda n: k[n]["ms"])
+    traffic = None      # ncu-measured DRAM bytes per launch of the dominant kernel (profiles/r01_traffic.csv)
+    tpath = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+    if os.path.exists(tpath):
+        for ln in open(tpath).read().splitlines()[1:]:
+            w, kn, bts = ln.split(",")
+            if w == args.workload and kn == dom:
+                traffic = float(bts) / 1e9
     roofline = {"bound": "hbm", "kernel": dom, "achieved": k[dom]["gbs"], "peak": peak, "unit": "GB/s",
-                "frac": k[dom]["gbs"] / peak, "traffic": None, "peak_source": peak_src,
+                "frac": k[dom]["gbs"] / peak, "traffic": traffic, "traffic_unit": "GB per launch (ncu dram read+write)",
+                "peak_source": peak_src,
                 "aprod1_plus_aprod2_gbs": (gb1 + gb2) / ((ms1g + ms2g) * 1e-3),
                 "aprod1_plus_aprod2_frac": (gb1 + gb2) / ((ms1g + ms2g) * 1e-3) / peak, "kernels": k}
 

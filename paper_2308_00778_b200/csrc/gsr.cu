@@ -203,10 +203,9 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(cudaEventCreateWithFlags(&h->evSlot[0], cudaEventDisableTiming));
     CK(cudaEventCreateWithFlags(&h->evSlot[1], cudaEventDisableTiming));
 
-    int occ1 = 1, occ2 = 1, occ2m = 1;
+    int occ1 = 1, occ2 = 1;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, k_aprod1, THREADS, 0));
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, k_aprod2<false, true>, THREADS, 0));
-    occ2m = 1;
     h->gridA1 = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ1, 1));
     h->gridA2 = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ2, 1));
     {   // main kernel without attitude: one CTA per SM with a private shared-memory table for the first
@@ -218,7 +217,6 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
         CK(cudaFuncSetAttribute(k_aprod2<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 int(h->nInsSm * sizeof(double))));
         h->gridA2m = gridFor(h->nTiles, PRIV_THREADS / 32, h->smCount);
-        (void)occ2m;
     }
     h->gridVec = gridFor(std::max(h->n, h->mTot), 256 * 4, h->smCount * 8);
     h->gridCon = gridFor(L->n_con, 8, h->smCount * 8);
