@@ -30,6 +30,7 @@ struct gsr_handle {
     double *carryFirst = nullptr, *carryLast = nullptr, *globPartial = nullptr;
     double *sqPartialU = nullptr, *sqPartialV = nullptr, *ddPartial = nullptr;
     double *coefOne = nullptr, *coefTime = nullptr, *trace = nullptr;
+    double *xPack = nullptr;   // attitude unknowns of the current aprod1 operand, [s][axis]
     // time-ordered attitude copy (aprod2 "bucketed scatter") and instrument replicas
     double *attT = nullptr, *insRep = nullptr;
     int32_t *sT = nullptr;
@@ -248,6 +249,7 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(dalloc(&h->sqPartialU, h->gridA1 + h->gridCon));
     CK(dalloc(&h->sqPartialV, h->gridVec));
     CK(dalloc(&h->ddPartial, h->gridVec));
+    CK(dalloc(&h->xPack, 3 * L->n_dof_att));
     CK(dalloc(&h->coefOne, 2));
     CK(dalloc(&h->coefTime, 2));
     CK(dalloc(&h->trace, 5 * GSR_TRACE_CAP));
@@ -299,7 +301,7 @@ int32_t gsr_destroy(gsr_handle *h)
     void *ptrs[] = {h->V, h->b, h->conVal, h->p, h->ia, h->iatt, h->rp, h->conRp, h->conCol, h->ic,
                     h->u, h->v, h->w, h->z, h->var, h->carryFirst, h->carryLast, h->globPartial,
                     h->sqPartialU, h->sqPartialV, h->ddPartial, h->coefOne, h->coefTime, h->trace,
-                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC};
+                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC, h->xPack};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (h->hostS) cudaFreeHost(h->hostS);
@@ -463,8 +465,10 @@ int enqueueAprod1(gsr_handle *h, const double *x, double *y, const double *coef,
                   const int *done, int *nPartial)
 {
     MatView A = view(h);
-    k_aprod1<<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sqPartial, done);
     int nk = 1, np = h->gridA1;
+    k_pack_att<<<h->gridVec, 256, 0, h->stream>>>(A, x, h->xPack, done);
+    ++nk;
+    k_aprod1<<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sqPartial, done, h->xPack);
     if (A.nCon > 0) {
         k_con_aprod1<<<h->gridCon, 256, 0, h->stream>>>(A, x, y, coef, sqPartial ? sqPartial + h->gridA1 : nullptr, done);
         ++nk;
@@ -767,11 +771,12 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
     // bounded operands: u = b, v = 1e-3; coefficients 0.5 keep repeated products finite
     CK(cudaMemcpyAsync(h->u, h->b, size_t(h->mTot) * sizeof(double), cudaMemcpyDeviceToDevice, st));
     k_fill<<<h->gridVec, 256, 0, st>>>(h->v, h->n, 1e-3);
+    k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, nullptr);   // operand of k_aprod1 timed alone
     auto once = [&]() {
         if (which == 1) enqueueAprod1(h, h->v, h->u, h->coefTime, h->sqPartialU, nullptr, nullptr);
         else if (which == 2) enqueueAprod2<false>(h, h->u, h->v, h->coefTime, nullptr, true);
         else if (which == 11)
-            k_aprod1<<<h->gridA1, THREADS, 0, st>>>(A, h->v, h->u, h->coefTime, h->sqPartialU, nullptr);
+            k_aprod1<<<h->gridA1, THREADS, 0, st>>>(A, h->v, h->u, h->coefTime, h->sqPartialU, nullptr, h->xPack);
         else if (which == 13)
             k_aprod2_att<false><<<h->gridAtt, 256, 0, st>>>(A, h->u, h->v, h->coefTime, nullptr);
         else if (h->useAttT)

@@ -103,16 +103,33 @@ __device__ __forceinline__ void load_row(const double *__restrict__ V, int64_t t
 // SURVEY a3).  coef = {cx, cy} in device memory.  Row i <-> one lane; a warp owns 32
 // consecutive rows, a CTA 256.
 // ---------------------------------------------------------------------------------------
+// xPack[3*s + a] = x[offAtt + a*nDof + s]: the attitude unknowns of the operand of aprod1 interleaved by
+// axis, so that the 12 unknowns of a row (3 axes x 4 consecutive starts; the paper keeps the axes N_DFA
+// apart) are one contiguous 96-byte run: 3-4 L2 sectors per row instead of 5-6, and the
+// 12 gathers of a lane fall into one or two L1 lines.  24 MB copied per product (~15 us).
+__global__ void k_pack_att(MatView A, const double *__restrict__ x, double *__restrict__ xPack, const int *done)
+{
+    if (done && *done) return;
+    const int64_t total = A.nDof * 3;
+    for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < total;
+         e += int64_t(gridDim.x) * blockDim.x) {
+        const int64_t s = e / 3;
+        const int a = int(e - s * 3);
+        xPack[e] = x[A.offAtt + a * A.nDof + s];
+    }
+}
+
 __global__ void __launch_bounds__(THREADS, 2)
 k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
-         const double *__restrict__ coef, double *__restrict__ sqPartial, const int *done)
+         const double *__restrict__ coef, double *__restrict__ sqPartial, const int *done,
+         const double *__restrict__ xPack)
 {
     __shared__ double red[32];
     if (done && *done) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const double cx = coef[0], cy = coef[1];
     const int64_t nTiles = (A.m + TILE - 1) / TILE;
-    const double *xAtt = x + A.offAtt, *xIns = x + A.offInstr;
+    const double *xIns = x + A.offInstr;
     const double xg = __ldg(x + A.offGlob);
     double sq = 0.0;
     for (int64_t tile = int64_t(blockIdx.x) * WARPS + warp; tile < nTiles;
@@ -124,7 +141,7 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
             double v[N_PAR];
             load_row<true>(A.V, tile, lane, v);
             const double *xa = x + __ldcs(A.ia + i);
-            const double *xt = xAtt + __ldcs(A.iatt + i);
+            const int64_t iatt = __ldcs(A.iatt + i);
             const int32_t *icp = A.ic + tile * (N_INSTR * TILE) + lane;
             int32_t c[N_INSTR];
 #pragma unroll
@@ -132,11 +149,13 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
             double sum = 0.0;
 #pragma unroll
             for (int k = 0; k < N_ASTRO; ++k) sum = fma(v[k], __ldg(xa + k), sum);
-#pragma unroll
-            for (int a = 0; a < 3; ++a)
+            {
+                const double *xp = xPack + 3 * iatt;
 #pragma unroll
                 for (int j = 0; j < 4; ++j)
-                    sum = fma(v[5 + 4 * a + j], __ldg(xt + a * A.nDof + j), sum);
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) sum = fma(v[5 + 4 * a + j], __ldg(xp + 3 * j + a), sum);
+            }
 #pragma unroll
             for (int j = 0; j < N_INSTR; ++j) sum = fma(v[17 + j], __ldg(xIns + c[j]), sum);
             sum = fma(v[23], xg, sum);
