@@ -318,3 +318,65 @@ def test_chunked_device_upload_equals_whole_upload():
                               dev(d["matrixIndexAtt"][r0:r1]), dev(d["instrCol"][r0:r1]), dev(b[r0:r1]))
         G.gsr_upload_finish()
         check_aprods(S, G)
+
+
+def test_two_attitude_blocks_and_mixed_instrument_table():
+    """2.2 M rows: more than one 2^21-row block of the block-time-ordered attitude copy, and 30,000 instrument
+    columns: more than the per-CTA shared-memory table holds, so both the ATOMS and the RED path run."""
+    cfg = synth.SynthConfig("blocks2", 22_000, 4_000, 30_000, obs_per_star=100, seed=11)
+    S, d = oracle_system(cfg)
+    assert S.m > (1 << 21)
+    b = make_b(S, d)
+    with make_gpu(S, d, b) as G:
+        check_aprods(S, G)
+        v, _ = G.gsr_get_values()
+        assert np.array_equal(v.cpu().numpy(), d["values"])                     # layout round trip, bit-exact
+        G.gsr_precondition()
+        S.precondition()
+        check_aprods(S, G, seed=1)
+        r = G.gsr_lsqr(8, 0.0, 0.0)
+        ro = S.lsqr(b, 8, 0.0, 0.0)
+        assert r.istop == ro.istop == 7 and r.itn == ro.itn == 8
+        xg = r.x.cpu().numpy()
+        assert np.linalg.norm(xg - ro.x) <= X_TOL * np.linalg.norm(ro.x)
+
+
+def test_medium_full_size_sampled():
+    """BASELINE configs[2] at full size (200 M rows) in the launch configuration bench.py times: sampled rows of
+    aprod1 and sampled stars of aprod2 against the oracle on the same bytes (rows regenerated on the device and
+    copied out), plus the adjoint identity <A x, y> = <x, A^T y> over the whole system."""
+    import bench
+    gsr = gsr_mod()
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90e9:
+        pytest.skip("needs ~80 GB of free HBM")
+    cfg = synth.medium()
+    dv = torch.device("cuda", 0)
+    rp = synth.star_rowptr(cfg)
+    m = int(rp[-1])
+    with gsr.Gsr(m, cfg.n_stars, cfg.n_dof_att, cfg.n_instr) as G:
+        bench.build_on_device(cfg, G, dv, torch, synth)
+        g = torch.Generator(device="cuda").manual_seed(5)
+        x = torch.randn(G.n, dtype=torch.float64, device=dv, generator=g)
+        y = torch.randn(m, dtype=torch.float64, device=dv, generator=g)
+        y1 = G.gsr_aprod1(x, torch.zeros(m, dtype=torch.float64, device=dv))
+        x2 = G.gsr_aprod2(y, torch.zeros(G.n, dtype=torch.float64, device=dv))
+        lhs, rhs = float(torch.dot(y1, y)), float(torch.dot(x, x2))
+        scale = float(torch.linalg.norm(y1) * torch.linalg.norm(y))
+        assert abs(lhs - rhs) <= 1e-11 * scale, (lhs, rhs, scale)
+        xc = x.cpu().numpy()
+        stars = np.random.default_rng(3).choice(cfg.n_stars, 48, replace=False)
+        stars = np.concatenate([stars, [0, cfg.n_stars - 1, 10485, 10486]])       # ends; stars around a 2^21-row block edge
+        for s in stars:
+            part = synth.generate_rows(cfg, int(s), int(s) + 1, dv, rp.to(dv))
+            r0, nr = part["row0"], part["values"].shape[0]
+            P = {k: part[k].cpu().numpy() for k in ("values", "matrixIndexAstro", "matrixIndexAtt", "instrCol")}
+            So = oracle.OracleSystem(cfg.n_stars, cfg.n_dof_att, cfg.n_instr, P["values"], P["matrixIndexAstro"],
+                                     P["matrixIndexAtt"], P["instrCol"])
+            yo, ab = So.aprod1(xc, np.zeros(nr), want_abs=True)
+            yg = y1[r0:r0 + nr].cpu().numpy()
+            assert np.all(np.abs(yg - yo) <= APROD_TOL * ab + 1e-300), (s, np.max(np.abs(yg - yo) / ab))
+            xo, ab2 = So.aprod2(y[r0:r0 + nr].cpu().numpy(), np.zeros(G.n), want_abs=True)
+            sl = slice(5 * int(s), 5 * int(s) + 5)                               # all rows of the star are in So
+            xg = x2[sl].cpu().numpy()
+            assert np.all(np.abs(xg - xo[sl]) <= APROD_TOL * ab2[sl] + 1e-300), (s, xg, xo[sl])
