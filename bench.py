@@ -170,6 +170,17 @@ def main_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def aggregate_replicas(loop_ms_rank, steps, world, dev, torch, dist):
+    """Replicas only: every rank runs the same workload on its own GPU.  The job's time is the
+    MAX of the ranks' device times (one all-reduce of a scalar, outside the timed region); the job's
+    throughput is all ranks' iterations over that time."""
+    t = torch.tensor([loop_ms_rank], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms = float(t.item())
+    return ms, world * steps / (ms * 1e-3)
+
+
 def main_ours(args):
     import torch
     import torch.distributed as dist
@@ -207,11 +218,7 @@ def main_ours(args):
         r = G.gsr_lsqr(args.steps, 0.0, 0.0)
         barrier()
     assert r.itn == args.steps and r.istop == 7, (r.itn, r.istop)
-    loop_ms = torch.tensor([r.loop_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(loop_ms, op=dist.ReduceOp.MAX)
-    loop_ms = float(loop_ms.item())
-    value = world * args.steps / (loop_ms * 1e-3)
+    loop_ms, value = aggregate_replicas(r.loop_ms, args.steps, world, dev, torch, dist)
     xt = synth.x_true(cfg, dev)
     x_err = float(torch.linalg.norm(r.x - xt) / torch.linalg.norm(xt))
     del xt
