@@ -37,6 +37,7 @@ struct gsr_handle {
     uint32_t *permT = nullptr;
     int nRep = 1, gridAtt = 1, perIter = 0, nInsSm = 0;
     bool useAttT = false;
+    bool instrSkewed = false;   // some instrument column holds > 64x the mean number of coefficients
     Scalars *S = nullptr;
     Scalars *hostS = nullptr;           // pinned, 2 slots
     unsigned long long *badDev = nullptr;
@@ -215,7 +216,9 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
         CK(cudaDeviceGetAttribute(&maxSm, cudaDevAttrMaxSharedMemoryPerBlockOptin, L->device));
         const int64_t fit = (int64_t(maxSm) - 1024) / int64_t(sizeof(double));
         h->nInsSm = int(std::max<int64_t>(0, std::min<int64_t>(L->n_instr, fit)));
-        CK(cudaFuncSetAttribute(k_aprod2<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        CK(cudaFuncSetAttribute(k_aprod2<false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                int(h->nInsSm * sizeof(double))));
+        CK(cudaFuncSetAttribute(k_aprod2<false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 int(h->nInsSm * sizeof(double))));
         h->gridA2m = gridFor(h->nTiles, PRIV_THREADS / 32, h->smCount);
     }
@@ -391,6 +394,26 @@ int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail)
     CK(cudaStreamSynchronize(h->stream));
     int rcT = buildAttT(h);
     if (rcT) return rcT;
+    {   // instrument column histogram -> warp-level pre-summation of equal columns in aprod2 or not
+        unsigned int *cnt = nullptr;
+        CK(dalloc(&cnt, h->L.n_instr + 1));
+        CK(cudaMemsetAsync(cnt, 0, sizeof(unsigned int) * size_t(h->L.n_instr + 1), h->stream));
+        if (A.m > 0) {
+            k_instr_hist<<<gridFor(h->nTiles * TILE * N_INSTR, 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(A, cnt);
+            k_max_u32<<<gridFor(h->L.n_instr, 256, h->smCount), 256, 0, h->stream>>>(cnt, h->L.n_instr, cnt + h->L.n_instr);
+        }
+        unsigned int mx = 0;
+        cudaError_t e = cudaMemcpyAsync(&mx, cnt + h->L.n_instr, sizeof(mx), cudaMemcpyDeviceToHost, h->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+        cudaFree(cnt);
+        CK(e);
+        const double mean = double(A.m) * N_INSTR / double(h->L.n_instr);
+        h->instrSkewed = double(mx) > 64.0 * std::max(mean, 1.0);
+        if (h->iterGraph) {   // the captured iteration names the kernel variant
+            cudaGraphExecDestroy(h->iterGraph);
+            h->iterGraph = nullptr;
+        }
+    }
     h->uploaded = true;
     h->preconditioned = false;
     return GSR_OK;
@@ -495,8 +518,12 @@ int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef,
                                                                             h->carryLast, h->globPartial, done);
     } else {
         k_aprod2_att<false><<<h->gridAtt, 256, 0, h->stream>>>(A, y, x, coef, done);
-        k_aprod2<false, false, true><<<h->gridA2m, PRIV_THREADS, size_t(h->nInsSm) * sizeof(double), h->stream>>>(A, y, x, coef, h->carryFirst,
-                                                                             h->carryLast, h->globPartial, done);
+        if (h->instrSkewed)
+            k_aprod2<false, false, true, true><<<h->gridA2m, PRIV_THREADS, size_t(h->nInsSm) * sizeof(double), h->stream>>>(
+                A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done);
+        else
+            k_aprod2<false, false, true, false><<<h->gridA2m, PRIV_THREADS, size_t(h->nInsSm) * sizeof(double), h->stream>>>(
+                A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done);
         ++nk;
     }
     k_astro_fixup<<<h->gridFix, 256, 0, h->stream>>>(A, x, coef, h->carryFirst, h->carryLast, h->globPartial,
@@ -779,9 +806,12 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
             k_aprod1<<<h->gridA1, THREADS, 0, st>>>(A, h->v, h->u, h->coefTime, h->sqPartialU, nullptr, h->xPack);
         else if (which == 13)
             k_aprod2_att<false><<<h->gridAtt, 256, 0, st>>>(A, h->u, h->v, h->coefTime, nullptr);
+        else if (h->useAttT && h->instrSkewed)
+            k_aprod2<false, false, true, true><<<h->gridA2m, PRIV_THREADS, size_t(h->nInsSm) * sizeof(double), st>>>(
+                A, h->u, h->v, h->coefTime, h->carryFirst, h->carryLast, h->globPartial, nullptr);
         else if (h->useAttT)
-            k_aprod2<false, false, true><<<h->gridA2m, PRIV_THREADS, size_t(h->nInsSm) * sizeof(double), st>>>(A, h->u, h->v, h->coefTime, h->carryFirst,
-                                                                        h->carryLast, h->globPartial, nullptr);
+            k_aprod2<false, false, true, false><<<h->gridA2m, PRIV_THREADS, size_t(h->nInsSm) * sizeof(double), st>>>(
+                A, h->u, h->v, h->coefTime, h->carryFirst, h->carryLast, h->globPartial, nullptr);
         else
             k_aprod2<false, true><<<h->gridA2, THREADS, 0, st>>>(A, h->u, h->v, h->coefTime, h->carryFirst,
                                                                        h->carryLast, h->globPartial, nullptr);

@@ -190,7 +190,10 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
 // columns are added with REDs; the private table is flushed with one RED per touched column at the end.
 // One CTA of PRIV_THREADS per SM (the table takes most of the shared memory).
 constexpr int PRIV_THREADS = 512;
-template <bool SQUARE, bool ATT_RED, bool PRIV = false>
+// MATCH: sum the lanes of a warp that hit the same instrument column before the atomic (one MATCH.ANY per
+// coefficient: costs 3.6 ms at Medium with uniform columns, saves 2.1 of 6.0 ms on the Zipf columns of Skewed;
+// chosen per upload from the column histogram).
+template <bool SQUARE, bool ATT_RED, bool PRIV = false, bool MATCH = false>
 __global__ void __launch_bounds__(PRIV ? PRIV_THREADS : THREADS, PRIV ? 1 : 2)
 k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
          const double *__restrict__ coef, double *__restrict__ carryFirst,
@@ -231,23 +234,44 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
 #pragma unroll
         for (int k = 0; k < N_PAR; ++k) v[k] = SQUARE ? v[k] * v[k] * yv : v[k] * yv;
 
-        // ---- attitude + instrumental scatter (valid lanes only; invalid lanes hold zeros)
-        if (valid) {
+        // ---- attitude + instrumental scatter (invalid lanes hold zeros and add nothing)
+        if (ATT_RED && valid) {
+            double *xt = xAtt + A.iatt[i];
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) atomicAdd(xt + a * A.nDof + j, v[5 + 4 * a + j]);
+        }
+        {
+            // padded storage: the lanes past the last row read column 0 and a zero coefficient
             const int32_t *icp = A.ic + tile * (N_INSTR * TILE) + lane;
             int32_t c[N_INSTR];
 #pragma unroll
             for (int j = 0; j < N_INSTR; ++j) c[j] = __ldcs(icp + j * TILE);
-            if (ATT_RED) {
-                double *xt = xAtt + A.iatt[i];
-#pragma unroll
-                for (int a = 0; a < 3; ++a)
-#pragma unroll
-                    for (int j = 0; j < 4; ++j) atomicAdd(xt + a * A.nDof + j, v[5 + 4 * a + j]);
-            }
 #pragma unroll
             for (int j = 0; j < N_INSTR; ++j) {
-                if (PRIV && c[j] < nSm) atomicAdd(sIns + c[j], v[17 + j]);
-                else atomicAdd(xIns + c[j], v[17 + j]);
+                // lanes of the warp that hit the same column (hot columns of a skewed distribution) are summed
+                // in lane order first and the lowest lane adds once: no same-address atomics inside a warp
+                double val = v[17 + j];
+                bool add = valid;
+                const unsigned peers = MATCH ? __match_any_sync(0xffffffffu, valid ? c[j] : -1 - lane) : 0u;
+                if (MATCH && __any_sync(0xffffffffu, (peers & (peers - 1)) != 0)) {
+                    const int n = __reduce_max_sync(0xffffffffu, __popc(peers));
+                    unsigned p = peers;
+                    double sum = 0.0;
+                    for (int it = 0; it < n; ++it) {
+                        const int src = p ? __ffs(p) - 1 : lane;
+                        const double t = __shfl_sync(0xffffffffu, val, src);
+                        if (p) sum += t;
+                        p &= p - 1;
+                    }
+                    val = sum;
+                    add = valid && lane == __ffs(peers) - 1;
+                }
+                if (add) {
+                    if (PRIV && c[j] < nSm) atomicAdd(sIns + c[j], val);
+                    else atomicAdd(xIns + c[j], val);
+                }
             }
         }
         // ---- gamma: fixed-order warp sum, accumulated per warp over its tiles
@@ -811,6 +835,26 @@ __global__ void k_export_rows(MatView A, int64_t row0, int64_t cnt, double *__re
         const int64_t r = e / N_PAR;
         out[e] = A.V[vpos(row0 + r, int(e - r * N_PAR))];
     }
+}
+
+// Setup: how uneven is the use of the instrument columns?  cnt[c] = number of coefficients in column c;
+// the largest count against the mean decides whether aprod2 pre-sums equal columns inside a warp.
+__global__ void k_instr_hist(MatView A, unsigned int *__restrict__ cnt)
+{
+    const int64_t total = ((A.m + TILE - 1) / TILE) * (N_INSTR * TILE);
+    for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < total;
+         e += int64_t(gridDim.x) * blockDim.x) {
+        const int64_t i = (e / (N_INSTR * TILE)) * TILE + (e & 31);
+        if (i < A.m) atomicAdd(cnt + A.ic[e], 1u);
+    }
+}
+__global__ void k_max_u32(const unsigned int *__restrict__ cnt, int64_t n, unsigned int *__restrict__ out)
+{
+    unsigned int mx = 0;
+    for (int64_t j = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < n; j += int64_t(gridDim.x) * blockDim.x)
+        mx = max(mx, cnt[j]);
+    mx = __reduce_max_sync(0xffffffffu, mx);
+    if ((threadIdx.x & 31) == 0) atomicMax(out, mx);
 }
 
 __global__ void k_fill(double *__restrict__ a, int64_t n, double v)

@@ -72,6 +72,9 @@ CASES = {
                                                  att_bursts=(5, 1e-2, 0.9), instr_zipf=1.1, seed=7)),
     "powerlaw": dict(cfg=synth.SynthConfig("pl8", 400, 300, 50, obs_powerlaw=(2.0, 8, 200),
                                            att_bursts=(5, 1e-2, 0.9), instr_zipf=1.1, seed=7)),
+    # Zipf(1.1) over 2,000 columns: the hottest column holds ~300x the mean, which switches aprod2 to the
+    # variant that pre-sums equal columns inside a warp (MATCH)
+    "zipf_hot": dict(cfg=synth.SynthConfig("zipf", 300, 200, 2_000, obs_per_star=30, instr_zipf=1.1, seed=9)),
 }
 
 
