@@ -10,6 +10,7 @@
 #include <algorithm>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -31,6 +32,9 @@ struct gsr_handle {
     double *sqPartialU = nullptr, *sqPartialV = nullptr, *ddPartial = nullptr;
     double *coefOne = nullptr, *coefTime = nullptr, *trace = nullptr;
     double *xPack = nullptr;   // attitude unknowns of the current aprod1 operand, [s][axis]
+    double *t = nullptr;       // fused iteration: unscaled A^T u' (n doubles)
+    double *coefRaw = nullptr; // {0, 1}: "x <- 0*x + 1*(A^T y)"
+    int nInsSmFused = 0;       // columns of the shared-memory table in the fused main kernel
     // time-ordered attitude copy (aprod2 "bucketed scatter") and instrument replicas
     double *attT = nullptr, *insRep = nullptr;
     int32_t *sT = nullptr;
@@ -220,6 +224,14 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
                                 int(h->nInsSm * sizeof(double))));
         CK(cudaFuncSetAttribute(k_aprod2<false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 int(h->nInsSm * sizeof(double))));
+        CK(cudaFuncSetAttribute(k_aprod2<false, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                int(h->nInsSm * sizeof(double))));
+        CK(cudaFuncSetAttribute(k_aprod2<false, false, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                int(h->nInsSm * sizeof(double))));
+        // the fused main kernel also gathers x: a 96 KB table leaves the rest of the SM's memory to L1
+        // (measured at Medium: 0 / 4 k / 8 k / 12 k / 16 k / 20 k / 24.5 k columns -> 23.7 / 23.6 / 23.7 / 23.4 / 23.8 /
+        // 24.1 / 28.5 ms per iteration)
+        h->nInsSmFused = std::min(h->nInsSm, 12288);
         h->gridA2m = gridFor(h->nTiles, PRIV_THREADS / 32, h->smCount);
     }
     h->gridVec = gridFor(std::max(h->n, h->mTot), 256 * 4, h->smCount * 8);
@@ -249,7 +261,9 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(dalloc(&h->carryFirst, h->nTiles * N_ASTRO));
     CK(dalloc(&h->carryLast, h->nTiles * N_ASTRO));
     CK(dalloc(&h->globPartial, std::max(h->gridA2, h->gridA2m)));
-    CK(dalloc(&h->sqPartialU, h->gridA1 + h->gridCon));
+    CK(dalloc(&h->sqPartialU, std::max(h->gridA1, h->gridA2m) + h->gridCon));
+    CK(dalloc(&h->t, h->n));
+    CK(dalloc(&h->coefRaw, 2));
     CK(dalloc(&h->sqPartialV, h->gridVec));
     CK(dalloc(&h->ddPartial, h->gridVec));
     CK(dalloc(&h->xPack, 3 * L->n_dof_att));
@@ -285,7 +299,8 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
         }
     }
     CK(cudaMallocHost(reinterpret_cast<void **>(&h->hostS), 2 * sizeof(Scalars)));
-    const double one[2] = {1.0, 1.0}, tm[2] = {0.5, 0.5};
+    const double one[2] = {1.0, 1.0}, tm[2] = {0.5, 0.5}, raw[2] = {0.0, 1.0};
+    CK(cudaMemcpy(h->coefRaw, raw, sizeof(raw), cudaMemcpyHostToDevice));
     CK(cudaMemcpy(h->coefOne, one, sizeof(one), cudaMemcpyHostToDevice));
     CK(cudaMemcpy(h->coefTime, tm, sizeof(tm), cudaMemcpyHostToDevice));
     CK(cudaMemset(h->conRp, 0, sizeof(int64_t) * size_t(L->n_con + 1)));
@@ -304,7 +319,7 @@ int32_t gsr_destroy(gsr_handle *h)
     void *ptrs[] = {h->V, h->b, h->conVal, h->p, h->ia, h->iatt, h->rp, h->conRp, h->conCol, h->ic,
                     h->u, h->v, h->w, h->z, h->var, h->carryFirst, h->carryLast, h->globPartial,
                     h->sqPartialU, h->sqPartialV, h->ddPartial, h->coefOne, h->coefTime, h->trace,
-                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC, h->xPack};
+                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC, h->xPack, h->t, h->coefRaw};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (h->hostS) cudaFreeHost(h->hostS);
@@ -548,9 +563,51 @@ int ensureWork(gsr_handle *h)
     return GSR_OK;
 }
 
+// Fused form of the iteration (k_a1_att in gsr_kernels.cuh): A is streamed once.  Only without constraint
+// rows and with the block-time-ordered attitude copy.
+bool canFuse(const gsr_handle *h)
+{
+    static const bool off = getenv("GSR_NO_FUSE") != nullptr;
+    return !off && h->useAttT && h->L.n_con == 0 && h->L.n_obs > 0;
+}
+
+int enqueueIterationFused(gsr_handle *h)
+{
+    Scalars *S = h->S;
+    const int *done = &S->done;
+    cudaStream_t st = h->stream;
+    MatView A = view(h);
+    A.nInsSm = h->nInsSmFused;
+    const size_t sm = size_t(A.nInsSm) * sizeof(double);
+    // u^ <- a1_cy*u^ + a1_cx*(attitude terms of A v^), on the attitude copy
+    k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, done);
+    k_a1_att<<<h->gridAtt, 256, 0, st>>>(A, h->xPack, h->u, &S->a1_cx, done);
+    // t <- 0 (and the instrument replicas); then the star-ordered pass finishes u^, sums u^2 and scatters the
+    // astro / instr / gamma sections of t = A^T u^
+    k_pre_aprod2<<<h->gridVec, 256, 0, st>>>(h->t, 0, A.n, h->coefRaw, h->insRep, int64_t(h->nRep) * A.nInstr, 2, done);
+    FuseArgs F{h->v, h->u, &S->a1_cx, h->sqPartialU};
+    if (h->instrSkewed)
+        k_aprod2<false, false, true, true, true><<<h->gridA2m, PRIV_THREADS, sm, st>>>(
+            A, h->u, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial, done, F);
+    else
+        k_aprod2<false, false, true, false, true><<<h->gridA2m, PRIV_THREADS, sm, st>>>(
+            A, h->u, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial, done, F);
+    k_scalar<<<1, 256, 0, st>>>(PH_AFTER_APROD1, S, h->sqPartialU, h->gridA2m, nullptr, 0);
+    k_aprod2_att<false><<<h->gridAtt, 256, 0, st>>>(A, h->u, h->t, h->coefRaw, done);
+    k_astro_fixup<<<h->gridFix, 256, 0, st>>>(A, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial,
+                                              h->gridA2m, done);
+    // v^ <- a2_cx*v^ + a2_cy*t  (= A^T u - beta v with the lazy scales), sum v^2
+    k_combine_sumsq<<<h->gridVec, 256, 0, st>>>(h->v, h->t, h->n, &S->a2_cx, h->sqPartialV, done);
+    k_scalar<<<1, 256, 0, st>>>(PH_AFTER_APROD2, S, h->sqPartialV, h->gridVec, nullptr, 0);
+    k_update<<<h->gridVec, 256, 0, st>>>(h->z, h->w, h->v, h->var, h->n, S, h->ddPartial);
+    k_scalar<<<1, 256, 0, st>>>(PH_AFTER_UPDATE, S, h->ddPartial, h->gridVec, h->trace, GSR_TRACE_CAP);
+    return 11;
+}
+
 // One LSQR iteration enqueued on h->stream.  Returns #kernels.
 int enqueueIteration(gsr_handle *h)
 {
+    if (canFuse(h)) return enqueueIterationFused(h);
     Scalars *S = h->S;
     const int *done = &S->done;
     int nk = 0, npU = 0;

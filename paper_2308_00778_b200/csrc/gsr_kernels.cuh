@@ -193,11 +193,21 @@ constexpr int PRIV_THREADS = 512;
 // MATCH: sum the lanes of a warp that hit the same instrument column before the atomic (one MATCH.ANY per
 // coefficient: costs 3.6 ms at Medium with uniform columns, saves 2.1 of 6.0 ms on the Zipf columns of Skewed;
 // chosen per upload from the column histogram).
-template <bool SQUARE, bool ATT_RED, bool PRIV = false, bool MATCH = false>
+// FUSE (fused iteration, see k_a1_att): before the scatter, the row's astro + instr + gamma terms of A*xin are
+// added to yrw (which already holds cy*y + cx*(attitude terms)), the finished y_i is stored, its square summed
+// into sqPartial, and y_i is the value that is scattered.
+struct FuseArgs {
+    const double *xin;     // operand of aprod1 (v), n doubles
+    double *yrw;           // u, read-modify-write
+    const double *coef1;   // {cx, cy} of aprod1 (only cx is used here)
+    double *sqPartial;     // per-CTA partial of sum y^2
+};
+template <bool SQUARE, bool ATT_RED, bool PRIV = false, bool MATCH = false, bool FUSE = false>
 __global__ void __launch_bounds__(PRIV ? PRIV_THREADS : THREADS, PRIV ? 1 : 2)
 k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
          const double *__restrict__ coef, double *__restrict__ carryFirst,
-         double *__restrict__ carryLast, double *__restrict__ globPartial, const int *done)
+         double *__restrict__ carryLast, double *__restrict__ globPartial, const int *done,
+         FuseArgs F = FuseArgs{nullptr, nullptr, nullptr, nullptr})
 {
     __shared__ double red[32];
     extern __shared__ double sIns[];   // PRIV: nInsSm private instrument accumulators
@@ -215,7 +225,9 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         for (int c = threadIdx.x; c < nSm; c += PRIV_THREADS) sIns[c] = 0.0;
         __syncthreads();
     }
-    double gsum = 0.0;
+    double gsum = 0.0, sq = 0.0;
+    const double cx1 = FUSE ? F.coef1[0] : 0.0;
+    const double xg1 = FUSE ? __ldg(F.xin + A.offGlob) : 0.0;
     for (int64_t tile = int64_t(blockIdx.x) * nWarpsCta + warp; tile < nTiles;
          tile += int64_t(gridDim.x) * nWarpsCta) {
         const int64_t r0 = tile * TILE;
@@ -225,12 +237,33 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         double v[N_PAR];
         load_row<ATT_RED>(A.V, tile, valid ? lane : nrows - 1, v);
         const int64_t ia = __ldcs(A.ia + i);
+        // padded storage: the lanes past the last row read column 0 and a zero coefficient
+        const int32_t *icp = A.ic + tile * (N_INSTR * TILE) + lane;
+        int32_t c[N_INSTR];
+#pragma unroll
+        for (int j = 0; j < N_INSTR; ++j) c[j] = __ldcs(icp + j * TILE);
         // astro index of the rows just before and just after the tile (-1: none), fetched with the
         // tile's other loads instead of after the scan
         const int64_t iaBefore = r0 > 0 ? __ldg(A.ia + r0 - 1) : int64_t(-1);
         const int64_t iaAfter = r0 + nrows < A.m ? __ldg(A.ia + r0 + nrows) : int64_t(-1);
         double yv = 0.0;
-        if (valid) yv = SQUARE ? 1.0 : cy * y[i];
+        if (FUSE) {
+            if (valid) {
+                const double *xa = F.xin + ia, *xIn = F.xin + A.offInstr;
+                double sum = 0.0;
+#pragma unroll
+                for (int k = 0; k < N_ASTRO; ++k) sum = fma(v[k], __ldg(xa + k), sum);
+#pragma unroll
+                for (int j = 0; j < N_INSTR; ++j) sum = fma(v[17 + j], __ldg(xIn + c[j]), sum);
+                sum = fma(v[23], xg1, sum);
+                const double yi = fma(cx1, sum, F.yrw[i]);
+                F.yrw[i] = yi;
+                sq = fma(yi, yi, sq);
+                yv = cy * yi;
+            }
+        } else if (valid) {
+            yv = SQUARE ? 1.0 : cy * y[i];
+        }
 #pragma unroll
         for (int k = 0; k < N_PAR; ++k) v[k] = SQUARE ? v[k] * v[k] * yv : v[k] * yv;
 
@@ -243,11 +276,6 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
                 for (int j = 0; j < 4; ++j) atomicAdd(xt + a * A.nDof + j, v[5 + 4 * a + j]);
         }
         {
-            // padded storage: the lanes past the last row read column 0 and a zero coefficient
-            const int32_t *icp = A.ic + tile * (N_INSTR * TILE) + lane;
-            int32_t c[N_INSTR];
-#pragma unroll
-            for (int j = 0; j < N_INSTR; ++j) c[j] = __ldcs(icp + j * TILE);
 #pragma unroll
             for (int j = 0; j < N_INSTR; ++j) {
                 // lanes of the warp that hit the same column (hot columns of a skewed distribution) are summed
@@ -320,6 +348,10 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         for (int w = 0; w < nWarpsCta; ++w) g += red[w];
         globPartial[blockIdx.x] = g;
     }
+    if (FUSE) {
+        const double b = block_sum(sq, red);
+        if (threadIdx.x == 0) F.sqPartial[blockIdx.x] = b;
+    }
     if (PRIV) {   // flush the private table (the barrier above ordered the ATOMS before these reads)
         for (int c = threadIdx.x; c < nSm; c += PRIV_THREADS) {
             const double t = sIns[c];
@@ -386,7 +418,9 @@ __global__ void k_pre_aprod2(double *__restrict__ x, int64_t lo, int64_t hi,
     if (done && *done) return;
     const int64_t tid = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
     const int64_t nth = int64_t(gridDim.x) * blockDim.x;
-    if (prescale) {
+    if (prescale == 2) {   // plain zero fill (the buffer may hold anything)
+        for (int64_t j = lo + tid; j < hi; j += nth) x[j] = 0.0;
+    } else if (prescale) {
         const double c = coef[0];
         for (int64_t j = lo + tid; j < hi; j += nth) x[j] *= c;
     }
@@ -466,6 +500,65 @@ k_aprod2_att(MatView A, const double *__restrict__ y, double *__restrict__ x,
             }
         }
     }
+}
+
+// ---------------------------------------------------------------------------------------
+// Fused LSQR iteration (used by gsr_lsqr when the attitude copy exists and there are no
+// constraint rows): u' = A v - alpha u is row-local and A^T is linear, so A^T u' can be accumulated, unscaled,
+// in the pass that finishes u'; 1/beta is applied afterwards to the n-vector.  Three passes per iteration:
+//   k_a1_att      attitude part of A v on the block-time-ordered copy:  y[row] <- cy*y[row] + cx*(att terms)
+//   k_fused_main  star order: y <- y + cx*(astro + instr + gamma terms) (now complete), sum y^2, and in the
+//                 same pass the astro / instr / gamma sections of t = A^T y
+//   k_aprod2_att  attitude section of t = A^T y (unchanged)
+// then v <- cxv*v + cyv*t with sum v^2 (k_combine_sumsq).  A is streamed once (376 B/row instead of 496).
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_a1_att(MatView A, const double *__restrict__ xPack, double *__restrict__ y,
+         const double *__restrict__ coef, const int *done)
+{
+    if (done && *done) return;
+    const int lane = threadIdx.x & 31;
+    const double cx = coef[0], cy = coef[1];
+    const int64_t nTiles = (A.m + TILE - 1) / TILE;
+    const int64_t warpId = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) >> 5;
+    const int64_t nWarps = (int64_t(gridDim.x) * blockDim.x) >> 5;
+    for (int64_t tile = warpId; tile < nTiles; tile += nWarps) {
+        const int64_t t = tile * TILE + lane;
+        if (t >= A.m) continue;
+        const int32_t sv = __ldcs(A.sT + t);
+        const uint32_t row = __ldcs(A.permT + t);
+        // next block's slice of y into L2, linearly (see k_aprod2_att)
+        if ((lane & 3) == 0 && t + (int64_t(1) << ATT_BLOCK_BITS) < A.m)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(y + t + (int64_t(1) << ATT_BLOCK_BITS)));
+        const double yOld = y[row];
+        const double *xp = xPack + 3 * int64_t(sv);
+        double sum = 0.0;
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+#pragma unroll
+            for (int j = 0; j < 4; ++j)
+                sum = fma(__ldcs(A.attT + int64_t(4 * a + j) * A.m + t), __ldg(xp + 3 * j + a), sum);
+        y[row] = fma(cy, yOld, cx * sum);
+    }
+}
+
+// v <- c[0]*v + c[1]*t and the per-CTA partial of sum v^2 (fixed order for a fixed grid)
+__global__ void __launch_bounds__(256)
+k_combine_sumsq(double *__restrict__ v, const double *__restrict__ t, int64_t n, const double *__restrict__ coef,
+                double *__restrict__ partial, const int *done)
+{
+    __shared__ double red[32];
+    if (done && *done) return;
+    const double cv = coef[0], ct = coef[1];
+    double s = 0.0;
+    for (int64_t j = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; j < n;
+         j += int64_t(gridDim.x) * blockDim.x) {
+        const double r = fma(cv, v[j], ct * t[j]);
+        v[j] = r;
+        s = fma(r, r, s);
+    }
+    s = block_sum(s, red);
+    if (threadIdx.x == 0) partial[blockIdx.x] = s;
 }
 
 // attT[k*m + t] = V[permT[t]*24 + 5 + k]  (re-run after the values are scaled by p)
