@@ -224,13 +224,12 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
                                 int(h->nInsSm * sizeof(double))));
         CK(cudaFuncSetAttribute(k_aprod2<false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 int(h->nInsSm * sizeof(double))));
-        CK(cudaFuncSetAttribute(k_aprod2<false, false, true, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        CK(cudaFuncSetAttribute(k_aprod2<false, false, true, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 int(h->nInsSm * sizeof(double))));
-        CK(cudaFuncSetAttribute(k_aprod2<false, false, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        CK(cudaFuncSetAttribute(k_aprod2<false, false, true, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                 int(h->nInsSm * sizeof(double))));
-        // the fused main kernel also gathers x: a 96 KB table leaves the rest of the SM's memory to L1
-        // (measured at Medium: 0 / 4 k / 8 k / 12 k / 16 k / 20 k / 24.5 k columns -> 23.7 / 23.6 / 23.7 / 23.4 / 23.8 /
-        // 24.1 / 28.5 ms per iteration)
+        // the fused kernel also gathers x: a 96 KB table leaves the rest of the SM's memory to L1 (measured at
+        // Medium: 0 / 3 k / 6 k / 12 k / 18 k / 24.5 k columns -> 22.3 / 22.5 / 22.8 / 22.4 / 22.7 / 24.4 ms per iteration)
         h->nInsSmFused = std::min(h->nInsSm, 12288);
         h->gridA2m = gridFor(h->nTiles, PRIV_THREADS / 32, h->smCount);
     }
@@ -563,7 +562,7 @@ int ensureWork(gsr_handle *h)
     return GSR_OK;
 }
 
-// Fused form of the iteration (k_a1_att in gsr_kernels.cuh): A is streamed once.  Only without constraint
+// Fused form of the iteration (k_combine_sumsq in gsr_kernels.cuh): the row layout is streamed once.  Only without constraint
 // rows and with the block-time-ordered attitude copy.
 bool canFuse(const gsr_handle *h)
 {
@@ -579,18 +578,16 @@ int enqueueIterationFused(gsr_handle *h)
     MatView A = view(h);
     A.nInsSm = h->nInsSmFused;
     const size_t sm = size_t(A.nInsSm) * sizeof(double);
-    // u^ <- a1_cy*u^ + a1_cx*(attitude terms of A v^), on the attitude copy
     k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, done);
-    k_a1_att<<<h->gridAtt, 256, 0, st>>>(A, h->xPack, h->u, &S->a1_cx, done);
-    // t <- 0 (and the instrument replicas); then the star-ordered pass finishes u^, sums u^2 and scatters the
-    // astro / instr / gamma sections of t = A^T u^
+    // t <- 0 (and the instrument replicas); then one star-ordered pass over A: u^ <- a1_cy*u^ + a1_cx*(A v^), sum u^2,
+    // and the astro / instr / gamma sections of t = A^T u^ (unscaled)
     k_pre_aprod2<<<h->gridVec, 256, 0, st>>>(h->t, 0, A.n, h->coefRaw, h->insRep, int64_t(h->nRep) * A.nInstr, 2, done);
-    FuseArgs F{h->v, h->u, &S->a1_cx, h->sqPartialU};
+    FuseArgs F{h->v, h->u, &S->a1_cx, h->sqPartialU, h->xPack};
     if (h->instrSkewed)
-        k_aprod2<false, false, true, true, true><<<h->gridA2m, PRIV_THREADS, sm, st>>>(
+        k_aprod2<false, false, true, true, true, true><<<h->gridA2m, PRIV_THREADS, sm, st>>>(
             A, h->u, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial, done, F);
     else
-        k_aprod2<false, false, true, false, true><<<h->gridA2m, PRIV_THREADS, sm, st>>>(
+        k_aprod2<false, false, true, false, true, true><<<h->gridA2m, PRIV_THREADS, sm, st>>>(
             A, h->u, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial, done, F);
     k_scalar<<<1, 256, 0, st>>>(PH_AFTER_APROD1, S, h->sqPartialU, h->gridA2m, nullptr, 0);
     k_aprod2_att<false><<<h->gridAtt, 256, 0, st>>>(A, h->u, h->t, h->coefRaw, done);
@@ -601,7 +598,7 @@ int enqueueIterationFused(gsr_handle *h)
     k_scalar<<<1, 256, 0, st>>>(PH_AFTER_APROD2, S, h->sqPartialV, h->gridVec, nullptr, 0);
     k_update<<<h->gridVec, 256, 0, st>>>(h->z, h->w, h->v, h->var, h->n, S, h->ddPartial);
     k_scalar<<<1, 256, 0, st>>>(PH_AFTER_UPDATE, S, h->ddPartial, h->gridVec, h->trace, GSR_TRACE_CAP);
-    return 11;
+    return 10;
 }
 
 // One LSQR iteration enqueued on h->stream.  Returns #kernels.

@@ -193,21 +193,24 @@ constexpr int PRIV_THREADS = 512;
 // MATCH: sum the lanes of a warp that hit the same instrument column before the atomic (one MATCH.ANY per
 // coefficient: costs 3.6 ms at Medium with uniform columns, saves 2.1 of 6.0 ms on the Zipf columns of Skewed;
 // chosen per upload from the column histogram).
-// FUSE (fused iteration, see k_a1_att): before the scatter, the row's astro + instr + gamma terms of A*xin are
+// FUSE (fused iteration, see k_combine_sumsq): before the scatter, the row's astro + instr + gamma terms of A*xin are
 // added to yrw (which already holds cy*y + cx*(attitude terms)), the finished y_i is stored, its square summed
 // into sqPartial, and y_i is the value that is scattered.
 struct FuseArgs {
     const double *xin;     // operand of aprod1 (v), n doubles
     double *yrw;           // u, read-modify-write
-    const double *coef1;   // {cx, cy} of aprod1 (only cx is used here)
+    const double *coef1;   // {cx, cy} of aprod1
     double *sqPartial;     // per-CTA partial of sum y^2
+    const double *xPack;   // FUSE_ATT: attitude unknowns of xin interleaved by axis (k_pack_att)
 };
-template <bool SQUARE, bool ATT_RED, bool PRIV = false, bool MATCH = false, bool FUSE = false>
+// FUSE_ATT: the attitude terms of A*xin are gathered here too, in star order (whole aprod1 in this pass,
+// y <- cy*y + cx*(A xin)); without it yrw must already hold cy*y + cx*(attitude terms).
+template <bool SQUARE, bool ATT_RED, bool PRIV = false, bool MATCH = false, bool FUSE = false, bool FUSE_ATT = false>
 __global__ void __launch_bounds__(PRIV ? PRIV_THREADS : THREADS, PRIV ? 1 : 2)
 k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
          const double *__restrict__ coef, double *__restrict__ carryFirst,
          double *__restrict__ carryLast, double *__restrict__ globPartial, const int *done,
-         FuseArgs F = FuseArgs{nullptr, nullptr, nullptr, nullptr})
+         FuseArgs F = FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr})
 {
     __shared__ double red[32];
     extern __shared__ double sIns[];   // PRIV: nInsSm private instrument accumulators
@@ -235,7 +238,7 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         const bool valid = lane < nrows;
         const int64_t i = r0 + (valid ? lane : nrows - 1);
         double v[N_PAR];
-        load_row<ATT_RED>(A.V, tile, valid ? lane : nrows - 1, v);
+        load_row<ATT_RED || FUSE_ATT>(A.V, tile, valid ? lane : nrows - 1, v);
         const int64_t ia = __ldcs(A.ia + i);
         // padded storage: the lanes past the last row read column 0 and a zero coefficient
         const int32_t *icp = A.ic + tile * (N_INSTR * TILE) + lane;
@@ -256,7 +259,16 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
 #pragma unroll
                 for (int j = 0; j < N_INSTR; ++j) sum = fma(v[17 + j], __ldg(xIn + c[j]), sum);
                 sum = fma(v[23], xg1, sum);
-                const double yi = fma(cx1, sum, F.yrw[i]);
+                double yOld = F.yrw[i];
+                if (FUSE_ATT) {
+                    const double *xp = F.xPack + 3 * __ldcs(A.iatt + i);
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+#pragma unroll
+                        for (int a = 0; a < 3; ++a) sum = fma(v[5 + 4 * a + j], __ldg(xp + 3 * j + a), sum);
+                    yOld *= F.coef1[1];
+                }
+                const double yi = fma(cx1, sum, yOld);
                 F.yrw[i] = yi;
                 sq = fma(yi, yi, sq);
                 yv = cy * yi;
@@ -503,45 +515,13 @@ k_aprod2_att(MatView A, const double *__restrict__ y, double *__restrict__ x,
 }
 
 // ---------------------------------------------------------------------------------------
-// Fused LSQR iteration (used by gsr_lsqr when the attitude copy exists and there are no
-// constraint rows): u' = A v - alpha u is row-local and A^T is linear, so A^T u' can be accumulated, unscaled,
-// in the pass that finishes u'; 1/beta is applied afterwards to the n-vector.  Three passes per iteration:
-//   k_a1_att      attitude part of A v on the block-time-ordered copy:  y[row] <- cy*y[row] + cx*(att terms)
-//   k_fused_main  star order: y <- y + cx*(astro + instr + gamma terms) (now complete), sum y^2, and in the
-//                 same pass the astro / instr / gamma sections of t = A^T y
-//   k_aprod2_att  attitude section of t = A^T y (unchanged)
-// then v <- cxv*v + cyv*t with sum v^2 (k_combine_sumsq).  A is streamed once (376 B/row instead of 496).
+// Fused LSQR iteration (gsr_lsqr uses it when the attitude copy exists and there are no
+// constraint rows): u' = A v - alpha u is row-local and A^T is linear, so the astro / instr / gamma sections of
+// t = A^T u' are accumulated, unscaled, by the star-ordered pass that computes u' (k_aprod2<.., FUSE, FUSE_ATT>:
+// the whole of aprod1 plus the scatter of aprod2's main kernel on one read of A); k_aprod2_att adds the
+// attitude section of t; then v <- cxv*v + cyv*t with sum v^2 (k_combine_sumsq), which applies 1/beta.
+// Per iteration 248 + 112 B/row are streamed instead of 248 + 136 + 112.
 // ---------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
-k_a1_att(MatView A, const double *__restrict__ xPack, double *__restrict__ y,
-         const double *__restrict__ coef, const int *done)
-{
-    if (done && *done) return;
-    const int lane = threadIdx.x & 31;
-    const double cx = coef[0], cy = coef[1];
-    const int64_t nTiles = (A.m + TILE - 1) / TILE;
-    const int64_t warpId = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) >> 5;
-    const int64_t nWarps = (int64_t(gridDim.x) * blockDim.x) >> 5;
-    for (int64_t tile = warpId; tile < nTiles; tile += nWarps) {
-        const int64_t t = tile * TILE + lane;
-        if (t >= A.m) continue;
-        const int32_t sv = __ldcs(A.sT + t);
-        const uint32_t row = __ldcs(A.permT + t);
-        // next block's slice of y into L2, linearly (see k_aprod2_att)
-        if ((lane & 3) == 0 && t + (int64_t(1) << ATT_BLOCK_BITS) < A.m)
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(y + t + (int64_t(1) << ATT_BLOCK_BITS)));
-        const double yOld = y[row];
-        const double *xp = xPack + 3 * int64_t(sv);
-        double sum = 0.0;
-#pragma unroll
-        for (int a = 0; a < 3; ++a)
-#pragma unroll
-            for (int j = 0; j < 4; ++j)
-                sum = fma(__ldcs(A.attT + int64_t(4 * a + j) * A.m + t), __ldg(xp + 3 * j + a), sum);
-        y[row] = fma(cy, yOld, cx * sum);
-    }
-}
-
 // v <- c[0]*v + c[1]*t and the per-CTA partial of sum v^2 (fixed order for a fixed grid)
 __global__ void __launch_bounds__(256)
 k_combine_sumsq(double *__restrict__ v, const double *__restrict__ t, int64_t n, const double *__restrict__ coef,
