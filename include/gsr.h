@@ -179,7 +179,9 @@ int32_t gsr_last_timing(gsr_handle *h, double *loop_ms, int64_t *kernel_launches
  * warm-up launch, and return the mean device time per launch in milliseconds (CUDA events on the
  * handle's stream).  which = 1: whole aprod1 group; 2: whole aprod2 group (pre-scale, attitude
  * kernel, main kernel, fix-up, constraints); 11: k_aprod1 alone; 12: k_aprod2 (main) alone;
- * 13: k_aprod2_att alone (GSR_ESTATE if the handle has no time-ordered attitude copy). */
+ * 13: k_aprod2_att alone (GSR_ESTATE if the handle has no time-ordered attitude copy);
+ * 21: the fused pass of gsr_lsqr alone (aprod1 + the astro/instr/gamma scatter of aprod2 on one
+ * read of A; GSR_ESTATE if the handle does not use the fused iteration). */
 int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_per_launch);
 
 #ifdef __cplusplus

@@ -839,7 +839,9 @@ int32_t gsr_last_timing(gsr_handle *h, double *loop_ms, int64_t *kernel_launches
 int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_per_launch)
 {
     if (!h || !ms_per_launch || reps < 1) return GSR_EINVAL;
-    if (which != 1 && which != 2 && which != 11 && which != 12 && which != 13) return fail(h, GSR_EINVAL, "which");
+    if (which != 1 && which != 2 && which != 11 && which != 12 && which != 13 && which != 21)
+        return fail(h, GSR_EINVAL, "which");
+    if (which == 21 && !canFuse(h)) return fail(h, GSR_ESTATE, "this handle does not use the fused iteration");
     if (which == 13 && !h->useAttT) return fail(h, GSR_ESTATE, "no time-ordered attitude copy on this handle");
     int rc = readyCheck(h);
     if (rc) return rc;
@@ -853,6 +855,7 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
     CK(cudaMemcpyAsync(h->u, h->b, size_t(h->mTot) * sizeof(double), cudaMemcpyDeviceToDevice, st));
     k_fill<<<h->gridVec, 256, 0, st>>>(h->v, h->n, 1e-3);
     k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, nullptr);   // operand of k_aprod1 timed alone
+    k_pre_aprod2<<<h->gridVec, 256, 0, st>>>(h->t, 0, A.n, h->coefRaw, h->insRep, int64_t(h->nRep) * A.nInstr, 2, nullptr);
     auto once = [&]() {
         if (which == 1) enqueueAprod1(h, h->v, h->u, h->coefTime, h->sqPartialU, nullptr, nullptr);
         else if (which == 2) enqueueAprod2<false>(h, h->u, h->v, h->coefTime, nullptr, true);
@@ -860,6 +863,18 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
             k_aprod1<<<h->gridA1, THREADS, 0, st>>>(A, h->v, h->u, h->coefTime, h->sqPartialU, nullptr, h->xPack);
         else if (which == 13)
             k_aprod2_att<false><<<h->gridAtt, 256, 0, st>>>(A, h->u, h->v, h->coefTime, nullptr);
+        else if (which == 21) {   // the fused pass of gsr_lsqr alone: u <- 0.5 u + 0.5 A v, t += A^T u (main sections)
+            MatView Af = A;
+            Af.nInsSm = h->nInsSmFused;
+            FuseArgs F{h->v, h->u, h->coefTime, h->sqPartialU, h->xPack};
+            const size_t sm = size_t(Af.nInsSm) * sizeof(double);
+            if (h->instrSkewed)
+                k_aprod2<false, false, true, true, true, true><<<h->gridA2m, PRIV_THREADS, sm, st>>>(
+                    Af, h->u, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial, nullptr, F);
+            else
+                k_aprod2<false, false, true, false, true, true><<<h->gridA2m, PRIV_THREADS, sm, st>>>(
+                    Af, h->u, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial, nullptr, F);
+        }
         else if (h->useAttT && h->instrSkewed)
             k_aprod2<false, false, true, true><<<h->gridA2m, PRIV_THREADS, size_t(h->nInsSm) * sizeof(double), st>>>(
                 A, h->u, h->v, h->coefTime, h->carryFirst, h->carryLast, h->globPartial, nullptr);
