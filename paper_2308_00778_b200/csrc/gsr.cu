@@ -283,8 +283,9 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
         size_t freeB = 0, totB = 0;
         CK(cudaMemGetInfo(&freeB, &totB));
         const size_t need = size_t(m) * (N_ATT * 8 + 4 + 4) + size_t(m) * 12 + (size_t(64) << 20);
+        // GSR_NO_ATT_COPY=1 forces the low-memory path (attitude REDs in k_aprod2, two-product iteration): tests
         if (m > 0 && m < (int64_t(1) << 32) && L->n_dof_att < (int64_t(1) << 31) &&
-            freeB > need + (size_t(2) << 30)) {
+            freeB > need + (size_t(2) << 30) && !getenv("GSR_NO_ATT_COPY")) {
             bool ok = dalloc(&h->attT, m * N_ATT) == cudaSuccess && dalloc(&h->sT, m) == cudaSuccess &&
                       dalloc(&h->permT, m) == cudaSuccess;
             if (!ok) {

@@ -383,3 +383,34 @@ def test_medium_full_size_sampled():
             sl = slice(5 * int(s), 5 * int(s) + 5)                               # all rows of the star are in So
             xg = x2[sl].cpu().numpy()
             assert np.all(np.abs(xg - xo[sl]) <= APROD_TOL * ab2[sl] + 1e-300), (s, xg, xo[sl])
+
+
+@pytest.mark.parametrize("env", ["GSR_NO_ATT_COPY", "GSR_NO_FUSE"])
+def test_fallback_paths(env, monkeypatch):
+    """The low-memory path (no block-time-ordered attitude copy: attitude REDs inside k_aprod2) and the two-product
+    form of the iteration give the same results as the default path.  GSR_NO_FUSE is read once per process, so that
+    case runs in a child process."""
+    import subprocess
+    import sys
+    code = (
+        "import numpy as np, sys; sys.path.insert(0, 'tests')\n"
+        "import test_gpu_parity as T\n"
+        "from helpers import make_b, oracle_system\n"
+        "cfg = T.CASES['ragged_tail']['cfg']\n"
+        "S, d = oracle_system(cfg); b = make_b(S, d)\n"
+        "G = T.make_gpu(S, d, b); T.check_aprods(S, G)\n"
+        "G.gsr_precondition(); S.precondition()\n"
+        "r = G.gsr_lsqr(40, 0.0, 0.0); ro = S.lsqr(b, 40, 0.0, 0.0)\n"
+        "x = r.x.cpu().numpy()\n"
+        "assert r.itn == ro.itn == 40 and r.istop == ro.istop == 7\n"
+        "assert np.linalg.norm(x - ro.x) <= T.X_TOL * np.linalg.norm(ro.x)\n"
+        "import pytest\n"
+        "which = 13 if '%s' == 'GSR_NO_ATT_COPY' else 21   # kernels that exist only on the default path\n"
+        "with pytest.raises(T.gsr_mod().GsrError): G.gsr_time_aprod(which, 1)\n"
+        "print('ok')\n" % env)
+    import os
+    envv = dict(os.environ, **{env: "1"})
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    p = subprocess.run([sys.executable, "-c", code], cwd=root, env=envv, capture_output=True, text=True, timeout=600)
+    assert p.returncode == 0, p.stderr[-2000:]
+    assert p.stdout.split()[-1] == "ok"
