@@ -132,7 +132,7 @@ def oracle_sample_run(cfg, steps, warmup):
     import oracle
     from paper_2308_00778_b200 import synth
     full_rows = int(synth.star_rowptr(cfg)[-1])
-    target_rows = 1_500_000
+    target_rows = 3_000_000
     ns = max(1, min(cfg.n_stars, int(cfg.n_stars * target_rows / max(full_rows, 1))))
     sub = dataclasses.replace(cfg, name=cfg.name + "_sample", n_stars=ns, n_con=0, con_nnz=0)
     d = {k: v.numpy() for k, v in synth.generate(sub).items()}
@@ -287,7 +287,7 @@ def main_ours(args):
     if not args.no_e2e and rank == 0:
         line["e2e"] = e2e_run(args, cfg, G, dev, torch, synth, gsr)
     if not args.no_cpu_baseline and rank == 0 and world == 1:
-        val, _, sample, cores = oracle_sample_run(cfg, 4, 1)
+        val, _, sample, cores = oracle_sample_run(cfg, 10, 1)
         line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
     G.close()
     if rank == 0:
