@@ -202,7 +202,14 @@ struct FuseArgs {
     const double *coef1;   // {cx, cy} of aprod1
     double *sqPartial;     // per-CTA partial of sum y^2
     const double *xPack;   // FUSE_ATT: attitude unknowns of xin interleaved by axis (k_pack_att)
+    cudaTextureObject_t texX;     // 0, or xin as a linear texture of int2 (gathers through the TEX path)
+    cudaTextureObject_t texPack;  // 0, or xPack likewise
 };
+__device__ __forceinline__ double tex_f64(cudaTextureObject_t t, int64_t idx)
+{
+    const int2 q = tex1Dfetch<int2>(t, int(idx));
+    return __hiloint2double(q.y, q.x);
+}
 // FUSE_ATT: the attitude terms of A*xin are gathered here too, in star order (whole aprod1 in this pass,
 // y <- cy*y + cx*(A xin)); without it yrw must already hold cy*y + cx*(attitude terms).
 template <bool SQUARE, bool ATT_RED, bool PRIV = false, bool MATCH = false, bool FUSE = false, bool FUSE_ATT = false>
@@ -210,7 +217,7 @@ __global__ void __launch_bounds__(PRIV ? PRIV_THREADS : THREADS, PRIV ? 1 : 2)
 k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
          const double *__restrict__ coef, double *__restrict__ carryFirst,
          double *__restrict__ carryLast, double *__restrict__ globPartial, const int *done,
-         FuseArgs F = FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr})
+         FuseArgs F = FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0})
 {
     __shared__ double red[32];
     extern __shared__ double sIns[];   // PRIV: nInsSm private instrument accumulators
@@ -257,15 +264,22 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
 #pragma unroll
                 for (int k = 0; k < N_ASTRO; ++k) sum = fma(v[k], __ldg(xa + k), sum);
 #pragma unroll
-                for (int j = 0; j < N_INSTR; ++j) sum = fma(v[17 + j], __ldg(xIn + c[j]), sum);
+                for (int j = 0; j < N_INSTR; ++j) {
+                    const double xj = F.texX ? tex_f64(F.texX, A.offInstr + c[j]) : __ldg(xIn + c[j]);
+                    sum = fma(v[17 + j], xj, sum);
+                }
                 sum = fma(v[23], xg1, sum);
                 double yOld = F.yrw[i];
                 if (FUSE_ATT) {
-                    const double *xp = F.xPack + 3 * __ldcs(A.iatt + i);
+                    const int64_t iattRow = __ldcs(A.iatt + i);
+                    const double *xp = F.xPack + 3 * iattRow;
 #pragma unroll
                     for (int j = 0; j < 4; ++j)
 #pragma unroll
-                        for (int a = 0; a < 3; ++a) sum = fma(v[5 + 4 * a + j], __ldg(xp + 3 * j + a), sum);
+                        for (int a = 0; a < 3; ++a) {
+                            const double xa3 = F.texPack ? tex_f64(F.texPack, 3 * iattRow + 3 * j + a) : __ldg(xp + 3 * j + a);
+                            sum = fma(v[5 + 4 * a + j], xa3, sum);
+                        }
                     yOld *= F.coef1[1];
                 }
                 const double yi = fma(cx1, sum, yOld);
