@@ -156,8 +156,8 @@ int32_t gsr_aprod2(gsr_handle *h, const double *y, double *x);
  * iterations; conlim <= 0 disables the condition-number test.  The whole iteration
  * (both aprods, norms, rotations, vector updates, stop tests) runs on the device;
  * the host only polls istop.  Writes x = p (.) z and se = p (.) se_z.
- * When the handle holds the block-time-ordered attitude copy and the system has no
- * constraint rows, each iteration streams A once: A^T u' is accumulated unscaled in the
+ * When the handle holds the block-time-ordered attitude copy, each iteration streams A's
+ * row layout once: A^T u' is accumulated unscaled in the
  * pass that finishes u' = A v - alpha u, and 1/beta is applied to the n-vector afterwards
  * (same arithmetic up to rounding order; the environment variable GSR_NO_FUSE=1 selects
  * the two-product form gsr_aprod1 / gsr_aprod2 expose). */

@@ -583,12 +583,12 @@ int ensureWork(gsr_handle *h)
     return GSR_OK;
 }
 
-// Fused form of the iteration (k_combine_sumsq in gsr_kernels.cuh): the row layout is streamed once.  Only without constraint
-// rows and with the block-time-ordered attitude copy.
+// Fused form of the iteration (k_combine_sumsq in gsr_kernels.cuh): the row layout is streamed once.  Needs the
+// block-time-ordered attitude copy; constraint rows are handled by their own two small kernels.
 bool canFuse(const gsr_handle *h)
 {
     static const bool off = getenv("GSR_NO_FUSE") != nullptr;
-    return !off && h->useAttT && h->L.n_con == 0 && h->L.n_obs > 0;
+    return !off && h->useAttT && h->L.n_obs > 0;
 }
 
 int enqueueIterationFused(gsr_handle *h)
@@ -610,16 +610,24 @@ int enqueueIterationFused(gsr_handle *h)
     else
         k_aprod2<false, false, true, false, true, true><<<h->gridA2m, PRIV_THREADS, sm, st>>>(
             A, h->u, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial, done, F);
-    k_scalar<<<1, 256, 0, st>>>(PH_AFTER_APROD1, S, h->sqPartialU, h->gridA2m, nullptr, 0);
+    int nk = 10, npU = h->gridA2m;
+    if (A.nCon > 0) {   // constraint rows: their part of u^ and of sum u^2, then (below) of t
+        k_con_aprod1<<<h->gridCon, 256, 0, st>>>(A, h->v, h->u, &S->a1_cx, h->sqPartialU + h->gridA2m, done);
+        npU += h->gridCon;
+        nk += 2;
+    }
+    k_scalar<<<1, 256, 0, st>>>(PH_AFTER_APROD1, S, h->sqPartialU, npU, nullptr, 0);
     k_aprod2_att<false><<<h->gridAtt, 256, 0, st>>>(A, h->u, h->t, h->coefRaw, done);
     k_astro_fixup<<<h->gridFix, 256, 0, st>>>(A, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial,
                                               h->gridA2m, done);
+    // after the fix-up: it overwrites the astro entries of stars cut by a tile edge
+    if (A.nCon > 0) k_con_aprod2<false><<<h->gridCon, 256, 0, st>>>(A, h->u, h->t, h->coefRaw, done);
     // v^ <- a2_cx*v^ + a2_cy*t  (= A^T u - beta v with the lazy scales), sum v^2
     k_combine_sumsq<<<h->gridVec, 256, 0, st>>>(h->v, h->t, h->n, &S->a2_cx, h->sqPartialV, done);
     k_scalar<<<1, 256, 0, st>>>(PH_AFTER_APROD2, S, h->sqPartialV, h->gridVec, nullptr, 0);
     k_update<<<h->gridVec, 256, 0, st>>>(h->z, h->w, h->v, h->var, h->n, S, h->ddPartial);
     k_scalar<<<1, 256, 0, st>>>(PH_AFTER_UPDATE, S, h->ddPartial, h->gridVec, h->trace, GSR_TRACE_CAP);
-    return 10;
+    return nk;
 }
 
 // One LSQR iteration enqueued on h->stream.  Returns #kernels.
