@@ -24,8 +24,9 @@ struct gsr_handle {
     int smCount = 148;
     // system
     double *V = nullptr, *b = nullptr, *conVal = nullptr, *p = nullptr;
-    int64_t *ia = nullptr, *iatt = nullptr, *rp = nullptr, *conRp = nullptr, *conCol = nullptr;
-    int32_t *ic = nullptr;
+    int64_t *rp = nullptr, *conRp = nullptr, *conCol = nullptr;
+    int32_t *ic = nullptr, *star = nullptr, *iatt = nullptr;   // 4-byte row indices
+    int64_t *stageI = nullptr;                                 // upload staging of the two i64 index arrays
     // work
     double *u = nullptr, *v = nullptr, *w = nullptr, *z = nullptr, *var = nullptr;
     double *carryFirst = nullptr, *carryLast = nullptr, *globPartial = nullptr;
@@ -92,7 +93,7 @@ cudaError_t dalloc(T **p, int64_t count)
 MatView view(const gsr_handle *h)
 {
     MatView A;
-    A.V = h->V; A.ia = h->ia; A.iatt = h->iatt; A.ic = h->ic; A.rp = h->rp;
+    A.V = h->V; A.star = h->star; A.iatt = h->iatt; A.ic = h->ic; A.rp = h->rp;
     A.m = h->L.n_obs; A.nStars = h->L.n_stars; A.nDof = h->L.n_dof_att; A.nInstr = h->L.n_instr;
     A.offAtt = 5 * h->L.n_stars;
     A.offInstr = A.offAtt + 3 * h->L.n_dof_att;
@@ -195,6 +196,8 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     if (L->n_obs < 0 || L->n_stars < 1 || L->n_dof_att < 4 || L->n_instr < 6 || L->n_con < 0 ||
         L->n_con_nnz < 0 || (L->n_con == 0 && L->n_con_nnz != 0))
         return fail(h, GSR_EINVAL, "bad sizes");
+    if (L->n_stars >= (int64_t(1) << 31) || L->n_dof_att >= (int64_t(1) << 31) || L->n_instr >= (int64_t(1) << 31))
+        return fail(h, GSR_EINVAL, "n_stars, n_dof_att and n_instr must fit 31 bits (4-byte row indices)");
     h->n = 5 * L->n_stars + 3 * L->n_dof_att + L->n_instr + 1;
     h->mTot = L->n_obs + L->n_con;
     h->nTiles = (L->n_obs + TILE - 1) / TILE;
@@ -245,7 +248,7 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     const int64_t m = L->n_obs;
     // coefficients and instrument columns are stored tile-transposed and padded to whole tiles
     CK(dalloc(&h->V, h->nTiles * TILE * N_PAR));
-    CK(dalloc(&h->ia, m));
+    CK(dalloc(&h->star, m));
     CK(dalloc(&h->iatt, m));
     CK(dalloc(&h->ic, h->nTiles * TILE * N_INSTR));
     if (h->nTiles > 0) {   // zero the padding rows of the last tile
@@ -336,7 +339,7 @@ int32_t gsr_destroy(gsr_handle *h)
     if (h->texV) cudaDestroyTextureObject(h->texV);
     if (h->texPack) cudaDestroyTextureObject(h->texPack);
     if (h->iterGraph) cudaGraphExecDestroy(h->iterGraph);
-    void *ptrs[] = {h->V, h->b, h->conVal, h->p, h->ia, h->iatt, h->rp, h->conRp, h->conCol, h->ic,
+    void *ptrs[] = {h->V, h->b, h->conVal, h->p, h->star, h->iatt, h->stageI, h->rp, h->conRp, h->conCol, h->ic,
                     h->u, h->v, h->w, h->z, h->var, h->carryFirst, h->carryLast, h->globPartial,
                     h->sqPartialU, h->sqPartialV, h->ddPartial, h->coefOne, h->coefTime, h->trace,
                     h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC, h->xPack, h->t, h->coefRaw};
@@ -369,9 +372,24 @@ int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double
     h->uploaded = false;
     h->preconditioned = false;
     const size_t r = size_t(nrows);
-    CK(cudaMemcpyAsync(h->ia + row0, ia, r * sizeof(int64_t), cudaMemcpyDefault, h->stream));
-    CK(cudaMemcpyAsync(h->iatt + row0, iatt, r * sizeof(int64_t), cudaMemcpyDefault, h->stream));
     CK(cudaMemcpyAsync(h->b + row0, b, r * sizeof(double), cudaMemcpyDefault, h->stream));
+    {   // the two i64 index arrays -> 4-byte star / attitude start (device sources in place, host sources staged)
+        const bool devI = nrows > 0 && isDevicePtr(ia) && isDevicePtr(iatt);
+        if (nrows > 0 && !devI && !h->stageI) CK(dalloc(&h->stageI, 2 * STAGE_ROWS));
+        for (int64_t q0 = 0; q0 < nrows; q0 += STAGE_ROWS) {
+            const int64_t cnt = std::min(STAGE_ROWS, nrows - q0);
+            const int64_t *sa = ia + q0, *st = iatt + q0;
+            if (!devI) {
+                CK(cudaMemcpyAsync(h->stageI, sa, size_t(cnt) * sizeof(int64_t), cudaMemcpyDefault, h->stream));
+                CK(cudaMemcpyAsync(h->stageI + STAGE_ROWS, st, size_t(cnt) * sizeof(int64_t), cudaMemcpyDefault, h->stream));
+                sa = h->stageI;
+                st = h->stageI + STAGE_ROWS;
+            }
+            k_ingest_index<<<gridFor(cnt, 256, h->smCount * 16), 256, 0, h->stream>>>(
+                cnt, sa, st, h->L.n_stars, h->L.n_dof_att, h->star + row0 + q0, h->iatt + row0 + q0);
+            CK(cudaGetLastError());
+        }
+    }
     // values and instrCol: row-major in the caller's memory -> tile-transposed on the device.
     // Device sources are read in place; host sources go through a bounded staging buffer.
     MatView A = view(h);
@@ -422,7 +440,7 @@ int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail)
         return fail(h, GSR_EINDEX, "index contract violated at observation row %lld", (long long)bad);
     }
     h->badRow = -1;
-    k_star_rowptr<<<int((h->L.n_stars + 1 + 255) / 256), 256, 0, h->stream>>>(h->ia, A.m, A.nStars, h->rp);
+    k_star_rowptr<<<int((h->L.n_stars + 1 + 255) / 256), 256, 0, h->stream>>>(h->star, A.m, A.nStars, h->rp);
     CK(cudaGetLastError());
     k_fill<<<h->gridVec, 256, 0, h->stream>>>(h->p, h->n, 1.0);
     CK(cudaGetLastError());

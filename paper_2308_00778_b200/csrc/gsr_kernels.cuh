@@ -24,8 +24,8 @@ __host__ __device__ __forceinline__ int64_t cpos(int64_t i, int j) { return ((i 
 // Device view of the uploaded system (A_d, M_i, I_c) in upload layout.
 struct MatView {
     double *V;             // [nTiles*24*32] tile-transposed, see vpos()
-    const int64_t *ia;     // [m] 5*star
-    const int64_t *iatt;   // [m] attitude start s_i (axis 0)
+    const int32_t *star;   // [m] star of the row (matrixIndexAstro / 5; -1: the uploaded value broke its contract)
+    const int32_t *iatt;   // [m] attitude start s_i (axis 0; -1: out of range) -- SURVEY 8(f) NEXT-2: 4-byte indices
     const int32_t *ic;     // [nTiles*6*32] tile-transposed, see cpos()
     const int64_t *rp;     // [nStars+1] derived star row pointer
     int64_t m, nStars, nDof, nInstr;
@@ -140,7 +140,7 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
             const int64_t i = r0 + lane;
             double v[N_PAR];
             load_row<true>(A.V, tile, lane, v);
-            const double *xa = x + __ldcs(A.ia + i);
+            const double *xa = x + 5 * int64_t(__ldcs(A.star + i));
             const int64_t iatt = __ldcs(A.iatt + i);
             const int32_t *icp = A.ic + tile * (N_INSTR * TILE) + lane;
             int32_t c[N_INSTR];
@@ -246,7 +246,7 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         const int64_t i = r0 + (valid ? lane : nrows - 1);
         double v[N_PAR];
         load_row<ATT_RED || FUSE_ATT>(A.V, tile, valid ? lane : nrows - 1, v);
-        const int64_t ia = __ldcs(A.ia + i);
+        const int64_t ia = 5 * int64_t(__ldcs(A.star + i));
         // padded storage: the lanes past the last row read column 0 and a zero coefficient
         const int32_t *icp = A.ic + tile * (N_INSTR * TILE) + lane;
         int32_t c[N_INSTR];
@@ -254,8 +254,8 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         for (int j = 0; j < N_INSTR; ++j) c[j] = __ldcs(icp + j * TILE);
         // astro index of the rows just before and just after the tile (-1: none), fetched with the
         // tile's other loads instead of after the scan
-        const int64_t iaBefore = r0 > 0 ? __ldg(A.ia + r0 - 1) : int64_t(-1);
-        const int64_t iaAfter = r0 + nrows < A.m ? __ldg(A.ia + r0 + nrows) : int64_t(-1);
+        const int64_t iaBefore = r0 > 0 ? 5 * int64_t(__ldg(A.star + r0 - 1)) : int64_t(-1);
+        const int64_t iaAfter = r0 + nrows < A.m ? 5 * int64_t(__ldg(A.star + r0 + nrows)) : int64_t(-1);
         double yv = 0.0;
         if (FUSE) {
             if (valid) {
@@ -567,12 +567,12 @@ __global__ void k_gather_att(MatView A)
 }
 
 // keys / values of the time sort of rows [i0, i0+cnt): key = attitude start (int32), value = row
-__global__ void k_sort_keys(const int64_t *__restrict__ iatt, int64_t i0, int64_t cnt, int32_t *__restrict__ key,
+__global__ void k_sort_keys(const int32_t *__restrict__ iatt, int64_t i0, int64_t cnt, int32_t *__restrict__ key,
                             uint32_t *__restrict__ val)
 {
     for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < cnt;
          q += int64_t(gridDim.x) * blockDim.x) {
-        key[q] = int32_t(iatt[i0 + q]);
+        key[q] = iatt[i0 + q];
         val[q] = uint32_t(i0 + q);
     }
 }
@@ -811,10 +811,10 @@ __global__ void k_validate(MatView A, unsigned long long *badRow)
 {
     for (int64_t i = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; i < A.m;
          i += int64_t(gridDim.x) * blockDim.x) {
-        const int64_t ia = A.ia[i], s = A.iatt[i];
-        bool bad = ia < 0 || ia > 5 * (A.nStars - 1) || (ia % 5) != 0;
-        if (i > 0) bad = bad || A.ia[i - 1] > ia;
-        bad = bad || s < 0 || s > A.nDof - 4;
+        // k_ingest_index stored -1 for a matrixIndexAstro that is not 5*star with star in [0, nStars) and for a
+        // matrixIndexAtt outside [0, nDof-4]
+        bool bad = A.star[i] < 0 || A.iatt[i] < 0;
+        if (i > 0) bad = bad || A.star[i - 1] > A.star[i];
 #pragma unroll
         for (int j = 0; j < N_INSTR; ++j) {
             const int32_t c = A.ic[cpos(i, j)];
@@ -824,19 +824,31 @@ __global__ void k_validate(MatView A, unsigned long long *badRow)
     }
 }
 
-// rp[s] = first row i with ia[i] >= 5*s  (rows sorted by star), s = 0..nStars
-__global__ void k_star_rowptr(const int64_t *__restrict__ ia, int64_t m, int64_t nStars,
+// rp[s] = first row i with star[i] >= s  (rows sorted by star), s = 0..nStars
+__global__ void k_star_rowptr(const int32_t *__restrict__ star, int64_t m, int64_t nStars,
                               int64_t *__restrict__ rp)
 {
     const int64_t s = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
     if (s > nStars) return;
-    const int64_t key = 5 * s;
     int64_t lo = 0, hi = m;
     while (lo < hi) {
         const int64_t mid = (lo + hi) >> 1;
-        if (ia[mid] < key) lo = mid + 1; else hi = mid;
+        if (star[mid] < s) lo = mid + 1; else hi = mid;
     }
     rp[s] = lo;
+}
+
+// Upload: matrixIndexAstro / matrixIndexAtt (i64, "M_i") -> 4-byte star and attitude start;
+// a value that breaks its contract becomes -1 and is reported by k_validate.
+__global__ void k_ingest_index(int64_t cnt, const int64_t *__restrict__ ia, const int64_t *__restrict__ iatt,
+                               int64_t nStars, int64_t nDof, int32_t *__restrict__ star, int32_t *__restrict__ att)
+{
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < cnt;
+         q += int64_t(gridDim.x) * blockDim.x) {
+        const int64_t a = ia[q], s = iatt[q];
+        star[q] = (a >= 0 && a % 5 == 0 && a / 5 < nStars) ? int32_t(a / 5) : -1;
+        att[q] = (s >= 0 && s <= nDof - 4) ? int32_t(s) : -1;
+    }
 }
 
 __global__ void k_validate_con(MatView A, int64_t nnz, unsigned long long *badRow)
@@ -879,7 +891,7 @@ __global__ void k_scale_values(MatView A, const double *__restrict__ p)
         const int64_t i = tile * TILE + (e & 31);
         if (i >= A.m) continue;
         int64_t c;
-        if (k < N_ASTRO) c = A.ia[i] + k;
+        if (k < N_ASTRO) c = 5 * int64_t(A.star[i]) + k;
         else if (k < N_ASTRO + N_ATT) c = A.offAtt + ((k - N_ASTRO) >> 2) * A.nDof + A.iatt[i] + ((k - N_ASTRO) & 3);
         else if (k < N_PAR - 1) c = A.offInstr + A.ic[cpos(i, k - N_ASTRO - N_ATT)];
         else c = A.offGlob;
