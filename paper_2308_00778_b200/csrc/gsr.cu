@@ -739,8 +739,8 @@ int32_t gsr_precondition(gsr_handle *h)
     k_scale_values<<<gridFor(h->nTiles * TILE * N_PAR, 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(A, h->p);
     if (A.nCon > 0)
         k_scale_con_values<<<gridFor(h->L.n_con_nnz, 256, h->smCount * 16), 256, 0, h->stream>>>(A, h->L.n_con_nnz, h->p);
-    if (h->useAttT)   // the time-ordered copy follows the scaled coefficients
-        k_gather_att<<<gridFor(A.m, 256, h->smCount * 16), 256, 0, h->stream>>>(A);
+    if (h->useAttT)   // the time-ordered copy takes the same factors
+        k_scale_attT<<<gridFor(A.m, 256, h->smCount * 16), 256, 0, h->stream>>>(A, h->p);
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(h->stream));
     h->preconditioned = true;

@@ -566,6 +566,21 @@ __global__ void k_gather_att(MatView A)
     }
 }
 
+// After the preconditioner: the copy takes the same factors as the row layout, attT[k][t] *= p[column of (t, k)]
+// (same operands as k_scale_values, so the two stay bit-identical), coalesced instead of a second gather.
+__global__ void k_scale_attT(MatView A, const double *__restrict__ p)
+{
+    for (int64_t t = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; t < A.m;
+         t += int64_t(gridDim.x) * blockDim.x) {
+        const double *pc = p + A.offAtt + A.sT[t];
+#pragma unroll
+        for (int kk = 0; kk < N_ATT; ++kk) {
+            const int64_t e = int64_t(kk) * A.m + t;
+            A.attT[e] = A.attT[e] * pc[(kk >> 2) * A.nDof + (kk & 3)];
+        }
+    }
+}
+
 // keys / values of the time sort of rows [i0, i0+cnt): key = attitude start (int32), value = row
 __global__ void k_sort_keys(const int32_t *__restrict__ iatt, int64_t i0, int64_t cnt, int32_t *__restrict__ key,
                             uint32_t *__restrict__ val)
