@@ -62,9 +62,28 @@ typedef struct {
     int64_t n_con_nnz;  /* non-zeros of the constraint rows                            */
     int32_t n_astro_par, n_att_par, n_instr_par, n_glob_par; /* must be 5, 12, 6, 1    */
     int32_t device;     /* CUDA device ordinal                                         */
-    void *stream;       /* cudaStream_t to run on (e.g. torch's current stream); NULL = the
-                           library creates its own non-blocking stream                */
+    uint32_t flags;     /* bitwise OR of GSR_FLAG_* (0 = default path)                 */
+    void *stream;       /* cudaStream_t of the CALLER (e.g. torch's current stream), or
+                           NULL for the legacy default stream.  The library always runs
+                           on a non-blocking stream of its own; on entry every call
+                           waits (cudaStreamSynchronize) for the work queued on THIS
+                           stream, and it synchronises its own stream before it
+                           returns.  Arguments produced on any other stream must be
+                           complete before the call.                                   */
 } gsr_layout;
+
+/* gsr_layout.flags: per-handle choice of the kernel path (all paths compute the same
+ * products; the tests run each of them against the oracle). */
+#define GSR_FLAG_NO_ATT_COPY 1u /* do not build the block-time-ordered attitude copy
+                                   (+104 B/row of HBM): aprod2 scatters the attitude
+                                   section with atomics and gsr_lsqr runs the
+                                   two-product iteration (low-memory path)            */
+#define GSR_FLAG_NO_FUSE 2u     /* gsr_lsqr runs the two-product iteration (aprod1,
+                                   then aprod2, as Alg. 1 l.17-25) instead of the
+                                   fused single pass over A                            */
+#define GSR_FLAG_NO_TEX 4u      /* fused pass: gather the unknowns with plain loads
+                                   instead of texture fetches (the path taken anyway
+                                   when n >= 2^27 texels)                              */
 
 typedef struct gsr_handle gsr_handle;
 
@@ -101,8 +120,9 @@ int64_t gsr_nrows(const gsr_handle *h);
  *   instrCol         i32 [n_obs*6] in [0, n_instr)
  *   b                f64 [n_obs+n_con] known terms
  * All host or device.  Validates the index contracts on the device (GSR_EINDEX,
- * gsr_bad_row) and derives the star row pointer.  Replaces any earlier upload and
- * clears the preconditioned state. */
+ * gsr_bad_row) and derives the star row pointer.  Replaces any earlier upload,
+ * clears the preconditioned state and DISCARDS the constraint rows (gsr_precondition
+ * scales them in place): call gsr_upload_constraints again after every upload. */
 int32_t gsr_upload(gsr_handle *h, const double *values, const int64_t *matrixIndexAstro,
                    const int64_t *matrixIndexAtt, const int32_t *instrCol, const double *b);
 
@@ -159,7 +179,7 @@ int32_t gsr_aprod2(gsr_handle *h, const double *y, double *x);
  * When the handle holds the block-time-ordered attitude copy, each iteration streams A's
  * row layout once: A^T u' is accumulated unscaled in the
  * pass that finishes u' = A v - alpha u, and 1/beta is applied to the n-vector afterwards
- * (same arithmetic up to rounding order; the environment variable GSR_NO_FUSE=1 selects
+ * (same arithmetic up to rounding order; GSR_FLAG_NO_FUSE in gsr_layout.flags selects
  * the two-product form gsr_aprod1 / gsr_aprod2 expose). */
 int32_t gsr_lsqr(gsr_handle *h, int64_t itnlim, double atol, double btol, double conlim,
                  gsr_result *result);
@@ -170,19 +190,21 @@ int32_t gsr_lsqr(gsr_handle *h, int64_t itnlim, double atol, double btol, double
 #define GSR_TRACE_CAP 4096
 int32_t gsr_get_trace(gsr_handle *h, double *out, int64_t max_itn, int64_t *n_written);
 
+/* Which kernel path this handle uses (after gsr_upload): bit 0 = block-time-ordered
+ * attitude copy in use, bit 1 = fused single-pass iteration, bit 2 = warp-level
+ * pre-summation of equal instrument columns (chosen from the column histogram at
+ * upload), bit 3 = texture gathers in the fused pass, bit 4 = 2-byte instrument
+ * columns on the device. */
+#define GSR_PATH_ATT_COPY 1
+#define GSR_PATH_FUSED 2
+#define GSR_PATH_INSTR_MATCH 4
+#define GSR_PATH_TEX 8
+#define GSR_PATH_IC16 16
+int32_t gsr_path_info(const gsr_handle *h);
+
 /* Device time of the last gsr_lsqr's iteration loop in milliseconds (CUDA events on
  * the handle's stream), and the number of kernels launched in it. */
 int32_t gsr_last_timing(gsr_handle *h, double *loop_ms, int64_t *kernel_launches);
-
-/* Timing hook for bench.py: run `reps` back-to-back launches of one product's kernels with the
- * LSQR coefficients set to 0.5 (bounded operands) on the internal u/v work vectors, after one
- * warm-up launch, and return the mean device time per launch in milliseconds (CUDA events on the
- * handle's stream).  which = 1: whole aprod1 group; 2: whole aprod2 group (pre-scale, attitude
- * kernel, main kernel, fix-up, constraints); 11: k_aprod1 alone; 12: k_aprod2 (main) alone;
- * 13: k_aprod2_att alone (GSR_ESTATE if the handle has no time-ordered attitude copy);
- * 21: the fused pass of gsr_lsqr alone (aprod1 + the astro/instr/gamma scatter of aprod2 on one
- * read of A; GSR_ESTATE if the handle does not use the fused iteration). */
-int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_per_launch);
 
 #ifdef __cplusplus
 }

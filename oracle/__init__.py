@@ -51,7 +51,40 @@ class _Res(C.Structure):
                 ("xnorm", C.c_double)]
 
 
+_SRC_OMP = os.path.join(_HERE, "gsr_oracle_omp.c")
+_LIB_OMP = os.path.join(_HERE, "libgsr_oracle_omp.so")
+
+
+def build_omp(force: bool = False) -> str:
+    """Compile the OpenMP-threaded restatement (bench.py's all-core cpu_baseline only; not the parity oracle)."""
+    if force or not os.path.exists(_LIB_OMP) or os.path.getmtime(_LIB_OMP) < os.path.getmtime(_SRC_OMP):
+        tmp = _LIB_OMP + f".tmp{os.getpid()}"
+        subprocess.check_call(
+            ["gcc", "-O2", "-fopenmp", "-ffp-contract=off", "-fno-fast-math", "-std=c11", "-shared", "-fPIC",
+             "-o", tmp, _SRC_OMP, "-lm"])
+        os.replace(tmp, _LIB_OMP)
+    return _LIB_OMP
+
+
 _lib = None
+_lib_omp = None
+
+
+def _load_omp():
+    global _lib_omp
+    if _lib_omp is None:
+        lib = C.CDLL(build_omp())
+        P = C.c_void_p
+        lib.gsr_omp_threads.restype = C.c_int
+        lib.gsr_omp_set_threads.argtypes = [C.c_int]
+        lib.gsr_omp_aprod1.restype = None
+        lib.gsr_omp_aprod1.argtypes = [P, P, P]
+        lib.gsr_omp_aprod2.restype = None
+        lib.gsr_omp_aprod2.argtypes = [P, P, P]
+        lib.gsr_omp_lsqr.restype = C.c_int
+        lib.gsr_omp_lsqr.argtypes = [P, P, C.c_int64, C.c_double, C.c_double, C.c_double, P, P, P, P]
+        _lib_omp = lib
+    return _lib_omp
 
 
 def _load():
@@ -175,6 +208,40 @@ class OracleSystem:
             raise MemoryError("oracle lsqr allocation failed")
         return LsqrResult(x, se, int(res.istop), int(res.itn), res.anorm, res.acond, res.rnorm,
                           res.arnorm, res.xnorm, None if trace is None else trace[: res.itn])
+
+
+class OmpRunner:
+    """The OpenMP-threaded restatement (gsr_oracle_omp.c) on an OracleSystem's arrays: the paper's section 3.1
+    threading.  For bench.py's all-core cpu_baseline; checked against the oracle in the tests."""
+
+    def __init__(self, S: OracleSystem, threads: int = 0):
+        self.S = S
+        self.lib = _load_omp()
+        self.lib.gsr_omp_set_threads(int(threads) if threads > 0 else (os.cpu_count() or 1))
+        self.threads = int(self.lib.gsr_omp_threads())
+
+    def aprod1(self, x, y):
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        y = np.array(y, dtype=np.float64, copy=True)
+        self.lib.gsr_omp_aprod1(self.S._sp, _ptr(x), _ptr(y))
+        return y
+
+    def aprod2(self, y, x):
+        y = np.ascontiguousarray(y, dtype=np.float64)
+        x = np.array(x, dtype=np.float64, copy=True)
+        self.lib.gsr_omp_aprod2(self.S._sp, _ptr(y), _ptr(x))
+        return x
+
+    def lsqr(self, b, itnlim, atol, btol, conlim=0.0) -> LsqrResult:
+        b = np.ascontiguousarray(b, dtype=np.float64)
+        x = np.zeros(self.S.n)
+        se = np.zeros(self.S.n)
+        res = _Res()
+        rc = self.lib.gsr_omp_lsqr(self.S._sp, _ptr(b), int(itnlim), float(atol), float(btol), float(conlim),
+                                   _ptr(self.S.p), _ptr(x), _ptr(se), C.addressof(res))
+        if rc != 0:
+            raise MemoryError("omp lsqr allocation failed")
+        return LsqrResult(x, se, int(res.istop), int(res.itn), res.anorm, res.acond, res.rnorm, res.arnorm, res.xnorm)
 
 
 def norm(a) -> float:

@@ -11,7 +11,8 @@ import subprocess
 _PKG = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_PKG)
 SRC = [os.path.join(_PKG, "csrc", "gsr.cu")]
-DEPS = SRC + [os.path.join(_PKG, "csrc", "gsr_kernels.cuh"), os.path.join(_ROOT, "include", "gsr.h")]
+DEPS = SRC + [os.path.join(_PKG, "csrc", "gsr_kernels.cuh"), os.path.join(_ROOT, "include", "gsr.h"),
+              os.path.join(_ROOT, "include", "gsr_bench.h")]
 LIB = os.path.join(_PKG, "libgsr.so")
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",

@@ -3,6 +3,7 @@
 // storage, validates uploads, orders the kernels on one stream and captures the LSQR
 // iteration in a CUDA graph.  No CPU arithmetic path exists.
 #include "gsr.h"
+#include "gsr_bench.h"
 #include "gsr_kernels.cuh"
 
 #include <cub/device/device_radix_sort.cuh>
@@ -13,6 +14,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <new>
+#include <string>
 
 using namespace gsr;
 
@@ -26,6 +28,8 @@ struct gsr_handle {
     double *V = nullptr, *b = nullptr, *conVal = nullptr, *p = nullptr;
     int64_t *rp = nullptr, *conRp = nullptr, *conCol = nullptr;
     int32_t *ic = nullptr, *star = nullptr, *iatt = nullptr;   // 4-byte row indices
+    uint16_t *ic16 = nullptr;                                  // instrument columns in 2 bytes when n_instr <= 65536 (ic stays null)
+    int64_t badIngest = -1;                                    // first row whose instrument column did not fit 2 bytes
     int64_t *stageI = nullptr;                                 // upload staging of the two i64 index arrays
     // work
     double *u = nullptr, *v = nullptr, *w = nullptr, *z = nullptr, *var = nullptr;
@@ -37,6 +41,9 @@ struct gsr_handle {
     double *coefRaw = nullptr; // {0, 1}: "x <- 0*x + 1*(A^T y)"
     int nInsSmFused = 0;       // columns of the shared-memory table in the fused main kernel
     cudaTextureObject_t texV = 0, texPack = 0;   // v and xPack as linear int2 textures (fused pass gathers)
+    int nRepAlloc = 1;
+    double *xPack4 = nullptr;  // attitude unknowns as [s][4] for the cooperative gather of the fused pass
+    bool coop = false, attMerge = true;
     // time-ordered attitude copy (aprod2 "bucketed scatter") and instrument replicas
     double *attT = nullptr, *insRep = nullptr;
     int32_t *sT = nullptr;
@@ -93,7 +100,7 @@ cudaError_t dalloc(T **p, int64_t count)
 MatView view(const gsr_handle *h)
 {
     MatView A;
-    A.V = h->V; A.star = h->star; A.iatt = h->iatt; A.ic = h->ic; A.rp = h->rp;
+    A.V = h->V; A.star = h->star; A.iatt = h->iatt; A.ic = h->ic; A.ic16 = h->ic16; A.rp = h->rp;
     A.m = h->L.n_obs; A.nStars = h->L.n_stars; A.nDof = h->L.n_dof_att; A.nInstr = h->L.n_instr;
     A.offAtt = 5 * h->L.n_stars;
     A.offInstr = A.offAtt + 3 * h->L.n_dof_att;
@@ -214,8 +221,8 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(cudaEventCreateWithFlags(&h->evSlot[1], cudaEventDisableTiming));
 
     int occ1 = 1, occ2 = 1;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, k_aprod1, THREADS, 0));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, k_aprod2<false, true>, THREADS, 0));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, k_aprod1<true>, THREADS, 0));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, k_aprod2<true, false, true>, THREADS, 0));
     h->gridA1 = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ1, 1));
     h->gridA2 = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ2, 1));
     {   // main kernel without attitude: one CTA per SM with a private shared-memory table for the first
@@ -224,14 +231,17 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
         CK(cudaDeviceGetAttribute(&maxSm, cudaDevAttrMaxSharedMemoryPerBlockOptin, L->device));
         const int64_t fit = (int64_t(maxSm) - 1024) / int64_t(sizeof(double));
         h->nInsSm = int(std::max<int64_t>(0, std::min<int64_t>(L->n_instr, fit)));
-        CK(cudaFuncSetAttribute(k_aprod2<false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                int(h->nInsSm * sizeof(double))));
-        CK(cudaFuncSetAttribute(k_aprod2<false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                int(h->nInsSm * sizeof(double))));
-        CK(cudaFuncSetAttribute(k_aprod2<false, false, true, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                int(h->nInsSm * sizeof(double))));
-        CK(cudaFuncSetAttribute(k_aprod2<false, false, true, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                int(h->nInsSm * sizeof(double))));
+        const int smB = int(h->nInsSm * sizeof(double));
+        CK(cudaFuncSetAttribute(k_aprod2<false, false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
+        CK(cudaFuncSetAttribute(k_aprod2<false, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
+        CK(cudaFuncSetAttribute(k_aprod2<false, false, false, true, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
+        CK(cudaFuncSetAttribute(k_aprod2<false, false, false, true, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
+        CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
+        CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
+        CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
+        CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
+        CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, false, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
+        CK(cudaFuncSetAttribute(k_aprod2<false, false, false, true, false, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
         // the fused kernel also gathers x: a 96 KB table leaves the rest of the SM's memory to L1 (measured at
         // Medium: 0 / 3 k / 6 k / 12 k / 18 k / 24.5 k columns -> 22.3 / 22.5 / 22.8 / 22.4 / 22.7 / 24.4 ms per iteration)
         h->nInsSmFused = std::min(h->nInsSm, 12288);
@@ -250,10 +260,14 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(dalloc(&h->V, h->nTiles * TILE * N_PAR));
     CK(dalloc(&h->star, m));
     CK(dalloc(&h->iatt, m));
-    CK(dalloc(&h->ic, h->nTiles * TILE * N_INSTR));
+    // instrument columns: 2 bytes each when they fit, else 4
+    const bool ic16 = L->n_instr <= 65536;
+    if (ic16) CK(dalloc(&h->ic16, h->nTiles * TILE * N_INSTR));
+    else CK(dalloc(&h->ic, h->nTiles * TILE * N_INSTR));
     if (h->nTiles > 0) {   // zero the padding rows of the last tile
         CK(cudaMemset(h->V + (h->nTiles - 1) * TILE * N_PAR, 0, sizeof(double) * TILE * N_PAR));
-        CK(cudaMemset(h->ic + (h->nTiles - 1) * TILE * N_INSTR, 0, sizeof(int32_t) * TILE * N_INSTR));
+        if (ic16) CK(cudaMemset(h->ic16 + (h->nTiles - 1) * TILE * N_INSTR, 0, sizeof(uint16_t) * TILE * N_INSTR));
+        else CK(cudaMemset(h->ic + (h->nTiles - 1) * TILE * N_INSTR, 0, sizeof(int32_t) * TILE * N_INSTR));
     }
     CK(dalloc(&h->b, h->mTot));
     CK(dalloc(&h->rp, L->n_stars + 1));
@@ -270,11 +284,13 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(dalloc(&h->sqPartialV, h->gridVec));
     CK(dalloc(&h->ddPartial, h->gridVec));
     CK(dalloc(&h->xPack, 3 * L->n_dof_att));
+    CK(dalloc(&h->xPack4, 4 * L->n_dof_att));
     CK(dalloc(&h->coefOne, 2));
     CK(dalloc(&h->coefTime, 2));
     CK(dalloc(&h->trace, 5 * GSR_TRACE_CAP));
     CK(dalloc(&h->S, 1));
     CK(dalloc(&h->badDev, 1));
+    h->nRepAlloc = h->nRep;
     CK(dalloc(&h->insRep, int64_t(h->nRep) * L->n_instr));
     CK(dalloc(&h->u, h->mTot));
     CK(dalloc(&h->v, h->n));
@@ -296,17 +312,18 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
             td.readMode = cudaReadModeElementType;
             return cudaCreateTextureObject(t, &rd, &td, nullptr);
         };
-        if (h->n < (int64_t(1) << 27)) CK(mk(&h->texV, h->v, h->n));
-        if (3 * L->n_dof_att < (int64_t(1) << 27)) CK(mk(&h->texPack, h->xPack, 3 * L->n_dof_att));
+        const bool tex = !(L->flags & GSR_FLAG_NO_TEX);
+        if (tex && h->n < (int64_t(1) << 27)) CK(mk(&h->texV, h->v, h->n));
+        if (tex && 3 * L->n_dof_att < (int64_t(1) << 27)) CK(mk(&h->texPack, h->xPack, 3 * L->n_dof_att));
     }
     {   // the time-ordered attitude copy costs 104 B/row (+ 12 B/row of sort scratch at upload): take it
-        // only if it fits beside everything else with 2 GB to spare (the 116 GB Large config does not)
+        // only if it fits beside everything else with 2 GB to spare (on a 180 GB B200 even the 116 GB Large config does)
         size_t freeB = 0, totB = 0;
         CK(cudaMemGetInfo(&freeB, &totB));
         const size_t need = size_t(m) * (N_ATT * 8 + 4 + 4) + size_t(m) * 12 + (size_t(64) << 20);
-        // GSR_NO_ATT_COPY=1 forces the low-memory path (attitude REDs in k_aprod2, two-product iteration): tests
+        // GSR_FLAG_NO_ATT_COPY forces the low-memory path (attitude REDs in k_aprod2, two-product iteration)
         if (m > 0 && m < (int64_t(1) << 32) && L->n_dof_att < (int64_t(1) << 31) &&
-            freeB > need + (size_t(2) << 30) && !getenv("GSR_NO_ATT_COPY")) {
+            freeB > need + (size_t(2) << 30) && !(L->flags & GSR_FLAG_NO_ATT_COPY)) {
             bool ok = dalloc(&h->attT, m * N_ATT) == cudaSuccess && dalloc(&h->sT, m) == cudaSuccess &&
                       dalloc(&h->permT, m) == cudaSuccess;
             if (!ok) {
@@ -339,10 +356,10 @@ int32_t gsr_destroy(gsr_handle *h)
     if (h->texV) cudaDestroyTextureObject(h->texV);
     if (h->texPack) cudaDestroyTextureObject(h->texPack);
     if (h->iterGraph) cudaGraphExecDestroy(h->iterGraph);
-    void *ptrs[] = {h->V, h->b, h->conVal, h->p, h->star, h->iatt, h->stageI, h->rp, h->conRp, h->conCol, h->ic,
+    void *ptrs[] = {h->V, h->b, h->conVal, h->p, h->star, h->iatt, h->stageI, h->rp, h->conRp, h->conCol, h->ic, h->ic16,
                     h->u, h->v, h->w, h->z, h->var, h->carryFirst, h->carryLast, h->globPartial,
                     h->sqPartialU, h->sqPartialV, h->ddPartial, h->coefOne, h->coefTime, h->trace,
-                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC, h->xPack, h->t, h->coefRaw};
+                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC, h->xPack, h->t, h->coefRaw, h->xPack4};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (h->hostS) cudaFreeHost(h->hostS);
@@ -371,6 +388,7 @@ int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double
     if (rc) return rc;
     h->uploaded = false;
     h->preconditioned = false;
+    h->conUploaded = false;   // gsr_precondition scaled conVal in place: the constraint rows must come again
     const size_t r = size_t(nrows);
     CK(cudaMemcpyAsync(h->b + row0, b, r * sizeof(double), cudaMemcpyDefault, h->stream));
     {   // the two i64 index arrays -> 4-byte star / attitude start (device sources in place, host sources staged)
@@ -393,6 +411,8 @@ int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double
     // values and instrCol: row-major in the caller's memory -> tile-transposed on the device.
     // Device sources are read in place; host sources go through a bounded staging buffer.
     MatView A = view(h);
+    const unsigned long long noneI = ~0ull;
+    CK(cudaMemcpyAsync(h->badDev, &noneI, sizeof(noneI), cudaMemcpyHostToDevice, h->stream));
     const bool devV = nrows > 0 && isDevicePtr(values), devC = nrows > 0 && isDevicePtr(ic);
     if (nrows > 0 && (!devV || !devC) && !h->stageV) {
         CK(dalloc(&h->stageV, STAGE_ROWS * N_PAR));
@@ -411,10 +431,13 @@ int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double
             srcC = h->stageC;
         }
         k_ingest_rows<<<gridFor(cnt * (N_PAR + N_INSTR), 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(
-            A, h->ic, row0 + q0, cnt, srcV, srcC);
+            A, h->ic, h->ic16, row0 + q0, cnt, srcV, srcC, h->badDev);
         CK(cudaGetLastError());
     }
+    unsigned long long badI = noneI;
+    CK(cudaMemcpyAsync(&badI, h->badDev, sizeof(badI), cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
+    if (badI != noneI && (h->badIngest < 0 || int64_t(badI) < h->badIngest)) h->badIngest = int64_t(badI);
     return GSR_OK;
 }
 
@@ -435,6 +458,8 @@ int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail)
     unsigned long long bad = none;
     CK(cudaMemcpyAsync(&bad, h->badDev, sizeof(bad), cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
+    if (h->badIngest >= 0 && (bad == none || h->badIngest < int64_t(bad))) bad = (unsigned long long)h->badIngest;
+    h->badIngest = -1;
     if (bad != none) {
         h->badRow = int64_t(bad);
         return fail(h, GSR_EINDEX, "index contract violated at observation row %lld", (long long)bad);
@@ -536,6 +561,61 @@ int readyCheck(gsr_handle *h)
     return GSR_OK;
 }
 
+void launchAtt(gsr_handle *h, const MatView &A, const double *y, double *x, const double *coef, const int *done)
+{
+    if (h->attMerge) k_aprod2_att<false, true><<<h->gridAtt, 256, 0, h->stream>>>(A, y, x, coef, done);
+    else k_aprod2_att<false, false><<<h->gridAtt, 256, 0, h->stream>>>(A, y, x, coef, done);
+}
+
+// Launches of the aprod kernels, dispatched on the stored width of the instrument columns.
+void launchAprod1(gsr_handle *h, const MatView &A, const double *x, double *y, const double *coef, double *sq,
+                  const int *done)
+{
+    if (h->ic16) k_aprod1<true><<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done, h->xPack);
+    else k_aprod1<false><<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done, h->xPack);
+}
+
+// all sections in one kernel, attitude by REDs (preconditioner pass; low-memory path)
+template <bool SQUARE>
+void launchAprod2Red(gsr_handle *h, const MatView &A, const double *y, double *x, const double *coef, const int *done)
+{
+    if (h->ic16)
+        k_aprod2<true, SQUARE, true><<<h->gridA2, THREADS, 0, h->stream>>>(A, y, x, coef, h->carryFirst, h->carryLast,
+                                                                          h->globPartial, done);
+    else
+        k_aprod2<false, SQUARE, true><<<h->gridA2, THREADS, 0, h->stream>>>(A, y, x, coef, h->carryFirst, h->carryLast,
+                                                                           h->globPartial, done);
+}
+
+// astro / instr / gamma with the shared-memory instrument table; FUSE: the fused pass of gsr_lsqr
+template <bool FUSE>
+void launchAprod2Main(gsr_handle *h, const MatView &A, const double *y, double *x, const double *coef, const int *done,
+                      const FuseArgs &F)
+{
+    size_t sm = size_t(A.nInsSm) * sizeof(double);
+    const int g = h->gridA2m;
+    cudaStream_t st = h->stream;
+    if (FUSE && h->coop && !h->instrSkewed) {   // cooperative attitude gather: exchange buffers behind the table
+        sm = (size_t((A.nInsSm + 1) & ~1) + size_t(PRIV_THREADS / 32) * COOP_WARP) * sizeof(double);
+        if (h->ic16)
+            k_aprod2<true, false, false, true, false, FUSE, FUSE, FUSE><<<g, PRIV_THREADS, sm, st>>>(
+                A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done, F);
+        else
+            k_aprod2<false, false, false, true, false, FUSE, FUSE, FUSE><<<g, PRIV_THREADS, sm, st>>>(
+                A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done, F);
+        return;
+    }
+#define GSR_A2M(IC, MA)                                                                                          \
+    k_aprod2<IC, false, false, true, MA, FUSE, FUSE><<<g, PRIV_THREADS, sm, st>>>(A, y, x, coef, h->carryFirst,    \
+                                                                                 h->carryLast, h->globPartial, done, F)
+    if (h->ic16) {
+        if (h->instrSkewed) GSR_A2M(true, true); else GSR_A2M(true, false);
+    } else {
+        if (h->instrSkewed) GSR_A2M(false, true); else GSR_A2M(false, false);
+    }
+#undef GSR_A2M
+}
+
 // y <- cy*y + cx*(A x); partials of sum y^2 go to sqPartial (or nowhere).  Returns #kernels.
 int enqueueAprod1(gsr_handle *h, const double *x, double *y, const double *coef, double *sqPartial,
                   const int *done, int *nPartial)
@@ -544,7 +624,7 @@ int enqueueAprod1(gsr_handle *h, const double *x, double *y, const double *coef,
     int nk = 1, np = h->gridA1;
     k_pack_att<<<h->gridVec, 256, 0, h->stream>>>(A, x, h->xPack, done);
     ++nk;
-    k_aprod1<<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sqPartial, done, h->xPack);
+    launchAprod1(h, A, x, y, coef, sqPartial, done);
     if (A.nCon > 0) {
         k_con_aprod1<<<h->gridCon, 256, 0, h->stream>>>(A, x, y, coef, sqPartial ? sqPartial + h->gridA1 : nullptr, done);
         ++nk;
@@ -567,16 +647,10 @@ int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef,
     // preconditioner pass (SQUARE) and the low-memory fallback scatter it with REDs in k_aprod2
     const bool attRed = SQUARE || !h->useAttT;
     if (attRed) {
-        k_aprod2<SQUARE, true><<<h->gridA2, THREADS, 0, h->stream>>>(A, y, x, coef, h->carryFirst,
-                                                                            h->carryLast, h->globPartial, done);
+        launchAprod2Red<SQUARE>(h, A, y, x, coef, done);
     } else {
-        k_aprod2_att<false><<<h->gridAtt, 256, 0, h->stream>>>(A, y, x, coef, done);
-        if (h->instrSkewed)
-            k_aprod2<false, false, true, true><<<h->gridA2m, PRIV_THREADS, size_t(h->nInsSm) * sizeof(double), h->stream>>>(
-                A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done);
-        else
-            k_aprod2<false, false, true, false><<<h->gridA2m, PRIV_THREADS, size_t(h->nInsSm) * sizeof(double), h->stream>>>(
-                A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done);
+        launchAtt(h, A, y, x, coef, done);
+        launchAprod2Main<false>(h, A, y, x, coef, done, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, nullptr});
         ++nk;
     }
     k_astro_fixup<<<h->gridFix, 256, 0, h->stream>>>(A, x, coef, h->carryFirst, h->carryLast, h->globPartial,
@@ -589,24 +663,12 @@ int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef,
     return nk;
 }
 
-int ensureWork(gsr_handle *h)
-{
-    if (h->workReady) return GSR_OK;   // allocated by gsr_create
-    CK(dalloc(&h->u, h->mTot));
-    CK(dalloc(&h->v, h->n));
-    CK(dalloc(&h->w, h->n));
-    CK(dalloc(&h->z, h->n));
-    CK(dalloc(&h->var, h->n));
-    h->workReady = true;
-    return GSR_OK;
-}
-
 // Fused form of the iteration (k_combine_sumsq in gsr_kernels.cuh): the row layout is streamed once.  Needs the
 // block-time-ordered attitude copy; constraint rows are handled by their own two small kernels.
+// GSR_FLAG_NO_FUSE (gsr_layout.flags) selects the two-product form.
 bool canFuse(const gsr_handle *h)
 {
-    static const bool off = getenv("GSR_NO_FUSE") != nullptr;
-    return !off && h->useAttT && h->L.n_obs > 0;
+    return !(h->L.flags & GSR_FLAG_NO_FUSE) && h->useAttT && h->L.n_obs > 0;
 }
 
 int enqueueIterationFused(gsr_handle *h)
@@ -616,18 +678,12 @@ int enqueueIterationFused(gsr_handle *h)
     cudaStream_t st = h->stream;
     MatView A = view(h);
     A.nInsSm = h->nInsSmFused;
-    const size_t sm = size_t(A.nInsSm) * sizeof(double);
-    k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, done);
+    k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, done, h->coop ? h->xPack4 : nullptr);
     // t <- 0 (and the instrument replicas); then one star-ordered pass over A: u^ <- a1_cy*u^ + a1_cx*(A v^), sum u^2,
     // and the astro / instr / gamma sections of t = A^T u^ (unscaled)
     k_pre_aprod2<<<h->gridVec, 256, 0, st>>>(h->t, 0, A.n, h->coefRaw, h->insRep, int64_t(h->nRep) * A.nInstr, 2, done);
-    FuseArgs F{h->v, h->u, &S->a1_cx, h->sqPartialU, h->xPack, h->texV, h->texPack};
-    if (h->instrSkewed)
-        k_aprod2<false, false, true, true, true, true><<<h->gridA2m, PRIV_THREADS, sm, st>>>(
-            A, h->u, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial, done, F);
-    else
-        k_aprod2<false, false, true, false, true, true><<<h->gridA2m, PRIV_THREADS, sm, st>>>(
-            A, h->u, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial, done, F);
+    FuseArgs F{h->v, h->u, &S->a1_cx, h->sqPartialU, h->xPack, h->texV, h->texPack, h->xPack4};
+    launchAprod2Main<true>(h, A, h->u, h->t, h->coefRaw, done, F);
     int nk = 10, npU = h->gridA2m;
     if (A.nCon > 0) {   // constraint rows: their part of u^ and of sum u^2, then (below) of t
         k_con_aprod1<<<h->gridCon, 256, 0, st>>>(A, h->v, h->u, &S->a1_cx, h->sqPartialU + h->gridA2m, done);
@@ -635,7 +691,7 @@ int enqueueIterationFused(gsr_handle *h)
         nk += 2;
     }
     k_scalar<<<1, 256, 0, st>>>(PH_AFTER_APROD1, S, h->sqPartialU, npU, nullptr, 0);
-    k_aprod2_att<false><<<h->gridAtt, 256, 0, st>>>(A, h->u, h->t, h->coefRaw, done);
+    launchAtt(h, A, h->u, h->t, h->coefRaw, done);
     k_astro_fixup<<<h->gridFix, 256, 0, st>>>(A, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial,
                                               h->gridA2m, done);
     // after the fix-up: it overwrites the astro entries of stars cut by a tile edge
@@ -780,8 +836,6 @@ int32_t gsr_lsqr(gsr_handle *h, int64_t itnlim, double atol, double btol, double
     if (rc) return rc;
     rc = enter(h);
     if (rc) return rc;
-    rc = ensureWork(h);
-    if (rc) return rc;
     cudaStream_t st = h->stream;
     Scalars init;
     memset(&init, 0, sizeof(init));
@@ -868,11 +922,27 @@ int32_t gsr_get_trace(gsr_handle *h, double *out, int64_t max_itn, int64_t *n_wr
     const int64_t have = std::min<int64_t>(h->lastItn, GSR_TRACE_CAP);
     const int64_t cnt = std::min(have, max_itn);
     const int64_t first = h->lastItn - cnt;   // iteration index (0-based) of the first row returned
-    for (int64_t k = 0; k < cnt; ++k)
-        CK(cudaMemcpy(out + 5 * k, h->trace + 5 * ((first + k) % GSR_TRACE_CAP), 5 * sizeof(double),
-                      cudaMemcpyDeviceToHost));
+    if (cnt > 0) {   // the ring holds iteration k at slot k % CAP: one copy, or two when the range wraps
+        const int64_t s0 = first % GSR_TRACE_CAP;
+        const int64_t c0 = std::min(cnt, GSR_TRACE_CAP - s0);
+        CK(cudaMemcpy(out, h->trace + 5 * s0, size_t(5 * c0) * sizeof(double), cudaMemcpyDeviceToHost));
+        if (cnt > c0)
+            CK(cudaMemcpy(out + 5 * c0, h->trace, size_t(5 * (cnt - c0)) * sizeof(double), cudaMemcpyDeviceToHost));
+    }
     *n_written = cnt;
     return GSR_OK;
+}
+
+int32_t gsr_path_info(const gsr_handle *h)
+{
+    if (!h) return GSR_EINVAL;
+    int32_t r = 0;
+    if (h->useAttT) r |= GSR_PATH_ATT_COPY;
+    if (canFuse(h)) r |= GSR_PATH_FUSED;
+    if (h->instrSkewed) r |= GSR_PATH_INSTR_MATCH;
+    if (h->texV && h->texPack) r |= GSR_PATH_TEX;
+    if (h->ic16) r |= GSR_PATH_IC16;
+    return r;
 }
 
 int32_t gsr_last_timing(gsr_handle *h, double *loop_ms, int64_t *kernel_launches)
@@ -883,54 +953,60 @@ int32_t gsr_last_timing(gsr_handle *h, double *loop_ms, int64_t *kernel_launches
     return GSR_OK;
 }
 
+int32_t gsr_bench_set(gsr_handle *h, const char *key, int64_t value)
+{
+    if (!h || !key) return GSR_EINVAL;
+    const std::string k(key);
+    if (k == "ins_sm_fused" && value >= 0 && value <= h->nInsSm) h->nInsSmFused = int(value);
+    else if (k == "n_rep" && value >= 1 && value <= h->nRepAlloc) h->nRep = int(value);
+    else if (k == "att_ctas_per_sm" && value >= 1 && value <= 16) h->gridAtt = gridFor(h->nTiles, 8, h->smCount * int(value));
+    else if (k == "coop" && (value == 0 || value == 1)) h->coop = value != 0;
+    else if (k == "att_merge" && (value == 0 || value == 1)) h->attMerge = value != 0;
+    else return fail(h, GSR_EINVAL, "gsr_bench_set: unknown key or value out of range: %s = %lld", key, (long long)value);
+    if (h->iterGraph) {
+        cudaGraphExecDestroy(h->iterGraph);
+        h->iterGraph = nullptr;
+    }
+    return GSR_OK;
+}
+
 int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_per_launch)
 {
     if (!h || !ms_per_launch || reps < 1) return GSR_EINVAL;
-    if (which != 1 && which != 2 && which != 11 && which != 12 && which != 13 && which != 21)
+    if (which != GSR_TIME_APROD1_GROUP && which != GSR_TIME_APROD2_GROUP && which != GSR_TIME_K_APROD1 &&
+        which != GSR_TIME_K_APROD2_MAIN && which != GSR_TIME_K_APROD2_ATT && which != GSR_TIME_K_FUSED)
         return fail(h, GSR_EINVAL, "which");
-    if (which == 21 && !canFuse(h)) return fail(h, GSR_ESTATE, "this handle does not use the fused iteration");
-    if (which == 13 && !h->useAttT) return fail(h, GSR_ESTATE, "no time-ordered attitude copy on this handle");
+    if (which == GSR_TIME_K_FUSED && !canFuse(h)) return fail(h, GSR_ESTATE, "this handle does not use the fused iteration");
+    if (which == GSR_TIME_K_APROD2_ATT && !h->useAttT) return fail(h, GSR_ESTATE, "no time-ordered attitude copy on this handle");
     int rc = readyCheck(h);
     if (rc) return rc;
     rc = enter(h);
-    if (rc) return rc;
-    rc = ensureWork(h);
     if (rc) return rc;
     cudaStream_t st = h->stream;
     MatView A = view(h);
     // bounded operands: u = b, v = 1e-3; coefficients 0.5 keep repeated products finite
     CK(cudaMemcpyAsync(h->u, h->b, size_t(h->mTot) * sizeof(double), cudaMemcpyDeviceToDevice, st));
     k_fill<<<h->gridVec, 256, 0, st>>>(h->v, h->n, 1e-3);
-    k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, nullptr);   // operand of k_aprod1 timed alone
+    k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, nullptr);   // operand of k_aprod1 / the fused pass timed alone
+    if (h->coop) k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, nullptr, h->xPack4);
     k_pre_aprod2<<<h->gridVec, 256, 0, st>>>(h->t, 0, A.n, h->coefRaw, h->insRep, int64_t(h->nRep) * A.nInstr, 2, nullptr);
     auto once = [&]() {
-        if (which == 1) enqueueAprod1(h, h->v, h->u, h->coefTime, h->sqPartialU, nullptr, nullptr);
-        else if (which == 2) enqueueAprod2<false>(h, h->u, h->v, h->coefTime, nullptr, true);
-        else if (which == 11)
-            k_aprod1<<<h->gridA1, THREADS, 0, st>>>(A, h->v, h->u, h->coefTime, h->sqPartialU, nullptr, h->xPack);
-        else if (which == 13)
-            k_aprod2_att<false><<<h->gridAtt, 256, 0, st>>>(A, h->u, h->v, h->coefTime, nullptr);
-        else if (which == 21) {   // the fused pass of gsr_lsqr alone: u <- 0.5 u + 0.5 A v, t += A^T u (main sections)
+        if (which == GSR_TIME_APROD1_GROUP) enqueueAprod1(h, h->v, h->u, h->coefTime, h->sqPartialU, nullptr, nullptr);
+        else if (which == GSR_TIME_APROD2_GROUP) enqueueAprod2<false>(h, h->u, h->v, h->coefTime, nullptr, true);
+        else if (which == GSR_TIME_K_APROD1)
+            launchAprod1(h, A, h->v, h->u, h->coefTime, h->sqPartialU, nullptr);
+        else if (which == GSR_TIME_K_APROD2_ATT)
+            launchAtt(h, A, h->u, h->v, h->coefTime, nullptr);
+        else if (which == GSR_TIME_K_FUSED) {   // the fused pass of gsr_lsqr alone: u <- 0.5 u + 0.5 A v, t += A^T u (main sections)
             MatView Af = A;
             Af.nInsSm = h->nInsSmFused;
-            FuseArgs F{h->v, h->u, h->coefTime, h->sqPartialU, h->xPack, h->texV, h->texPack};
-            const size_t sm = size_t(Af.nInsSm) * sizeof(double);
-            if (h->instrSkewed)
-                k_aprod2<false, false, true, true, true, true><<<h->gridA2m, PRIV_THREADS, sm, st>>>(
-                    Af, h->u, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial, nullptr, F);
-            else
-                k_aprod2<false, false, true, false, true, true><<<h->gridA2m, PRIV_THREADS, sm, st>>>(
-                    Af, h->u, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial, nullptr, F);
+            FuseArgs F{h->v, h->u, h->coefTime, h->sqPartialU, h->xPack, h->texV, h->texPack, h->xPack4};
+            launchAprod2Main<true>(h, Af, h->u, h->t, h->coefRaw, nullptr, F);
         }
-        else if (h->useAttT && h->instrSkewed)
-            k_aprod2<false, false, true, true><<<h->gridA2m, PRIV_THREADS, size_t(h->nInsSm) * sizeof(double), st>>>(
-                A, h->u, h->v, h->coefTime, h->carryFirst, h->carryLast, h->globPartial, nullptr);
         else if (h->useAttT)
-            k_aprod2<false, false, true, false><<<h->gridA2m, PRIV_THREADS, size_t(h->nInsSm) * sizeof(double), st>>>(
-                A, h->u, h->v, h->coefTime, h->carryFirst, h->carryLast, h->globPartial, nullptr);
+            launchAprod2Main<false>(h, A, h->u, h->v, h->coefTime, nullptr, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, nullptr});
         else
-            k_aprod2<false, true><<<h->gridA2, THREADS, 0, st>>>(A, h->u, h->v, h->coefTime, h->carryFirst,
-                                                                       h->carryLast, h->globPartial, nullptr);
+            launchAprod2Red<false>(h, A, h->u, h->v, h->coefTime, nullptr);
     };
     once();   // warm-up
     CK(cudaGetLastError());

@@ -11,6 +11,7 @@ constexpr int N_ASTRO = 5, N_ATT = 12, N_INSTR = 6, N_PAR = 24;
 constexpr int TILE = 32;          // rows per warp tile
 constexpr int WARPS = 8;          // warps per CTA of the aprod kernels
 constexpr int THREADS = WARPS * 32;
+constexpr int ATT_WIN = 64;          // coefficients per axis of the per-warp window of k_aprod2_att
 constexpr int ATT_BLOCK_BITS = 21;   // rows per block of the time-ordered attitude copy (2^21)
 
 // Device layout of the coefficients ("tile-transposed"): the 32 rows of a warp tile are stored
@@ -26,7 +27,8 @@ struct MatView {
     double *V;             // [nTiles*24*32] tile-transposed, see vpos()
     const int32_t *star;   // [m] star of the row (matrixIndexAstro / 5; -1: the uploaded value broke its contract)
     const int32_t *iatt;   // [m] attitude start s_i (axis 0; -1: out of range) -- SURVEY 8(f) NEXT-2: 4-byte indices
-    const int32_t *ic;     // [nTiles*6*32] tile-transposed, see cpos()
+    const int32_t *ic;     // [nTiles*6*32] tile-transposed, see cpos(); nullptr when ic16 is in use
+    const uint16_t *ic16;  // the same as 2-byte columns when nInstr <= 65536 (-12 B/row)
     const int64_t *rp;     // [nStars+1] derived star row pointer
     int64_t m, nStars, nDof, nInstr;
     int64_t offAtt, offInstr, offGlob, n;
@@ -97,6 +99,23 @@ __device__ __forceinline__ void load_row(const double *__restrict__ V, int64_t t
     }
 }
 
+// The 6 instrument columns of row (tile, lane): coalesced streaming loads of 2- or 4-byte columns.
+template <bool IC16>
+__device__ __forceinline__ void load_ic(const MatView &A, int64_t tile, int lane, int32_t (&c)[N_INSTR])
+{
+    if (IC16) {
+        const uint16_t *p = A.ic16 + tile * (N_INSTR * TILE) + lane;
+#pragma unroll
+        for (int j = 0; j < N_INSTR; ++j) c[j] = int32_t(__ldcs(p + j * TILE));
+    } else {
+        const int32_t *p = A.ic + tile * (N_INSTR * TILE) + lane;
+#pragma unroll
+        for (int j = 0; j < N_INSTR; ++j) c[j] = __ldcs(p + j * TILE);
+    }
+}
+// setup kernels: one stored instrument column, either width
+__device__ __forceinline__ int32_t ic_at(const MatView &A, int64_t pos) { return A.ic16 ? int32_t(A.ic16[pos]) : A.ic[pos]; }
+
 // ---------------------------------------------------------------------------------------
 // aprod mode 1 (Eq. 2; Algorithm 2):  y <- cy*y + cx*(A x), one pass over A,
 // all four sections in one kernel, plus the per-CTA partial of sum y^2 (Eq. 4's norm, fused:
@@ -107,9 +126,19 @@ __device__ __forceinline__ void load_row(const double *__restrict__ V, int64_t t
 // axis, so that the 12 unknowns of a row (3 axes x 4 consecutive starts; the paper keeps the axes N_DFA
 // apart) are one contiguous 96-byte run: 3-4 L2 sectors per row instead of 5-6, and the
 // 12 gathers of a lane fall into one or two L1 lines.  24 MB copied per product (~15 us).
-__global__ void k_pack_att(MatView A, const double *__restrict__ x, double *__restrict__ xPack, const int *done)
+__global__ void k_pack_att(MatView A, const double *__restrict__ x, double *__restrict__ xPack, const int *done,
+                           double *__restrict__ xPack4 = nullptr)
 {
     if (done && *done) return;
+    if (xPack4) {   // [s][4] = {axis0, axis1, axis2, 0}: the layout the cooperative gather of the fused pass reads
+        for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < A.nDof * 4;
+             e += int64_t(gridDim.x) * blockDim.x) {
+            const int64_t s = e >> 2;
+            const int a = int(e & 3);
+            xPack4[e] = a < 3 ? x[A.offAtt + a * A.nDof + s] : 0.0;
+        }
+        return;
+    }
     const int64_t total = A.nDof * 3;
     for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < total;
          e += int64_t(gridDim.x) * blockDim.x) {
@@ -119,6 +148,7 @@ __global__ void k_pack_att(MatView A, const double *__restrict__ x, double *__re
     }
 }
 
+template <bool IC16>
 __global__ void __launch_bounds__(THREADS, 2)
 k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
          const double *__restrict__ coef, double *__restrict__ sqPartial, const int *done,
@@ -142,10 +172,8 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
             load_row<true>(A.V, tile, lane, v);
             const double *xa = x + 5 * int64_t(__ldcs(A.star + i));
             const int64_t iatt = __ldcs(A.iatt + i);
-            const int32_t *icp = A.ic + tile * (N_INSTR * TILE) + lane;
             int32_t c[N_INSTR];
-#pragma unroll
-            for (int j = 0; j < N_INSTR; ++j) c[j] = __ldcs(icp + j * TILE);
+            load_ic<IC16>(A, tile, lane, c);
             double sum = 0.0;
 #pragma unroll
             for (int k = 0; k < N_ASTRO; ++k) sum = fma(v[k], __ldg(xa + k), sum);
@@ -204,7 +232,15 @@ struct FuseArgs {
     const double *xPack;   // FUSE_ATT: attitude unknowns of xin interleaved by axis (k_pack_att)
     cudaTextureObject_t texX;     // 0, or xin as a linear texture of int2 (gathers through the TEX path)
     cudaTextureObject_t texPack;  // 0, or xPack likewise
+    const double *xPack4;  // COOP: attitude unknowns as [s][4] = {axis0, axis1, axis2, 0}: a row's 12 unknowns are 4
+                           // consecutive 32-byte sectors, fetched by 4 lanes with one 256-bit load each
 };
+constexpr int COOP_STRIDE = 33;                      // doubles per (offset, axis) line of the per-warp exchange buffer
+constexpr int COOP_WARP = N_ATT * COOP_STRIDE;       // doubles per warp
+__device__ __forceinline__ void ld256_na(const double *p, double &a, double &b, double &c, double &d)
+{
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
+}
 __device__ __forceinline__ double tex_f64(cudaTextureObject_t t, int64_t idx)
 {
     const int2 q = tex1Dfetch<int2>(t, int(idx));
@@ -212,15 +248,20 @@ __device__ __forceinline__ double tex_f64(cudaTextureObject_t t, int64_t idx)
 }
 // FUSE_ATT: the attitude terms of A*xin are gathered here too, in star order (whole aprod1 in this pass,
 // y <- cy*y + cx*(A xin)); without it yrw must already hold cy*y + cx*(attitude terms).
-template <bool SQUARE, bool ATT_RED, bool PRIV = false, bool MATCH = false, bool FUSE = false, bool FUSE_ATT = false>
+// COOP (with FUSE_ATT): the attitude unknowns of a row are fetched cooperatively -- lanes 4q..4q+3 load the four
+// 32-byte sectors of row q's run of xPack4 with one LDG.256 each (8 rows per instruction, 4 instructions per tile) and
+// the values reach their row's lane through a per-warp shared-memory buffer: one or two L2 requests per row instead
+// of ~3.75 single-sector ones, and the attitude gathers no longer need L1.
+template <bool IC16, bool SQUARE, bool ATT_RED, bool PRIV = false, bool MATCH = false, bool FUSE = false, bool FUSE_ATT = false,
+          bool COOP = false>
 __global__ void __launch_bounds__(PRIV ? PRIV_THREADS : THREADS, PRIV ? 1 : 2)
 k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
          const double *__restrict__ coef, double *__restrict__ carryFirst,
          double *__restrict__ carryLast, double *__restrict__ globPartial, const int *done,
-         FuseArgs F = FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0})
+         FuseArgs F = FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, nullptr})
 {
     __shared__ double red[32];
-    extern __shared__ double sIns[];   // PRIV: nInsSm private instrument accumulators
+    extern __shared__ double sIns[];   // PRIV: nInsSm private instrument accumulators (+ COOP: exchange buffers)
     if (done && *done) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int nWarpsCta = PRIV ? PRIV_THREADS / 32 : WARPS;
@@ -248,15 +289,34 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         load_row<ATT_RED || FUSE_ATT>(A.V, tile, valid ? lane : nrows - 1, v);
         const int64_t ia = 5 * int64_t(__ldcs(A.star + i));
         // padded storage: the lanes past the last row read column 0 and a zero coefficient
-        const int32_t *icp = A.ic + tile * (N_INSTR * TILE) + lane;
         int32_t c[N_INSTR];
-#pragma unroll
-        for (int j = 0; j < N_INSTR; ++j) c[j] = __ldcs(icp + j * TILE);
+        load_ic<IC16>(A, tile, lane, c);
         // astro index of the rows just before and just after the tile (-1: none), fetched with the
         // tile's other loads instead of after the scan
         const int64_t iaBefore = r0 > 0 ? 5 * int64_t(__ldg(A.star + r0 - 1)) : int64_t(-1);
         const int64_t iaAfter = r0 + nrows < A.m ? 5 * int64_t(__ldg(A.star + r0 + nrows)) : int64_t(-1);
         double yv = 0.0;
+        double xatt[COOP ? N_ATT : 1];     // COOP: xatt[3*j + a] = unknown of axis a at start + j
+        int64_t iattRow = 0;
+        if (FUSE_ATT) iattRow = __ldcs(A.iatt + i);
+        if (COOP) {
+            double *buf = sIns + ((A.nInsSm + 1) & ~1) + warp * COOP_WARP;
+            const int p = lane & 3;
+#pragma unroll
+            for (int r = 0; r < 4; ++r) {
+                const int q = 8 * r + (lane >> 2);
+                const int64_t sq = __shfl_sync(0xffffffffu, iattRow, q);
+                double d0, d1, d2, d3;
+                ld256_na(F.xPack4 + (sq + p) * 4, d0, d1, d2, d3);
+                buf[(3 * p + 0) * COOP_STRIDE + q] = d0;
+                buf[(3 * p + 1) * COOP_STRIDE + q] = d1;
+                buf[(3 * p + 2) * COOP_STRIDE + q] = d2;
+            }
+            __syncwarp();
+#pragma unroll
+            for (int k = 0; k < N_ATT; ++k) xatt[k] = buf[k * COOP_STRIDE + lane];
+            __syncwarp();
+        }
         if (FUSE) {
             if (valid) {
                 const double *xa = F.xin + ia, *xIn = F.xin + A.offInstr;
@@ -271,15 +331,21 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
                 sum = fma(v[23], xg1, sum);
                 double yOld = F.yrw[i];
                 if (FUSE_ATT) {
-                    const int64_t iattRow = __ldcs(A.iatt + i);
-                    const double *xp = F.xPack + 3 * iattRow;
+                    if (COOP) {
 #pragma unroll
-                    for (int j = 0; j < 4; ++j)
+                        for (int j = 0; j < 4; ++j)
 #pragma unroll
-                        for (int a = 0; a < 3; ++a) {
-                            const double xa3 = F.texPack ? tex_f64(F.texPack, 3 * iattRow + 3 * j + a) : __ldg(xp + 3 * j + a);
-                            sum = fma(v[5 + 4 * a + j], xa3, sum);
-                        }
+                            for (int a = 0; a < 3; ++a) sum = fma(v[5 + 4 * a + j], xatt[3 * j + a], sum);
+                    } else {
+                        const double *xp = F.xPack + 3 * iattRow;
+#pragma unroll
+                        for (int j = 0; j < 4; ++j)
+#pragma unroll
+                            for (int a = 0; a < 3; ++a) {
+                                const double xa3 = F.texPack ? tex_f64(F.texPack, 3 * iattRow + 3 * j + a) : __ldg(xp + 3 * j + a);
+                                sum = fma(v[5 + 4 * a + j], xa3, sum);
+                            }
+                    }
                     yOld *= F.coef1[1];
                 }
                 const double yi = fma(cx1, sum, yOld);
@@ -460,11 +526,12 @@ __global__ void k_pre_aprod2(double *__restrict__ x, int64_t lo, int64_t hi,
 // segmented scan by s over the tile leaves one sum per (s, axis, j) and only those are added to x
 // (RED), instead of 12 REDs per row.  y is gathered through permT (one 8-byte gather per row).
 // ---------------------------------------------------------------------------------------
-template <bool SQUARE>
+template <bool SQUARE, bool MERGE = true>
 __global__ void __launch_bounds__(256)
 k_aprod2_att(MatView A, const double *__restrict__ y, double *__restrict__ x,
              const double *__restrict__ coef, const int *done)
 {
+    __shared__ double win[MERGE ? 8 : 1][3 * ATT_WIN];
     if (done && *done) return;
     const int lane = threadIdx.x & 31;
     const double cy = coef[1];
@@ -518,7 +585,40 @@ k_aprod2_att(MatView A, const double *__restrict__ y, double *__restrict__ x,
                     if (dist >= d) v[k] += t2;
                 }
             }
-            if (tail) {
+            // The 4-wide windows of neighbouring starts overlap (start s touches coefficients s..s+3 of each axis):
+            // when the tile's starts span less than ATT_WIN coefficients, the per-start sums are first added into a
+            // per-warp shared-memory window (tails have distinct s, so for a fixed j they hit distinct words: plain
+            // read-modify-write, one j at a time) and each coefficient of the window gets ONE RED per axis instead of
+            // one per (start, j): ~3x fewer REDs at Medium (16 starts per tile -> 3 x 19 instead of 16 x 12).
+            const int32_t sMin = __shfl_sync(0xffffffffu, sv, 0);
+            const int32_t span = __shfl_sync(0xffffffffu, sv, 31) - sMin + 4;
+            if (MERGE && span <= ATT_WIN) {
+                double *w = win[threadIdx.x >> 5];
+#pragma unroll
+                for (int q = 0; q < 3 * ATT_WIN / 32; ++q) w[q * 32 + lane] = 0.0;
+                __syncwarp();
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    if (tail) {
+                        double *wj = w + (sv - sMin + j);
+#pragma unroll
+                        for (int a = 0; a < 3; ++a) wj[a * ATT_WIN] += v[4 * a + j];
+                    }
+                    __syncwarp();
+                }
+#pragma unroll
+                for (int q = 0; q < ATT_WIN / 32; ++q) {
+                    const int idx = q * 32 + lane;
+                    if (idx < span) {
+#pragma unroll
+                        for (int a = 0; a < 3; ++a) {
+                            const double t2 = w[a * ATT_WIN + idx];
+                            if (t2 != 0.0) atomicAdd(xAtt + int64_t(a) * A.nDof + sMin + idx, t2);
+                        }
+                    }
+                }
+                __syncwarp();
+            } else if (tail) {
 #pragma unroll
                 for (int a = 0; a < 3; ++a)
 #pragma unroll
@@ -529,8 +629,8 @@ k_aprod2_att(MatView A, const double *__restrict__ y, double *__restrict__ x,
 }
 
 // ---------------------------------------------------------------------------------------
-// Fused LSQR iteration (gsr_lsqr uses it when the attitude copy exists and there are no
-// constraint rows): u' = A v - alpha u is row-local and A^T is linear, so the astro / instr / gamma sections of
+// Fused LSQR iteration (gsr_lsqr uses it when the attitude copy exists; constraint rows keep
+// their own two kernels): u' = A v - alpha u is row-local and A^T is linear, so the astro / instr / gamma sections of
 // t = A^T u' are accumulated, unscaled, by the star-ordered pass that computes u' (k_aprod2<.., FUSE, FUSE_ATT>:
 // the whole of aprod1 plus the scatter of aprod2's main kernel on one read of A); k_aprod2_att adds the
 // attitude section of t; then v <- cxv*v + cyv*t with sum v^2 (k_combine_sumsq), which applies 1/beta.
@@ -555,7 +655,7 @@ k_combine_sumsq(double *__restrict__ v, const double *__restrict__ t, int64_t n,
     if (threadIdx.x == 0) partial[blockIdx.x] = s;
 }
 
-// attT[k*m + t] = V[permT[t]*24 + 5 + k]  (re-run after the values are scaled by p)
+// attT[k*m + t] = V[permT[t]*24 + 5 + k]  (at upload; k_scale_attT applies the preconditioner to the copy)
 __global__ void k_gather_att(MatView A)
 {
     for (int64_t t = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; t < A.m;
@@ -832,7 +932,7 @@ __global__ void k_validate(MatView A, unsigned long long *badRow)
         if (i > 0) bad = bad || A.star[i - 1] > A.star[i];
 #pragma unroll
         for (int j = 0; j < N_INSTR; ++j) {
-            const int32_t c = A.ic[cpos(i, j)];
+            const int32_t c = ic_at(A, cpos(i, j));
             bad = bad || c < 0 || c >= A.nInstr;
         }
         if (bad) atomicMin(badRow, (unsigned long long)i);
@@ -908,7 +1008,7 @@ __global__ void k_scale_values(MatView A, const double *__restrict__ p)
         int64_t c;
         if (k < N_ASTRO) c = 5 * int64_t(A.star[i]) + k;
         else if (k < N_ASTRO + N_ATT) c = A.offAtt + ((k - N_ASTRO) >> 2) * A.nDof + A.iatt[i] + ((k - N_ASTRO) & 3);
-        else if (k < N_PAR - 1) c = A.offInstr + A.ic[cpos(i, k - N_ASTRO - N_ATT)];
+        else if (k < N_PAR - 1) c = A.offInstr + ic_at(A, cpos(i, k - N_ASTRO - N_ATT));
         else c = A.offGlob;
         A.V[e] = A.V[e] * p[c];
     }
@@ -924,8 +1024,11 @@ __global__ void k_scale_con_values(MatView A, int64_t nnz, const double *__restr
 // Upload (Alg. 1 l.6-12): rows [row0, row0+cnt) arrive row-major (A_d, I_c as the paper
 // stores them) and are written tile-transposed.  One thread per stored element; the
 // reads are coalesced, the writes hit 32 lines per warp but only once per upload.
-__global__ void k_ingest_rows(MatView A, int32_t *__restrict__ icDev, int64_t row0, int64_t cnt,
-                              const double *__restrict__ values, const int32_t *__restrict__ ic)
+// A column outside [0, 65536) cannot be stored in 2 bytes: it is written as column 0 and the row is reported through
+// badRow (k_validate would not see it any more).
+__global__ void k_ingest_rows(MatView A, int32_t *__restrict__ icDev, uint16_t *__restrict__ ic16Dev, int64_t row0, int64_t cnt,
+                              const double *__restrict__ values, const int32_t *__restrict__ ic,
+                              unsigned long long *badRow)
 {
     const int64_t nV = cnt * N_PAR, nC = cnt * N_INSTR;
     for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < nV + nC;
@@ -935,7 +1038,14 @@ __global__ void k_ingest_rows(MatView A, int32_t *__restrict__ icDev, int64_t ro
             A.V[vpos(row0 + r, int(e - r * N_PAR))] = values[e];
         } else {
             const int64_t f = e - nV, r = f / N_INSTR;
-            icDev[cpos(row0 + r, int(f - r * N_INSTR))] = ic[f];
+            const int32_t c = ic[f];
+            if (ic16Dev) {
+                const bool ok = c >= 0 && c < A.nInstr;
+                ic16Dev[cpos(row0 + r, int(f - r * N_INSTR))] = ok ? uint16_t(c) : uint16_t(0);
+                if (!ok) atomicMin(badRow, (unsigned long long)(row0 + r));
+            } else {
+                icDev[cpos(row0 + r, int(f - r * N_INSTR))] = c;
+            }
         }
     }
 }
@@ -959,7 +1069,7 @@ __global__ void k_instr_hist(MatView A, unsigned int *__restrict__ cnt)
     for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < total;
          e += int64_t(gridDim.x) * blockDim.x) {
         const int64_t i = (e / (N_INSTR * TILE)) * TILE + (e & 31);
-        if (i < A.m) atomicAdd(cnt + A.ic[e], 1u);
+        if (i < A.m) atomicAdd(cnt + ic_at(A, e), 1u);
     }
 }
 __global__ void k_max_u32(const unsigned int *__restrict__ cnt, int64_t n, unsigned int *__restrict__ out)

@@ -18,14 +18,23 @@ LIB_PATH = os.path.join(_PKG, "libgsr.so")
 
 GSR_OK, GSR_EINVAL, GSR_EINDEX, GSR_ENOMEM, GSR_ECUDA, GSR_ESTATE = 0, -1, -2, -3, -4, -5
 TRACE_CAP = 4096
+# gsr_layout.flags (include/gsr.h)
+GSR_FLAG_NO_ATT_COPY, GSR_FLAG_NO_FUSE, GSR_FLAG_NO_TEX = 1, 2, 4
+# gsr_path_info bits
+GSR_PATH_ATT_COPY, GSR_PATH_FUSED, GSR_PATH_INSTR_MATCH, GSR_PATH_TEX, GSR_PATH_IC16 = 1, 2, 4, 8, 16
+# gsr_time_aprod selectors (include/gsr_bench.h)
+GSR_TIME_APROD1_GROUP, GSR_TIME_APROD2_GROUP = 1, 2
+GSR_TIME_K_APROD1, GSR_TIME_K_APROD2_MAIN, GSR_TIME_K_APROD2_ATT, GSR_TIME_K_FUSED = 11, 12, 13, 21
 
 # every symbol include/gsr.h declares (tests check that the library exports each one)
 SYMBOLS = [
     "gsr_create", "gsr_destroy", "gsr_last_error", "gsr_bad_row", "gsr_ncols", "gsr_nrows",
     "gsr_upload", "gsr_upload_rows", "gsr_upload_finish", "gsr_upload_constraints", "gsr_set_b",
     "gsr_get_star_rowptr", "gsr_precondition", "gsr_get_colscale", "gsr_get_values",
-    "gsr_aprod1", "gsr_aprod2", "gsr_lsqr", "gsr_get_trace", "gsr_last_timing", "gsr_time_aprod",
+    "gsr_aprod1", "gsr_aprod2", "gsr_lsqr", "gsr_get_trace", "gsr_path_info", "gsr_last_timing",
 ]
+# the measurement hook of include/gsr_bench.h
+BENCH_SYMBOLS = ["gsr_bench_set", "gsr_time_aprod"]
 
 
 class GsrError(RuntimeError):
@@ -38,7 +47,8 @@ class _Layout(C.Structure):
     _fields_ = [("n_obs", C.c_int64), ("n_stars", C.c_int64), ("n_dof_att", C.c_int64),
                 ("n_instr", C.c_int64), ("n_con", C.c_int64), ("n_con_nnz", C.c_int64),
                 ("n_astro_par", C.c_int32), ("n_att_par", C.c_int32), ("n_instr_par", C.c_int32),
-                ("n_glob_par", C.c_int32), ("device", C.c_int32), ("stream", C.c_void_p)]
+                ("n_glob_par", C.c_int32), ("device", C.c_int32), ("flags", C.c_uint32),
+                ("stream", C.c_void_p)]
 
 
 class _Result(C.Structure):
@@ -80,8 +90,10 @@ def load_library():
         "gsr_aprod2": (I32, [P, P, P]),
         "gsr_lsqr": (I32, [P, I64, D, D, D, C.POINTER(_Result)]),
         "gsr_get_trace": (I32, [P, P, I64, C.POINTER(I64)]),
+        "gsr_path_info": (I32, [P]),
         "gsr_last_timing": (I32, [P, C.POINTER(D), C.POINTER(I64)]),
         "gsr_time_aprod": (I32, [P, I32, I32, C.POINTER(D)]),
+        "gsr_bench_set": (I32, [P, C.c_char_p, I64]),
     }
     for name, (res, args) in sig.items():
         f = getattr(lib, name)
@@ -136,12 +148,14 @@ class LsqrResult:
 class Gsr:
     """One system on one GPU.  Methods mirror the C entry points one to one."""
 
-    def __init__(self, n_obs, n_stars, n_dof_att, n_instr, n_con=0, n_con_nnz=0, device=0, stream=None):
+    def __init__(self, n_obs, n_stars, n_dof_att, n_instr, n_con=0, n_con_nnz=0, device=0, stream=None, flags=0,
+                 n_glob=1):
         self.lib = load_library()
         self._h = C.c_void_p()
         if stream is None and torch.cuda.is_available():
             stream = torch.cuda.current_stream(device).cuda_stream
-        L = _Layout(n_obs, n_stars, n_dof_att, n_instr, n_con, n_con_nnz, 5, 12, 6, 1, device, stream or None)
+        L = _Layout(n_obs, n_stars, n_dof_att, n_instr, n_con, n_con_nnz, 5, 12, 6, n_glob, device, flags,
+                    stream or None)
         rc = self.lib.gsr_create(C.byref(L), C.byref(self._h))
         if rc != GSR_OK:
             msg = self.lib.gsr_last_error(self._h).decode() if self._h else "gsr_create failed"
@@ -250,6 +264,12 @@ class Gsr:
         nw = C.c_int64()
         self._ck(self.lib.gsr_get_trace(self._h, out.ctypes.data, max_itn, C.byref(nw)))
         return out[: nw.value]
+
+    def gsr_path_info(self):
+        return int(self.lib.gsr_path_info(self._h))
+
+    def gsr_bench_set(self, key, value):
+        self._ck(self.lib.gsr_bench_set(self._h, key.encode(), int(value)))
 
     def gsr_time_aprod(self, which, reps):
         ms = C.c_double()

@@ -28,9 +28,9 @@ def dev(a):
     return torch.from_numpy(np.ascontiguousarray(a)).cuda()
 
 
-def make_gpu(S, d, b, upload_constraints=True):
+def make_gpu(S, d, b, upload_constraints=True, flags=0):
     gsr = gsr_mod()
-    G = gsr.Gsr(S.m, S.n_stars, S.n_dof_att, S.n_instr, S.n_con, len(S.con_col))
+    G = gsr.Gsr(S.m, S.n_stars, S.n_dof_att, S.n_instr, S.n_con, len(S.con_col), flags=flags)
     G.gsr_upload(np.ascontiguousarray(d["values"]), np.ascontiguousarray(d["matrixIndexAstro"]),
                  np.ascontiguousarray(d["matrixIndexAtt"]), np.ascontiguousarray(d["instrCol"]), b)
     if S.n_con and upload_constraints:
@@ -75,6 +75,10 @@ CASES = {
     # Zipf(1.1) over 2,000 columns: the hottest column holds ~300x the mean, which switches aprod2 to the
     # variant that pre-sums equal columns inside a warp (MATCH)
     "zipf_hot": dict(cfg=synth.SynthConfig("zipf", 300, 200, 2_000, obs_per_star=30, instr_zipf=1.1, seed=9)),
+    # more than 65,536 instrument columns: the device keeps 4-byte columns (2-byte ones otherwise)
+    "wide_instr": dict(cfg=synth.SynthConfig("wide", 200, 150, 70_000, obs_per_star=40, seed=12)),
+    "zipf_con": dict(cfg=synth.SynthConfig("zipfc", 300, 200, 2_000, obs_per_star=30, instr_zipf=1.1, n_con=6,
+                                           con_nnz=40, seed=10)),
 }
 
 
@@ -85,6 +89,7 @@ def test_aprod_parity_and_layout(name):
     b = make_b(S, d)
     with make_gpu(S, d, b) as G:
         assert G.n == S.n and G.m_tot == S.m_tot
+        assert bool(G.gsr_path_info() & gsr_mod().GSR_PATH_IC16) == (cfg.n_instr <= 65536)
         rp = G.gsr_get_star_rowptr().cpu().numpy()
         assert np.array_equal(rp, d["rowptr"])                                   # generator's own
         assert np.array_equal(rp, np.searchsorted(S.ia, 5 * np.arange(S.n_stars + 1), side="left"))
@@ -202,10 +207,13 @@ def rel(a, b):
     return np.linalg.norm(a - b) / max(np.linalg.norm(b), 1e-300)
 
 
-@pytest.mark.parametrize("name,itn", [("mini", 30), ("mini_con", 25), ("ragged_tail", 40), ("powerlaw", 40)])
+@pytest.mark.parametrize("name,itn", [("mini", 30), ("mini_con", 25), ("ragged_tail", 40), ("powerlaw", 40),
+                                      ("zipf_hot", 30), ("zipf_con", 30), ("wide_instr", 20)])
 def test_lsqr_fixed_iterations_small(name, itn):
     S, d, G, r, ro = lsqr_both(CASES[name]["cfg"], itn, 0.0, 0.0)
     with G:
+        if name.startswith("zipf"):      # the variant that pre-sums equal instrument columns inside a warp was chosen
+            assert G.gsr_path_info() & gsr_mod().GSR_PATH_INSTR_MATCH
         assert (r.istop, r.itn) == (ro.istop, ro.itn) == (7, itn)
         assert rel(r.x.cpu().numpy(), ro.x) <= X_TOL
         assert rel(r.se.cpu().numpy(), ro.se) <= 1e-8
@@ -288,7 +296,8 @@ def test_index_validation():
     S, d = oracle_system(cfg)
     b = make_b(S, d)
     for key, row, val in (("matrixIndexAstro", 17, 3), ("matrixIndexAtt", 40, cfg.n_dof_att - 3),
-                          ("instrCol", 100, cfg.n_instr), ("matrixIndexAstro", 5, 5 * cfg.n_stars)):
+                          ("instrCol", 100, cfg.n_instr), ("matrixIndexAstro", 5, 5 * cfg.n_stars),
+                          ("instrCol", 33, 65536 + 3), ("instrCol", 7, -1)):      # would alias a valid 2-byte column
         bad = {k: np.array(v, copy=True) for k, v in d.items()}
         if key == "instrCol":
             bad[key][row, 2] = val
@@ -385,32 +394,36 @@ def test_medium_full_size_sampled():
             assert np.all(np.abs(xg - xo[sl]) <= APROD_TOL * ab2[sl] + 1e-300), (s, xg, xo[sl])
 
 
-@pytest.mark.parametrize("env", ["GSR_NO_ATT_COPY", "GSR_NO_FUSE"])
-def test_fallback_paths(env, monkeypatch):
-    """The low-memory path (no block-time-ordered attitude copy: attitude REDs inside k_aprod2) and the two-product
-    form of the iteration give the same results as the default path.  GSR_NO_FUSE is read once per process, so that
-    case runs in a child process."""
-    import subprocess
-    import sys
-    code = (
-        "import numpy as np, sys; sys.path.insert(0, 'tests')\n"
-        "import test_gpu_parity as T\n"
-        "from helpers import make_b, oracle_system\n"
-        "cfg = T.CASES['mini_con']['cfg']\n"
-        "S, d = oracle_system(cfg); b = make_b(S, d)\n"
-        "G = T.make_gpu(S, d, b); T.check_aprods(S, G)\n"
-        "G.gsr_precondition(); S.precondition()\n"
-        "r = G.gsr_lsqr(25, 0.0, 0.0); ro = S.lsqr(b, 25, 0.0, 0.0)\n"
-        "x = r.x.cpu().numpy()\n"
-        "assert r.itn == ro.itn == 25 and r.istop == ro.istop == 7\n"
-        "assert np.linalg.norm(x - ro.x) <= T.X_TOL * np.linalg.norm(ro.x)\n"
-        "import pytest\n"
-        "which = 13 if '%s' == 'GSR_NO_ATT_COPY' else 21   # kernels that exist only on the default path\n"
-        "with pytest.raises(T.gsr_mod().GsrError): G.gsr_time_aprod(which, 1)\n"
-        "print('ok')\n" % env)
-    import os
-    envv = dict(os.environ, **{env: "1"})
-    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    p = subprocess.run([sys.executable, "-c", code], cwd=root, env=envv, capture_output=True, text=True, timeout=600)
-    assert p.returncode == 0, p.stderr[-2000:]
-    assert p.stdout.split()[-1] == "ok"
+@pytest.mark.parametrize("flag", ["NO_ATT_COPY", "NO_FUSE", "NO_TEX"])
+@pytest.mark.parametrize("case", ["mini_con", "zipf_hot", "ragged_tail"])
+def test_fallback_paths(flag, case):
+    """gsr_layout.flags, per handle and in-process: the low-memory path (no block-time-ordered attitude copy:
+    attitude REDs inside k_aprod2, two-product iteration), the two-product form of the iteration on the default
+    layout, and the fused pass without texture objects (the path systems with n >= 2^27 take) all give the
+    oracle's results."""
+    gsr = gsr_mod()
+    fl = {"NO_ATT_COPY": gsr.GSR_FLAG_NO_ATT_COPY, "NO_FUSE": gsr.GSR_FLAG_NO_FUSE, "NO_TEX": gsr.GSR_FLAG_NO_TEX}[flag]
+    cfg = CASES[case]["cfg"]
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    with make_gpu(S, d, b, flags=fl) as G:
+        info = G.gsr_path_info()
+        assert bool(info & gsr.GSR_PATH_ATT_COPY) == (flag != "NO_ATT_COPY")
+        assert bool(info & gsr.GSR_PATH_FUSED) == (flag == "NO_TEX")
+        assert bool(info & gsr.GSR_PATH_TEX) == (flag != "NO_TEX")
+        assert bool(info & gsr.GSR_PATH_INSTR_MATCH) == (case == "zipf_hot")
+        check_aprods(S, G)
+        G.gsr_precondition()
+        S.precondition()
+        r = G.gsr_lsqr(25, 0.0, 0.0)
+        ro = S.lsqr(b, 25, 0.0, 0.0)
+        assert r.itn == ro.itn == 25 and r.istop == ro.istop == 7
+        assert rel(r.x.cpu().numpy(), ro.x) <= X_TOL
+        assert rel(r.se.cpu().numpy(), ro.se) <= 1e-8
+        # kernels that exist only on the default path
+        if flag == "NO_ATT_COPY":
+            with pytest.raises(gsr.GsrError):
+                G.gsr_time_aprod(gsr.GSR_TIME_K_APROD2_ATT, 1)
+        if flag != "NO_TEX":
+            with pytest.raises(gsr.GsrError):
+                G.gsr_time_aprod(gsr.GSR_TIME_K_FUSED, 1)

@@ -315,6 +315,112 @@ def test_x_and_se_against_krylov_closed_form():
         var = (rk.se / p / rk.rnorm * np.sqrt(S.m_tot - S.n)) ** 2
         assert np.linalg.norm(rk.x / p - zk) <= 1e-12 * np.linalg.norm(zk)
         np.testing.assert_allclose(var, var_ref, rtol=1e-9)
+        # the scale of se, with nothing taken from the oracle: the TRUE residual of the dense Krylov solution
+        # over sqrt(m - n) (m_tot > n here), times p (Alg. 1 l.27)
+        se_ref = p * np.sqrt(var_ref) * np.linalg.norm(b - A @ zk) / np.sqrt(S.m_tot - S.n)
+        np.testing.assert_allclose(rk.se, se_ref, rtol=1e-9)
         assert (var <= full * (1 + 1e-9)).all()
         assert (var >= prev * (1 - 1e-12)).all()     # non-decreasing in the iteration count
         prev = var
+
+
+# ----------------------------------------------------------------------------- last corners
+def _dense24(A, con=None):
+    """Any dense m x 24 matrix IS a Gaia-shaped system: one star (5 astro columns), N_DFA = 4 (3 x 4 attitude
+    columns, start 0), 6 instrument columns 0..5, gamma: every row touches all 24 columns exactly once."""
+    m = A.shape[0]
+    return oracle.OracleSystem(1, 4, 6, A, np.zeros(m, np.int64), np.zeros(m, np.int64),
+                               np.tile(np.arange(6, dtype=np.int32), (m, 1)))
+
+
+def test_dense24_column_map_is_identity():
+    A = np.arange(3 * 24, dtype=np.float64).reshape(3, 24) + 1
+    S = _dense24(A)
+    assert S.n == 24 and [S.col(1, k) for k in range(24)] == list(range(24))
+    x = np.linspace(-1, 1, 24)
+    np.testing.assert_allclose(S.aprod1(x, np.zeros(3)), A @ x, rtol=1e-14)
+
+
+def test_istop4_consistent_system_solved_to_machine_precision():
+    """atol = btol = 0 on a consistent system: the residual reaches the rounding floor and the only test that can
+    fire is 1 + test1/(1 + anorm*xnorm/bnorm) <= 1, i.e. istop 4 (test1 <= rtol = 0 needs rnorm == 0 exactly).
+    Pin: scipy's LSQR (same published algorithm) stops with 4 within one iteration of the oracle, and the
+    solution is the planted one."""
+    rng = np.random.default_rng(2)
+    A = rng.standard_normal((40, 24))
+    xt = rng.standard_normal(24)
+    b = A @ xt
+    r = _dense24(A).lsqr(b, 500, 0.0, 0.0)
+    rs = spla.lsqr(A, b, atol=0.0, btol=0.0, conlim=0.0, iter_lim=500)
+    assert r.istop == 4 == rs[1]
+    assert abs(r.itn - rs[2]) <= 1
+    assert np.linalg.norm(r.x - xt) <= 1e-12 * np.linalg.norm(xt)
+    assert r.rnorm <= 1e-13 * np.linalg.norm(b)
+
+
+def test_istop6_condition_estimate_exceeds_one_over_eps():
+    """A 19 x 24 matrix of rank 11 with 4 singular values in [0.5, 1] and 7 near 10^-15.66: the Krylov process
+    resolves the small cluster while A^T r is still far from zero, so acond = anorm*sqrt(ddnorm) passes 1/eps
+    (1 + 1/acond <= 1, istop 6) before test 2 can fire.  Pins: the true condition number of the non-zero spectrum
+    is > 1/eps (so 6 is the right answer), and scipy's LSQR stops with the same code at the same iteration."""
+    rng = np.random.default_rng(16)
+    k1, k2 = int(rng.integers(1, 8)), int(rng.integers(2, 12))
+    k = k1 + k2
+    m = k + int(rng.integers(1, 10))
+    U, _ = np.linalg.qr(rng.standard_normal((m, k)))
+    V, _ = np.linalg.qr(rng.standard_normal((24, k)))
+    e = rng.uniform(15.5, 17.5)
+    sig = np.concatenate([rng.uniform(0.5, 1, k1), 10 ** (-e) * rng.uniform(0.5, 2, k2)])
+    A = U @ np.diag(sig) @ V.T
+    b = rng.standard_normal(m)
+    assert (k1, k2, m) == (4, 7, 19) and sig.max() / sig.min() > 1.0 / np.finfo(float).eps
+    r = _dense24(A).lsqr(b, 200, 0.0, 0.0)
+    rs = spla.lsqr(A, b, atol=0.0, btol=0.0, conlim=0.0, iter_lim=200)
+    assert r.istop == 6 == rs[1]
+    assert r.itn == rs[2]
+    assert 1.0 + 1.0 / r.acond <= 1.0
+    assert abs(r.acond - rs[6]) <= 1e-2 * rs[6]
+
+
+def test_se_scale_when_m_not_greater_than_n():
+    """m_tot <= n (the other branch): se = sqrt(var) * rnorm without the sqrt(m - n)
+    divisor.  Pin: the Krylov closed form for var and the true residual of the dense Krylov solution."""
+    rng = np.random.default_rng(5)
+    A = rng.standard_normal((10, 24))
+    b = rng.standard_normal(10)
+    S = _dense24(A)
+    assert S.m_tot <= S.n
+    B, V, beta = _golub_kahan_reorth(A, b, 6)
+    for k in (1, 3, 6):
+        Bk, Vk = B[:k + 1, :k], V[:, :k]
+        e1 = np.zeros(k + 1)
+        e1[0] = beta
+        zk = Vk @ np.linalg.lstsq(Bk, e1, rcond=None)[0]
+        var_ref = np.diag(Vk @ np.linalg.inv(Bk.T @ Bk) @ Vk.T)
+        rk = S.lsqr(b, k, 0.0, 0.0)
+        assert (rk.istop, rk.itn) == (7, k)
+        np.testing.assert_allclose(rk.se, np.sqrt(var_ref) * np.linalg.norm(b - A @ zk), rtol=1e-9)
+
+
+# ----------------------------------------------------------------------------- OpenMP restatement (bench only)
+@pytest.mark.parametrize("threads", [1, 3, 8])
+def test_omp_restatement_matches_the_oracle(threads):
+    """oracle/gsr_oracle_omp.c (PAPER.md:150 threading; used only for bench.py's all-core cpu_baseline) against
+    the parity oracle: aprods within 1e-12 * sum|terms|, LSQR x within 1e-10 after 30 iterations."""
+    cfg = synth.SynthConfig("omp", 700, 400, 90, obs_powerlaw=(2.0, 12, 60), n_con=7, con_nnz=30, seed=3)   # m > n, well posed
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    R = oracle.OmpRunner(S, threads)
+    assert R.threads == threads
+    rng = np.random.default_rng(0)
+    x, y = rng.standard_normal(S.n), rng.standard_normal(S.m_tot)
+    y1, ab = S.aprod1(x, y, want_abs=True)
+    assert np.all(np.abs(R.aprod1(x, y) - y1) <= 1e-12 * ab)
+    x1, ab = S.aprod2(y, x, want_abs=True)
+    assert np.all(np.abs(R.aprod2(y, x) - x1) <= 1e-12 * ab)
+    S.precondition()
+    r1, r2 = S.lsqr(b, 30, 0.0, 0.0), R.lsqr(b, 30, 0.0, 0.0)
+    assert (r1.istop, r1.itn) == (r2.istop, r2.itn) == (7, 30)
+    assert np.linalg.norm(r1.x - r2.x) <= 1e-10 * np.linalg.norm(r1.x)
+    assert np.linalg.norm(r1.se - r2.se) <= 1e-9 * np.linalg.norm(r1.se)
+    assert abs(r1.rnorm - r2.rnorm) <= 1e-10 * r1.rnorm
