@@ -130,7 +130,10 @@ int32_t gsr_upload(gsr_handle *h, const double *values, const int64_t *matrixInd
  * 116 GB "Large" config cannot exist twice in HBM): copies rows [row0, row0+nrows)
  * of the four arrays and of b.  Call gsr_upload_finish() once every row is in; it
  * validates and derives layouts exactly as gsr_upload does.  b_tail (n_con entries,
- * may be NULL when n_con == 0) holds the known terms of the constraint rows. */
+ * may be NULL when n_con == 0) holds the known terms of the constraint rows.
+ * A new upload always starts from scratch: every row must come again before the next
+ * gsr_upload_finish (the 4-byte star indices of the rows are upload scratch that the
+ * finish step turns into the star row pointer and frees). */
 int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double *values,
                         const int64_t *matrixIndexAstro, const int64_t *matrixIndexAtt,
                         const int32_t *instrCol, const double *b);

@@ -29,6 +29,7 @@ struct gsr_handle {
     int64_t *rp = nullptr, *conRp = nullptr, *conCol = nullptr;
     int32_t *ic = nullptr, *star = nullptr, *iatt = nullptr;   // 4-byte row indices
     uint16_t *ic16 = nullptr;                                  // instrument columns in 2 bytes when n_instr <= 65536 (ic stays null)
+    unsigned long long *tw = nullptr;                          // per-tile star word (MatView::tw); star[] is upload scratch
     int64_t badIngest = -1;                                    // first row whose instrument column did not fit 2 bytes
     int64_t *stageI = nullptr;                                 // upload staging of the two i64 index arrays
     // work
@@ -42,8 +43,9 @@ struct gsr_handle {
     int nInsSmFused = 0;       // columns of the shared-memory table in the fused main kernel
     cudaTextureObject_t texV = 0, texPack = 0;   // v and xPack as linear int2 textures (fused pass gathers)
     int nRepAlloc = 1;
-    double *xPack4 = nullptr;  // attitude unknowns as [s][4] for the cooperative gather of the fused pass
-    bool coop = false, attMerge = true;
+    double *uT = nullptr;      // u^ in block-time order: k_u_to_time fills it, k_aprod2_att<.., LINEAR> reads it (fused iteration)
+    bool useUT = false;
+    int gridUT = 1;
     // time-ordered attitude copy (aprod2 "bucketed scatter") and instrument replicas
     double *attT = nullptr, *insRep = nullptr;
     int32_t *sT = nullptr;
@@ -100,7 +102,7 @@ cudaError_t dalloc(T **p, int64_t count)
 MatView view(const gsr_handle *h)
 {
     MatView A;
-    A.V = h->V; A.star = h->star; A.iatt = h->iatt; A.ic = h->ic; A.ic16 = h->ic16; A.rp = h->rp;
+    A.V = h->V; A.star = h->star; A.iatt = h->iatt; A.ic = h->ic; A.ic16 = h->ic16; A.rp = h->rp; A.tw = h->tw;
     A.m = h->L.n_obs; A.nStars = h->L.n_stars; A.nDof = h->L.n_dof_att; A.nInstr = h->L.n_instr;
     A.offAtt = 5 * h->L.n_stars;
     A.offInstr = A.offAtt + 3 * h->L.n_dof_att;
@@ -203,8 +205,8 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     if (L->n_obs < 0 || L->n_stars < 1 || L->n_dof_att < 4 || L->n_instr < 6 || L->n_con < 0 ||
         L->n_con_nnz < 0 || (L->n_con == 0 && L->n_con_nnz != 0))
         return fail(h, GSR_EINVAL, "bad sizes");
-    if (L->n_stars >= (int64_t(1) << 31) || L->n_dof_att >= (int64_t(1) << 31) || L->n_instr >= (int64_t(1) << 31))
-        return fail(h, GSR_EINVAL, "n_stars, n_dof_att and n_instr must fit 31 bits (4-byte row indices)");
+    if (L->n_stars >= (int64_t(1) << TW_STAR_BITS) || L->n_dof_att >= (int64_t(1) << 31) || L->n_instr >= (int64_t(1) << 31))
+        return fail(h, GSR_EINVAL, "n_stars must be below 2^29, n_dof_att and n_instr below 2^31 (packed row indices)");
     h->n = 5 * L->n_stars + 3 * L->n_dof_att + L->n_instr + 1;
     h->mTot = L->n_obs + L->n_con;
     h->nTiles = (L->n_obs + TILE - 1) / TILE;
@@ -240,8 +242,6 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
         CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
         CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
         CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
-        CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, false, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
-        CK(cudaFuncSetAttribute(k_aprod2<false, false, false, true, false, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
         // the fused kernel also gathers x: a 96 KB table leaves the rest of the SM's memory to L1 (measured at
         // Medium: 0 / 3 k / 6 k / 12 k / 18 k / 24.5 k columns -> 22.3 / 22.5 / 22.8 / 22.4 / 22.7 / 24.4 ms per iteration)
         h->nInsSmFused = std::min(h->nInsSm, 12288);
@@ -252,13 +252,15 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     // fix-up grid: one thread per star, then one per instrument column (replica fold), then gamma
     h->gridFix = int((L->n_stars + 255) / 256) + int((L->n_instr + 255) / 256) + 1;
     h->gridAtt = gridFor(h->nTiles, 8, h->smCount * 4);
+    h->gridUT = gridFor(L->n_obs, 256, h->smCount * 4);
     // instrument replicas: spread the REDs of aprod2 over >= ~512k distinct addresses
     h->nRep = int(std::max<int64_t>(1, std::min<int64_t>(128, (524288 + L->n_instr - 1) / L->n_instr)));
 
     const int64_t m = L->n_obs;
     // coefficients and instrument columns are stored tile-transposed and padded to whole tiles
     CK(dalloc(&h->V, h->nTiles * TILE * N_PAR));
-    CK(dalloc(&h->star, m));
+    CK(dalloc(&h->star, m));   // scratch of the upload: freed by gsr_upload_finish, allocated again by the next upload
+    CK(dalloc(&h->tw, h->nTiles));
     CK(dalloc(&h->iatt, m));
     // instrument columns: 2 bytes each when they fit, else 4
     const bool ic16 = L->n_instr <= 65536;
@@ -284,7 +286,6 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(dalloc(&h->sqPartialV, h->gridVec));
     CK(dalloc(&h->ddPartial, h->gridVec));
     CK(dalloc(&h->xPack, 3 * L->n_dof_att));
-    CK(dalloc(&h->xPack4, 4 * L->n_dof_att));
     CK(dalloc(&h->coefOne, 2));
     CK(dalloc(&h->coefTime, 2));
     CK(dalloc(&h->trace, 5 * GSR_TRACE_CAP));
@@ -334,6 +335,15 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
                 h->attT = nullptr; h->sT = nullptr; h->permT = nullptr;
             }
             h->useAttT = ok;
+            if (ok && !(L->flags & GSR_FLAG_NO_FUSE)) {   // u^ in time order for the fused iteration (+8 B/row); optional
+                bool ok2 = dalloc(&h->uT, m) == cudaSuccess;
+                if (!ok2) {
+                    cudaGetLastError();
+                    h->uT = nullptr;
+                }
+                if (ok2) ok2 = cudaMemset(h->uT, 0, size_t(m) * sizeof(double)) == cudaSuccess;
+                h->useUT = ok2;
+            }
         }
     }
     CK(cudaMallocHost(reinterpret_cast<void **>(&h->hostS), 2 * sizeof(Scalars)));
@@ -356,10 +366,10 @@ int32_t gsr_destroy(gsr_handle *h)
     if (h->texV) cudaDestroyTextureObject(h->texV);
     if (h->texPack) cudaDestroyTextureObject(h->texPack);
     if (h->iterGraph) cudaGraphExecDestroy(h->iterGraph);
-    void *ptrs[] = {h->V, h->b, h->conVal, h->p, h->star, h->iatt, h->stageI, h->rp, h->conRp, h->conCol, h->ic, h->ic16,
+    void *ptrs[] = {h->V, h->b, h->conVal, h->p, h->star, h->iatt, h->stageI, h->rp, h->conRp, h->conCol, h->ic, h->ic16, h->tw,
                     h->u, h->v, h->w, h->z, h->var, h->carryFirst, h->carryLast, h->globPartial,
                     h->sqPartialU, h->sqPartialV, h->ddPartial, h->coefOne, h->coefTime, h->trace,
-                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC, h->xPack, h->t, h->coefRaw, h->xPack4};
+                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC, h->xPack, h->t, h->coefRaw, h->uT};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (h->hostS) cudaFreeHost(h->hostS);
@@ -389,6 +399,7 @@ int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double
     h->uploaded = false;
     h->preconditioned = false;
     h->conUploaded = false;   // gsr_precondition scaled conVal in place: the constraint rows must come again
+    if (!h->star) CK(dalloc(&h->star, h->L.n_obs));
     const size_t r = size_t(nrows);
     CK(cudaMemcpyAsync(h->b + row0, b, r * sizeof(double), cudaMemcpyDefault, h->stream));
     {   // the two i64 index arrays -> 4-byte star / attitude start (device sources in place, host sources staged)
@@ -445,6 +456,7 @@ int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail)
 {
     if (!h) return GSR_EINVAL;
     if (h->L.n_con > 0 && !b_tail) return fail(h, GSR_EINVAL, "b_tail is NULL but n_con > 0");
+    if (!h->star) return fail(h, GSR_ESTATE, "no rows uploaded since the last gsr_upload_finish");
     int rc = enter(h);
     if (rc) return rc;
     if (h->L.n_con > 0)
@@ -466,6 +478,7 @@ int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail)
     }
     h->badRow = -1;
     k_star_rowptr<<<int((h->L.n_stars + 1 + 255) / 256), 256, 0, h->stream>>>(h->star, A.m, A.nStars, h->rp);
+    if (A.m > 0) k_tile_words<<<gridFor(h->nTiles, 8, h->smCount * 16), 256, 0, h->stream>>>(h->star, A.m, h->tw);
     CK(cudaGetLastError());
     k_fill<<<h->gridVec, 256, 0, h->stream>>>(h->p, h->n, 1.0);
     CK(cudaGetLastError());
@@ -492,6 +505,9 @@ int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail)
             h->iterGraph = nullptr;
         }
     }
+    CK(cudaStreamSynchronize(h->stream));
+    cudaFree(h->star);   // the kernels read the row pointer and the tile words from here on
+    h->star = nullptr;
     h->uploaded = true;
     h->preconditioned = false;
     return GSR_OK;
@@ -561,9 +577,11 @@ int readyCheck(gsr_handle *h)
     return GSR_OK;
 }
 
-void launchAtt(gsr_handle *h, const MatView &A, const double *y, double *x, const double *coef, const int *done)
+// attitude section of aprod2 on the time-ordered copy; linear: y is already in that order (uT)
+void launchAtt(gsr_handle *h, const MatView &A, const double *y, double *x, const double *coef, const int *done,
+               bool linear = false)
 {
-    if (h->attMerge) k_aprod2_att<false, true><<<h->gridAtt, 256, 0, h->stream>>>(A, y, x, coef, done);
+    if (linear) k_aprod2_att<false, true><<<h->gridAtt, 256, 0, h->stream>>>(A, y, x, coef, done);
     else k_aprod2_att<false, false><<<h->gridAtt, 256, 0, h->stream>>>(A, y, x, coef, done);
 }
 
@@ -592,19 +610,9 @@ template <bool FUSE>
 void launchAprod2Main(gsr_handle *h, const MatView &A, const double *y, double *x, const double *coef, const int *done,
                       const FuseArgs &F)
 {
-    size_t sm = size_t(A.nInsSm) * sizeof(double);
+    const size_t sm = size_t(A.nInsSm) * sizeof(double);
     const int g = h->gridA2m;
     cudaStream_t st = h->stream;
-    if (FUSE && h->coop && !h->instrSkewed) {   // cooperative attitude gather: exchange buffers behind the table
-        sm = (size_t((A.nInsSm + 1) & ~1) + size_t(PRIV_THREADS / 32) * COOP_WARP) * sizeof(double);
-        if (h->ic16)
-            k_aprod2<true, false, false, true, false, FUSE, FUSE, FUSE><<<g, PRIV_THREADS, sm, st>>>(
-                A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done, F);
-        else
-            k_aprod2<false, false, false, true, false, FUSE, FUSE, FUSE><<<g, PRIV_THREADS, sm, st>>>(
-                A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done, F);
-        return;
-    }
 #define GSR_A2M(IC, MA)                                                                                          \
     k_aprod2<IC, false, false, true, MA, FUSE, FUSE><<<g, PRIV_THREADS, sm, st>>>(A, y, x, coef, h->carryFirst,    \
                                                                                  h->carryLast, h->globPartial, done, F)
@@ -650,7 +658,7 @@ int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef,
         launchAprod2Red<SQUARE>(h, A, y, x, coef, done);
     } else {
         launchAtt(h, A, y, x, coef, done);
-        launchAprod2Main<false>(h, A, y, x, coef, done, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, nullptr});
+        launchAprod2Main<false>(h, A, y, x, coef, done, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0});
         ++nk;
     }
     k_astro_fixup<<<h->gridFix, 256, 0, h->stream>>>(A, x, coef, h->carryFirst, h->carryLast, h->globPartial,
@@ -678,11 +686,11 @@ int enqueueIterationFused(gsr_handle *h)
     cudaStream_t st = h->stream;
     MatView A = view(h);
     A.nInsSm = h->nInsSmFused;
-    k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, done, h->coop ? h->xPack4 : nullptr);
+    k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, done);
     // t <- 0 (and the instrument replicas); then one star-ordered pass over A: u^ <- a1_cy*u^ + a1_cx*(A v^), sum u^2,
     // and the astro / instr / gamma sections of t = A^T u^ (unscaled)
     k_pre_aprod2<<<h->gridVec, 256, 0, st>>>(h->t, 0, A.n, h->coefRaw, h->insRep, int64_t(h->nRep) * A.nInstr, 2, done);
-    FuseArgs F{h->v, h->u, &S->a1_cx, h->sqPartialU, h->xPack, h->texV, h->texPack, h->xPack4};
+    FuseArgs F{h->v, h->u, &S->a1_cx, h->sqPartialU, h->xPack, h->texV, h->texPack};
     launchAprod2Main<true>(h, A, h->u, h->t, h->coefRaw, done, F);
     int nk = 10, npU = h->gridA2m;
     if (A.nCon > 0) {   // constraint rows: their part of u^ and of sum u^2, then (below) of t
@@ -691,7 +699,11 @@ int enqueueIterationFused(gsr_handle *h)
         nk += 2;
     }
     k_scalar<<<1, 256, 0, st>>>(PH_AFTER_APROD1, S, h->sqPartialU, npU, nullptr, 0);
-    launchAtt(h, A, h->u, h->t, h->coefRaw, done);
+    if (h->useUT) {   // u^ into block-time order first: the attitude kernel then streams it
+        k_u_to_time<<<h->gridUT, 256, 0, st>>>(h->u, h->permT, A.m, h->uT, done);
+        launchAtt(h, A, h->uT, h->t, h->coefRaw, done, true);
+        ++nk;
+    } else launchAtt(h, A, h->u, h->t, h->coefRaw, done);
     k_astro_fixup<<<h->gridFix, 256, 0, st>>>(A, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial,
                                               h->gridA2m, done);
     // after the fix-up: it overwrites the astro entries of stars cut by a tile edge
@@ -960,8 +972,8 @@ int32_t gsr_bench_set(gsr_handle *h, const char *key, int64_t value)
     if (k == "ins_sm_fused" && value >= 0 && value <= h->nInsSm) h->nInsSmFused = int(value);
     else if (k == "n_rep" && value >= 1 && value <= h->nRepAlloc) h->nRep = int(value);
     else if (k == "att_ctas_per_sm" && value >= 1 && value <= 16) h->gridAtt = gridFor(h->nTiles, 8, h->smCount * int(value));
-    else if (k == "coop" && (value == 0 || value == 1)) h->coop = value != 0;
-    else if (k == "att_merge" && (value == 0 || value == 1)) h->attMerge = value != 0;
+    else if (k == "use_ut" && (value == 0 || (value == 1 && h->uT))) h->useUT = value != 0;
+    else if (k == "ut_ctas_per_sm" && value >= 1 && value <= 16) h->gridUT = gridFor(h->L.n_obs, 256, h->smCount * int(value));
     else return fail(h, GSR_EINVAL, "gsr_bench_set: unknown key or value out of range: %s = %lld", key, (long long)value);
     if (h->iterGraph) {
         cudaGraphExecDestroy(h->iterGraph);
@@ -988,7 +1000,6 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
     CK(cudaMemcpyAsync(h->u, h->b, size_t(h->mTot) * sizeof(double), cudaMemcpyDeviceToDevice, st));
     k_fill<<<h->gridVec, 256, 0, st>>>(h->v, h->n, 1e-3);
     k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, nullptr);   // operand of k_aprod1 / the fused pass timed alone
-    if (h->coop) k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, nullptr, h->xPack4);
     k_pre_aprod2<<<h->gridVec, 256, 0, st>>>(h->t, 0, A.n, h->coefRaw, h->insRep, int64_t(h->nRep) * A.nInstr, 2, nullptr);
     auto once = [&]() {
         if (which == GSR_TIME_APROD1_GROUP) enqueueAprod1(h, h->v, h->u, h->coefTime, h->sqPartialU, nullptr, nullptr);
@@ -996,15 +1007,15 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
         else if (which == GSR_TIME_K_APROD1)
             launchAprod1(h, A, h->v, h->u, h->coefTime, h->sqPartialU, nullptr);
         else if (which == GSR_TIME_K_APROD2_ATT)
-            launchAtt(h, A, h->u, h->v, h->coefTime, nullptr);
+            launchAtt(h, A, h->useUT ? h->uT : h->u, h->v, h->coefTime, nullptr, h->useUT);
         else if (which == GSR_TIME_K_FUSED) {   // the fused pass of gsr_lsqr alone: u <- 0.5 u + 0.5 A v, t += A^T u (main sections)
             MatView Af = A;
             Af.nInsSm = h->nInsSmFused;
-            FuseArgs F{h->v, h->u, h->coefTime, h->sqPartialU, h->xPack, h->texV, h->texPack, h->xPack4};
+            FuseArgs F{h->v, h->u, h->coefTime, h->sqPartialU, h->xPack, h->texV, h->texPack};
             launchAprod2Main<true>(h, Af, h->u, h->t, h->coefRaw, nullptr, F);
         }
         else if (h->useAttT)
-            launchAprod2Main<false>(h, A, h->u, h->v, h->coefTime, nullptr, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, nullptr});
+            launchAprod2Main<false>(h, A, h->u, h->v, h->coefTime, nullptr, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0});
         else
             launchAprod2Red<false>(h, A, h->u, h->v, h->coefTime, nullptr);
     };

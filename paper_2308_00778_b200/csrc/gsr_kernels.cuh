@@ -11,7 +11,6 @@ constexpr int N_ASTRO = 5, N_ATT = 12, N_INSTR = 6, N_PAR = 24;
 constexpr int TILE = 32;          // rows per warp tile
 constexpr int WARPS = 8;          // warps per CTA of the aprod kernels
 constexpr int THREADS = WARPS * 32;
-constexpr int ATT_WIN = 64;          // coefficients per axis of the per-warp window of k_aprod2_att
 constexpr int ATT_BLOCK_BITS = 21;   // rows per block of the time-ordered attitude copy (2^21)
 
 // Device layout of the coefficients ("tile-transposed"): the 32 rows of a warp tile are stored
@@ -25,7 +24,13 @@ __host__ __device__ __forceinline__ int64_t cpos(int64_t i, int j) { return ((i 
 // Device view of the uploaded system (A_d, M_i, I_c) in upload layout.
 struct MatView {
     double *V;             // [nTiles*24*32] tile-transposed, see vpos()
-    const int32_t *star;   // [m] star of the row (matrixIndexAstro / 5; -1: the uploaded value broke its contract)
+    const int32_t *star;   // [m] star of the row (matrixIndexAstro / 5; -1: the uploaded value broke its contract);
+                           // upload scratch only: validated, turned into rp and tw, then freed
+    const unsigned long long *tw;   // [nTiles] "tile word" (the star row pointer in place of a per-row
+                           // star index, 0.25 B/row): bits 0-31 head mask (bit l: row l of the tile starts a star; bit 0
+                           // refers to the last row of the previous tile), bits 32-60 star of the tile's first row,
+                           // bit 61: the star of the tile's last row goes on in the next tile, bit 62: some star between
+                           // two rows of the tile has no rows (star of a lane then comes from a search in rp)
     const int32_t *iatt;   // [m] attitude start s_i (axis 0; -1: out of range) -- SURVEY 8(f) NEXT-2: 4-byte indices
     const int32_t *ic;     // [nTiles*6*32] tile-transposed, see cpos(); nullptr when ic16 is in use
     const uint16_t *ic16;  // the same as 2-byte columns when nInstr <= 65536 (-12 B/row)
@@ -61,6 +66,23 @@ struct Scalars {
     int istop;
     int done;              // 1: loop body is a no-op (stopped, or trivial system)
 };
+
+constexpr int TW_STAR_BITS = 29;   // n_stars < 2^29
+__device__ __forceinline__ int64_t star_search(const int64_t *__restrict__ rp, int64_t nStars, int64_t i)
+{
+    int64_t lo = 0, hi = nStars;   // largest s with rp[s] <= i among stars that own rows: first s with rp[s+1] > i
+    while (lo < hi) {
+        const int64_t mid = (lo + hi) >> 1;
+        if (rp[mid + 1] <= i) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+// star of row (tile, lane) from the tile word
+__device__ __forceinline__ int64_t star_of(const MatView &A, unsigned long long w, int64_t i, int lane)
+{
+    if ((w >> 62) & 1ull) return star_search(A.rp, A.nStars, i);
+    return int64_t((w >> 32) & ((1ull << TW_STAR_BITS) - 1)) + __popc(uint32_t(w) & (0xffffffffu >> (31 - lane)) & 0xfffffffeu);
+}
 
 __device__ __forceinline__ double warp_sum(double v)
 {
@@ -126,19 +148,9 @@ __device__ __forceinline__ int32_t ic_at(const MatView &A, int64_t pos) { return
 // axis, so that the 12 unknowns of a row (3 axes x 4 consecutive starts; the paper keeps the axes N_DFA
 // apart) are one contiguous 96-byte run: 3-4 L2 sectors per row instead of 5-6, and the
 // 12 gathers of a lane fall into one or two L1 lines.  24 MB copied per product (~15 us).
-__global__ void k_pack_att(MatView A, const double *__restrict__ x, double *__restrict__ xPack, const int *done,
-                           double *__restrict__ xPack4 = nullptr)
+__global__ void k_pack_att(MatView A, const double *__restrict__ x, double *__restrict__ xPack, const int *done)
 {
     if (done && *done) return;
-    if (xPack4) {   // [s][4] = {axis0, axis1, axis2, 0}: the layout the cooperative gather of the fused pass reads
-        for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < A.nDof * 4;
-             e += int64_t(gridDim.x) * blockDim.x) {
-            const int64_t s = e >> 2;
-            const int a = int(e & 3);
-            xPack4[e] = a < 3 ? x[A.offAtt + a * A.nDof + s] : 0.0;
-        }
-        return;
-    }
     const int64_t total = A.nDof * 3;
     for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < total;
          e += int64_t(gridDim.x) * blockDim.x) {
@@ -170,7 +182,7 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
             const int64_t i = r0 + lane;
             double v[N_PAR];
             load_row<true>(A.V, tile, lane, v);
-            const double *xa = x + 5 * int64_t(__ldcs(A.star + i));
+            const double *xa = x + 5 * star_of(A, __ldg(A.tw + tile), i, lane);
             const int64_t iatt = __ldcs(A.iatt + i);
             int32_t c[N_INSTR];
             load_ic<IC16>(A, tile, lane, c);
@@ -232,15 +244,7 @@ struct FuseArgs {
     const double *xPack;   // FUSE_ATT: attitude unknowns of xin interleaved by axis (k_pack_att)
     cudaTextureObject_t texX;     // 0, or xin as a linear texture of int2 (gathers through the TEX path)
     cudaTextureObject_t texPack;  // 0, or xPack likewise
-    const double *xPack4;  // COOP: attitude unknowns as [s][4] = {axis0, axis1, axis2, 0}: a row's 12 unknowns are 4
-                           // consecutive 32-byte sectors, fetched by 4 lanes with one 256-bit load each
 };
-constexpr int COOP_STRIDE = 33;                      // doubles per (offset, axis) line of the per-warp exchange buffer
-constexpr int COOP_WARP = N_ATT * COOP_STRIDE;       // doubles per warp
-__device__ __forceinline__ void ld256_na(const double *p, double &a, double &b, double &c, double &d)
-{
-    asm volatile("ld.global.nc.L1::no_allocate.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p));
-}
 __device__ __forceinline__ double tex_f64(cudaTextureObject_t t, int64_t idx)
 {
     const int2 q = tex1Dfetch<int2>(t, int(idx));
@@ -248,20 +252,15 @@ __device__ __forceinline__ double tex_f64(cudaTextureObject_t t, int64_t idx)
 }
 // FUSE_ATT: the attitude terms of A*xin are gathered here too, in star order (whole aprod1 in this pass,
 // y <- cy*y + cx*(A xin)); without it yrw must already hold cy*y + cx*(attitude terms).
-// COOP (with FUSE_ATT): the attitude unknowns of a row are fetched cooperatively -- lanes 4q..4q+3 load the four
-// 32-byte sectors of row q's run of xPack4 with one LDG.256 each (8 rows per instruction, 4 instructions per tile) and
-// the values reach their row's lane through a per-warp shared-memory buffer: one or two L2 requests per row instead
-// of ~3.75 single-sector ones, and the attitude gathers no longer need L1.
-template <bool IC16, bool SQUARE, bool ATT_RED, bool PRIV = false, bool MATCH = false, bool FUSE = false, bool FUSE_ATT = false,
-          bool COOP = false>
+template <bool IC16, bool SQUARE, bool ATT_RED, bool PRIV = false, bool MATCH = false, bool FUSE = false, bool FUSE_ATT = false>
 __global__ void __launch_bounds__(PRIV ? PRIV_THREADS : THREADS, PRIV ? 1 : 2)
 k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
          const double *__restrict__ coef, double *__restrict__ carryFirst,
          double *__restrict__ carryLast, double *__restrict__ globPartial, const int *done,
-         FuseArgs F = FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0, nullptr})
+         FuseArgs F = FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0})
 {
     __shared__ double red[32];
-    extern __shared__ double sIns[];   // PRIV: nInsSm private instrument accumulators (+ COOP: exchange buffers)
+    extern __shared__ double sIns[];   // PRIV: nInsSm private instrument accumulators
     if (done && *done) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int nWarpsCta = PRIV ? PRIV_THREADS / 32 : WARPS;
@@ -287,36 +286,12 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         const int64_t i = r0 + (valid ? lane : nrows - 1);
         double v[N_PAR];
         load_row<ATT_RED || FUSE_ATT>(A.V, tile, valid ? lane : nrows - 1, v);
-        const int64_t ia = 5 * int64_t(__ldcs(A.star + i));
+        const unsigned long long tw = __ldg(A.tw + tile);   // one 8-byte word per tile: first star, head mask, cut flags
+        const int64_t ia = 5 * star_of(A, tw, i, valid ? lane : nrows - 1);
         // padded storage: the lanes past the last row read column 0 and a zero coefficient
         int32_t c[N_INSTR];
         load_ic<IC16>(A, tile, lane, c);
-        // astro index of the rows just before and just after the tile (-1: none), fetched with the
-        // tile's other loads instead of after the scan
-        const int64_t iaBefore = r0 > 0 ? 5 * int64_t(__ldg(A.star + r0 - 1)) : int64_t(-1);
-        const int64_t iaAfter = r0 + nrows < A.m ? 5 * int64_t(__ldg(A.star + r0 + nrows)) : int64_t(-1);
         double yv = 0.0;
-        double xatt[COOP ? N_ATT : 1];     // COOP: xatt[3*j + a] = unknown of axis a at start + j
-        int64_t iattRow = 0;
-        if (FUSE_ATT) iattRow = __ldcs(A.iatt + i);
-        if (COOP) {
-            double *buf = sIns + ((A.nInsSm + 1) & ~1) + warp * COOP_WARP;
-            const int p = lane & 3;
-#pragma unroll
-            for (int r = 0; r < 4; ++r) {
-                const int q = 8 * r + (lane >> 2);
-                const int64_t sq = __shfl_sync(0xffffffffu, iattRow, q);
-                double d0, d1, d2, d3;
-                ld256_na(F.xPack4 + (sq + p) * 4, d0, d1, d2, d3);
-                buf[(3 * p + 0) * COOP_STRIDE + q] = d0;
-                buf[(3 * p + 1) * COOP_STRIDE + q] = d1;
-                buf[(3 * p + 2) * COOP_STRIDE + q] = d2;
-            }
-            __syncwarp();
-#pragma unroll
-            for (int k = 0; k < N_ATT; ++k) xatt[k] = buf[k * COOP_STRIDE + lane];
-            __syncwarp();
-        }
         if (FUSE) {
             if (valid) {
                 const double *xa = F.xin + ia, *xIn = F.xin + A.offInstr;
@@ -331,21 +306,15 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
                 sum = fma(v[23], xg1, sum);
                 double yOld = F.yrw[i];
                 if (FUSE_ATT) {
-                    if (COOP) {
+                    const int64_t iattRow = __ldcs(A.iatt + i);
+                    const double *xp = F.xPack + 3 * iattRow;
 #pragma unroll
-                        for (int j = 0; j < 4; ++j)
+                    for (int j = 0; j < 4; ++j)
 #pragma unroll
-                            for (int a = 0; a < 3; ++a) sum = fma(v[5 + 4 * a + j], xatt[3 * j + a], sum);
-                    } else {
-                        const double *xp = F.xPack + 3 * iattRow;
-#pragma unroll
-                        for (int j = 0; j < 4; ++j)
-#pragma unroll
-                            for (int a = 0; a < 3; ++a) {
-                                const double xa3 = F.texPack ? tex_f64(F.texPack, 3 * iattRow + 3 * j + a) : __ldg(xp + 3 * j + a);
-                                sum = fma(v[5 + 4 * a + j], xa3, sum);
-                            }
-                    }
+                        for (int a = 0; a < 3; ++a) {
+                            const double xa3 = F.texPack ? tex_f64(F.texPack, 3 * iattRow + 3 * j + a) : __ldg(xp + 3 * j + a);
+                            sum = fma(v[5 + 4 * a + j], xa3, sum);
+                        }
                     yOld *= F.coef1[1];
                 }
                 const double yi = fma(cx1, sum, yOld);
@@ -398,11 +367,8 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         gsum += warp_sum(v[23]);
 
         // ---- astro: segmented scan by star over the tile's rows
-        const int64_t iaPrev = __shfl_up_sync(0xffffffffu, ia, 1);
-        const int64_t iaNext = __shfl_down_sync(0xffffffffu, ia, 1);
-        const bool head = (lane == 0) || (ia != iaPrev);
-        const bool tail = valid && ((lane == nrows - 1) || (ia != iaNext));
-        const unsigned heads = __ballot_sync(0xffffffffu, head);
+        const unsigned heads = uint32_t(tw) | 1u;          // segment starts inside the tile (lane 0 always opens one)
+        const bool tail = valid && ((lane == nrows - 1) || ((heads >> 1) >> lane) & 1u);
         const int segStart = 31 - __clz(heads & (0xffffffffu >> (31 - lane)));
         const int dist = lane - segStart;
         double s[N_ASTRO];
@@ -418,8 +384,8 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         }
         if (tail) {
             bool cut = false;
-            if (segStart == 0) cut = (iaBefore == ia);
-            if (lane == nrows - 1) cut = cut || (iaAfter == ia);
+            if (segStart == 0) cut = !(uint32_t(tw) & 1u);            // the star began in an earlier tile
+            if (lane == nrows - 1) cut = cut || ((tw >> 61) & 1ull);   // and / or goes on in the next one
             if (!cut) {
                 double *xa = x + ia;
 #pragma unroll
@@ -526,12 +492,12 @@ __global__ void k_pre_aprod2(double *__restrict__ x, int64_t lo, int64_t hi,
 // segmented scan by s over the tile leaves one sum per (s, axis, j) and only those are added to x
 // (RED), instead of 12 REDs per row.  y is gathered through permT (one 8-byte gather per row).
 // ---------------------------------------------------------------------------------------
-template <bool SQUARE, bool MERGE = true>
+// LINEAR: y is already in block-time order (the uT copy written by the fused pass): no permT, no gather, no prefetch.
+template <bool SQUARE, bool LINEAR = false>
 __global__ void __launch_bounds__(256)
 k_aprod2_att(MatView A, const double *__restrict__ y, double *__restrict__ x,
              const double *__restrict__ coef, const int *done)
 {
-    __shared__ double win[MERGE ? 8 : 1][3 * ATT_WIN];
     if (done && *done) return;
     const int lane = threadIdx.x & 31;
     const double cy = coef[1];
@@ -548,10 +514,10 @@ k_aprod2_att(MatView A, const double *__restrict__ y, double *__restrict__ x,
         // The gathers below land anywhere in this block's slice of y.  Pull the NEXT block's slice
         // into L2 linearly while this block is processed (one 32-byte sector per 4 rows): first touches
         // that arrive together are not merged by L2 and would each go to DRAM (measured).
-        if (!SQUARE && (lane & 3) == 0 && t + (int64_t(1) << ATT_BLOCK_BITS) < A.m)
+        if (!SQUARE && !LINEAR && (lane & 3) == 0 && t + (int64_t(1) << ATT_BLOCK_BITS) < A.m)
             asm volatile("prefetch.global.L2 [%0];" ::"l"(y + t + (int64_t(1) << ATT_BLOCK_BITS)));
         double yv = 0.0;
-        if (valid) yv = SQUARE ? 1.0 : cy * __ldg(y + __ldcs(A.permT + t));
+        if (valid) yv = SQUARE ? 1.0 : cy * (LINEAR ? __ldcs(y + t) : __ldg(y + __ldcs(A.permT + t)));
         double v[N_ATT];
 #pragma unroll
         for (int k = 0; k < N_ATT; ++k) {
@@ -585,40 +551,7 @@ k_aprod2_att(MatView A, const double *__restrict__ y, double *__restrict__ x,
                     if (dist >= d) v[k] += t2;
                 }
             }
-            // The 4-wide windows of neighbouring starts overlap (start s touches coefficients s..s+3 of each axis):
-            // when the tile's starts span less than ATT_WIN coefficients, the per-start sums are first added into a
-            // per-warp shared-memory window (tails have distinct s, so for a fixed j they hit distinct words: plain
-            // read-modify-write, one j at a time) and each coefficient of the window gets ONE RED per axis instead of
-            // one per (start, j): ~3x fewer REDs at Medium (16 starts per tile -> 3 x 19 instead of 16 x 12).
-            const int32_t sMin = __shfl_sync(0xffffffffu, sv, 0);
-            const int32_t span = __shfl_sync(0xffffffffu, sv, 31) - sMin + 4;
-            if (MERGE && span <= ATT_WIN) {
-                double *w = win[threadIdx.x >> 5];
-#pragma unroll
-                for (int q = 0; q < 3 * ATT_WIN / 32; ++q) w[q * 32 + lane] = 0.0;
-                __syncwarp();
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    if (tail) {
-                        double *wj = w + (sv - sMin + j);
-#pragma unroll
-                        for (int a = 0; a < 3; ++a) wj[a * ATT_WIN] += v[4 * a + j];
-                    }
-                    __syncwarp();
-                }
-#pragma unroll
-                for (int q = 0; q < ATT_WIN / 32; ++q) {
-                    const int idx = q * 32 + lane;
-                    if (idx < span) {
-#pragma unroll
-                        for (int a = 0; a < 3; ++a) {
-                            const double t2 = w[a * ATT_WIN + idx];
-                            if (t2 != 0.0) atomicAdd(xAtt + int64_t(a) * A.nDof + sMin + idx, t2);
-                        }
-                    }
-                }
-                __syncwarp();
-            } else if (tail) {
+            if (tail) {
 #pragma unroll
                 for (int a = 0; a < 3; ++a)
 #pragma unroll
@@ -678,6 +611,23 @@ __global__ void k_scale_attT(MatView A, const double *__restrict__ p)
             const int64_t e = int64_t(kk) * A.m + t;
             A.attT[e] = A.attT[e] * pc[(kk >> 2) * A.nDof + (kk & 3)];
         }
+    }
+}
+
+// uT[t] = u[permT[t]]: u^ brought into block-time order for k_aprod2_att<.., LINEAR>.  A pass of its own: the gather
+// (inside the block's 16 MB slice of u, pulled into L2 linearly one block ahead as in k_aprod2_att) runs with far more
+// parallelism here than as a dependent step of the attitude kernel, and the writes are coalesced.
+__global__ void __launch_bounds__(256)
+k_u_to_time(const double *__restrict__ u, const uint32_t *__restrict__ permT, int64_t m, double *__restrict__ uT,
+            const int *done)
+{
+    if (done && *done) return;
+    // one row per thread: four rows per thread with the gathers batched ran 2 ms slower (the gathers then outrun the
+    // linear prefetch of the next block and their first touches go to DRAM one by one)
+    for (int64_t t = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; t < m; t += int64_t(gridDim.x) * blockDim.x) {
+        if ((t & 3) == 0 && t + (int64_t(1) << ATT_BLOCK_BITS) < m)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(u + t + (int64_t(1) << ATT_BLOCK_BITS)));
+        uT[t] = __ldg(u + __ldcs(permT + t));
     }
 }
 
@@ -953,6 +903,31 @@ __global__ void k_star_rowptr(const int32_t *__restrict__ star, int64_t m, int64
     rp[s] = lo;
 }
 
+// tw[tile] from the validated per-row star array (see MatView::tw)
+__global__ void k_tile_words(const int32_t *__restrict__ star, int64_t m, unsigned long long *__restrict__ tw)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t nTiles = (m + TILE - 1) / TILE;
+    for (int64_t tile = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) >> 5; tile < nTiles;
+         tile += (int64_t(gridDim.x) * blockDim.x) >> 5) {
+        const int64_t r0 = tile * TILE;
+        const int nrows = int(min(int64_t(TILE), m - r0));
+        const int64_t i = r0 + min(lane, nrows - 1);
+        const int32_t s = star[i];
+        const int32_t sp = i > 0 ? star[i - 1] : -1;
+        const bool head = lane < nrows && s != sp;
+        const bool gap = lane < nrows && lane > 0 && s > sp + 1;
+        const unsigned hm = __ballot_sync(0xffffffffu, head);
+        const unsigned gm = __ballot_sync(0xffffffffu, gap);
+        if (lane == 0) {
+            const int64_t last = r0 + nrows - 1;
+            const bool contNext = last + 1 < m && star[last + 1] == star[last];
+            tw[tile] = (unsigned long long)hm | ((unsigned long long)uint32_t(s) << 32) | (contNext ? 1ull << 61 : 0ull) |
+                       (gm ? 1ull << 62 : 0ull);
+        }
+    }
+}
+
 // Upload: matrixIndexAstro / matrixIndexAtt (i64, "M_i") -> 4-byte star and attitude start;
 // a value that breaks its contract becomes -1 and is reported by k_validate.
 __global__ void k_ingest_index(int64_t cnt, const int64_t *__restrict__ ia, const int64_t *__restrict__ iatt,
@@ -1006,7 +981,7 @@ __global__ void k_scale_values(MatView A, const double *__restrict__ p)
         const int64_t i = tile * TILE + (e & 31);
         if (i >= A.m) continue;
         int64_t c;
-        if (k < N_ASTRO) c = 5 * int64_t(A.star[i]) + k;
+        if (k < N_ASTRO) c = 5 * star_of(A, A.tw[tile], i, int(e & 31)) + k;
         else if (k < N_ASTRO + N_ATT) c = A.offAtt + ((k - N_ASTRO) >> 2) * A.nDof + A.iatt[i] + ((k - N_ASTRO) & 3);
         else if (k < N_PAR - 1) c = A.offInstr + ic_at(A, cpos(i, k - N_ASTRO - N_ATT));
         else c = A.offGlob;
