@@ -197,12 +197,14 @@ int32_t gsr_get_trace(gsr_handle *h, double *out, int64_t max_itn, int64_t *n_wr
  * attitude copy in use, bit 1 = fused single-pass iteration, bit 2 = warp-level
  * pre-summation of equal instrument columns (chosen from the column histogram at
  * upload), bit 3 = texture gathers in the fused pass, bit 4 = 2-byte instrument
- * columns on the device. */
+ * columns on the device, bit 5 = the fused iteration keeps a copy of u in block-time
+ * order for the attitude kernel (+8 B/row of HBM; dropped when it does not fit). */
 #define GSR_PATH_ATT_COPY 1
 #define GSR_PATH_FUSED 2
 #define GSR_PATH_INSTR_MATCH 4
 #define GSR_PATH_TEX 8
 #define GSR_PATH_IC16 16
+#define GSR_PATH_UT 32
 int32_t gsr_path_info(const gsr_handle *h);
 
 /* Device time of the last gsr_lsqr's iteration loop in milliseconds (CUDA events on

@@ -22,7 +22,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "gsr_oracle.c")
 _LIB = os.path.join(_HERE, "libgsr_oracle.so")
 
-N_PAR = 24
+N_PAR = 24          # row width of the production layout (n_glob = 1); in general 23 + n_glob
 
 
 def build(force: bool = False) -> str:
@@ -39,7 +39,7 @@ def build(force: bool = False) -> str:
 class _Sys(C.Structure):
     _fields_ = [
         ("n_obs", C.c_int64), ("n_stars", C.c_int64), ("n_dof_att", C.c_int64),
-        ("n_instr", C.c_int64), ("n_con", C.c_int64),
+        ("n_instr", C.c_int64), ("n_con", C.c_int64), ("n_glob", C.c_int64),
         ("V", C.c_void_p), ("ia", C.c_void_p), ("iatt", C.c_void_p), ("ic", C.c_void_p),
         ("con_rowptr", C.c_void_p), ("con_col", C.c_void_p), ("con_val", C.c_void_p),
     ]
@@ -132,15 +132,17 @@ class LsqrResult:
 class OracleSystem:
     """Holds (private copies of) the upload-format arrays of one system.
 
-    values [m,24] f64 row-major; matrixIndexAstro [m] i64 (= 5*star, non-decreasing);
+    values [m,23+n_glob] f64 row-major; matrixIndexAstro [m] i64 (= 5*star, non-decreasing);
     matrixIndexAtt [m] i64 (axis-0 start); instrCol [m,6] i32; optional constraint rows
-    as CSR with absolute columns.
+    as CSR with absolute columns.  n_glob = 1 is the paper's production layout (24 per row).
     """
 
     def __init__(self, n_stars, n_dof_att, n_instr, values, matrixIndexAstro, matrixIndexAtt,
-                 instrCol, con_rowptr=None, con_col=None, con_val=None):
+                 instrCol, con_rowptr=None, con_col=None, con_val=None, n_glob=1):
         self.lib = _load()
-        self.V = np.array(values, dtype=np.float64, order="C", copy=True).reshape(-1, N_PAR)
+        self.n_glob = int(n_glob)
+        self.n_par = 23 + self.n_glob
+        self.V = np.array(values, dtype=np.float64, order="C", copy=True).reshape(-1, self.n_par)
         self.m = self.V.shape[0]
         self.ia = np.array(matrixIndexAstro, dtype=np.int64, copy=True).reshape(-1)
         self.iatt = np.array(matrixIndexAtt, dtype=np.int64, copy=True).reshape(-1)
@@ -158,7 +160,7 @@ class OracleSystem:
             self.con_val = np.zeros(0, dtype=np.float64)
             self.n_con = 0
         self.p = None
-        self._s = _Sys(self.m, self.n_stars, self.n_dof_att, self.n_instr, self.n_con,
+        self._s = _Sys(self.m, self.n_stars, self.n_dof_att, self.n_instr, self.n_con, self.n_glob,
                        _ptr(self.V), _ptr(self.ia), _ptr(self.iatt), _ptr(self.ic),
                        _ptr(self.con_rowptr), _ptr(self.con_col), _ptr(self.con_val))
         self._sp = C.addressof(self._s)

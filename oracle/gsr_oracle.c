@@ -26,14 +26,15 @@
  *                                 (k <= 20), upper bound diag((A'^T A')^-1), scipy var
  *
  * Matrix definition (PAPER.md:78-80 and the index expressions
- * of Algorithm 2, PAPER.md:339, 360-362, 373, 393, 398, 418).  Row i of A holds
- * 24 stored coefficients V[i*24 + k], k = 0..23, in the section order
- *   [ 5 astrometric | 12 attitude = 3 axes x 4 | 6 instrumental | 1 global ]
- * and coefficient k sits in column
+ * of Algorithm 2, PAPER.md:339, 360-362, 373, 393, 398, 418, 451).  Row i of A holds
+ * N_par = 23 + nGlob stored coefficients V[i*N_par + k] in the section order
+ *   [ 5 astrometric | 12 attitude = 3 axes x 4 | 6 instrumental | nGlob global ]
+ * (nGlob = 1, N_par = 24 in the paper's production layout; the paper
+ * also ran 5 global parameters, and allows 0) and coefficient k sits in column
  *   k <  5 : ia[i] + k                                   (ia[i] = 5*star(i))
  *   k < 17 : 5*nStars + a*nDofAtt + iatt[i] + j          a=(k-5)/4, j=(k-5)%4
  *   k < 23 : 5*nStars + 3*nDofAtt + ic[i*6 + (k-17)]
- *   k = 23 : 5*nStars + 3*nDofAtt + nInstr
+ *   k >= 23: 5*nStars + 3*nDofAtt + nInstr + (k-23)      (Alg. 2 "glob": x[j + offset])
  * Constraint rows are generic sparse rows appended below
  * the observation rows, given as CSR (rowptr, col, val) with absolute columns.
  */
@@ -47,8 +48,7 @@
 #define N_PAR_AXIS 4
 #define N_ATT (N_AXES * N_PAR_AXIS)
 #define N_INSTR 6
-#define N_GLOB 1
-#define N_PAR (N_ASTRO + N_ATT + N_INSTR + N_GLOB) /* 24 */
+#define N_FIXED (N_ASTRO + N_ATT + N_INSTR) /* 23; N_par = 23 + n_glob = 24 for n_glob = 1 */
 
 typedef struct {
     int64_t n_obs;      /* observation rows m                                  */
@@ -56,7 +56,8 @@ typedef struct {
     int64_t n_dof_att;  /* N_DFA, per axis                                     */
     int64_t n_instr;    /* number of instrumental columns                      */
     int64_t n_con;      /* constraint rows                                     */
-    double *V;          /* [n_obs*24] row-major A_d              */
+    int64_t n_glob;     /* N_Glob global columns (1 in production)*/
+    double *V;          /* [n_obs*N_par] row-major A_d           */
     const int64_t *ia;  /* [n_obs]   M_i astro part: 5*star, non-decreasing    */
     const int64_t *iatt;/* [n_obs]   M_i attitude part: start s_i, axis 0      */
     const int32_t *ic;  /* [n_obs*6] I_c instrumental columns                  */
@@ -67,8 +68,10 @@ typedef struct {
 
 int64_t gsr_oracle_ncols(const gsr_oracle_system *S)
 {
-    return N_ASTRO * S->n_stars + N_AXES * S->n_dof_att + S->n_instr + N_GLOB;
+    return N_ASTRO * S->n_stars + N_AXES * S->n_dof_att + S->n_instr + S->n_glob;
 }
+
+static int npar(const gsr_oracle_system *S) { return N_FIXED + (int)S->n_glob; }
 
 /* Column of stored coefficient k of observation row i (see header). */
 int64_t gsr_oracle_col(const gsr_oracle_system *S, int64_t i, int k)
@@ -84,7 +87,7 @@ int64_t gsr_oracle_col(const gsr_oracle_system *S, int64_t i, int k)
     }
     if (k < N_ASTRO + N_ATT + N_INSTR)
         return off_instr + S->ic[i * N_INSTR + (k - N_ASTRO - N_ATT)];
-    return off_glob;
+    return off_glob + (k - N_FIXED);
 }
 
 /*
@@ -96,6 +99,7 @@ int64_t gsr_oracle_col(const gsr_oracle_system *S, int64_t i, int k)
  */
 void gsr_oracle_aprod1(const gsr_oracle_system *S, const double *x, double *y, double *abs_y)
 {
+    const int N_PAR = npar(S);
     for (int64_t i = 0; i < S->n_obs; ++i) {
         double sum = 0.0, asum = 0.0;
         for (int k = 0; k < N_PAR; ++k) {
@@ -128,6 +132,7 @@ void gsr_oracle_aprod1(const gsr_oracle_system *S, const double *x, double *y, d
 void gsr_oracle_aprod2(const gsr_oracle_system *S, const double *y, double *x, double *abs_x)
 {
     const int64_t n = gsr_oracle_ncols(S);
+    const int N_PAR = npar(S);
     if (abs_x)
         for (int64_t j = 0; j < n; ++j)
             abs_x[j] = fabs(x[j]);
@@ -182,6 +187,7 @@ double gsr_oracle_norm(const double *a, int64_t n)
 void gsr_oracle_precondition(gsr_oracle_system *S, double *p)
 {
     const int64_t n = gsr_oracle_ncols(S);
+    const int N_PAR = npar(S);
     for (int64_t j = 0; j < n; ++j)
         p[j] = 0.0;
     for (int64_t i = 0; i < S->n_obs; ++i)

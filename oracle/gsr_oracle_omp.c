@@ -20,11 +20,11 @@
 #include <stdlib.h>
 #include <string.h>
 
-enum { NA = 5, NAX = 3, NPA = 4, NATT = 12, NI = 6, NP = 24 };
+enum { NA = 5, NAX = 3, NPA = 4, NATT = 12, NI = 6, NF = 23 };   /* row width 23 + n_glob */
 
 /* same field order as gsr_oracle_system (oracle/__init__.py passes one ctypes struct to both) */
 typedef struct {
-    int64_t n_obs, n_stars, n_dof_att, n_instr, n_con;
+    int64_t n_obs, n_stars, n_dof_att, n_instr, n_con, n_glob;
     double *V;
     const int64_t *ia, *iatt;
     const int32_t *ic;
@@ -32,7 +32,7 @@ typedef struct {
     double *con_val;
 } omp_system;
 
-static int64_t ncols(const omp_system *S) { return NA * S->n_stars + NAX * S->n_dof_att + S->n_instr + 1; }
+static int64_t ncols(const omp_system *S) { return NA * S->n_stars + NAX * S->n_dof_att + S->n_instr + S->n_glob; }
 
 int gsr_omp_threads(void) { return omp_get_max_threads(); }
 void gsr_omp_set_threads(int t) { omp_set_num_threads(t > 0 ? t : 1); }
@@ -41,6 +41,7 @@ void gsr_omp_set_threads(int t) { omp_set_num_threads(t > 0 ? t : 1); }
 void gsr_omp_aprod1(const omp_system *S, const double *x, double *y)
 {
     const int64_t offAtt = NA * S->n_stars, offIns = offAtt + NAX * S->n_dof_att, offGlob = offIns + S->n_instr;
+    const int NP = NF + (int)S->n_glob;
 #pragma omp parallel for schedule(static)
     for (int64_t i = 0; i < S->n_obs; ++i) {
         const double *v = S->V + i * NP;
@@ -49,7 +50,7 @@ void gsr_omp_aprod1(const omp_system *S, const double *x, double *y)
         for (int a = 0; a < NAX; ++a)
             for (int j = 0; j < NPA; ++j) sum += v[NA + a * NPA + j] * x[offAtt + a * S->n_dof_att + S->iatt[i] + j];
         for (int j = 0; j < NI; ++j) sum += v[NA + NATT + j] * x[offIns + S->ic[i * NI + j]];
-        sum += v[NP - 1] * x[offGlob];
+        for (int g = 0; g < S->n_glob; ++g) sum += v[NF + g] * x[offGlob + g];
         y[i] += sum;
     }
 #pragma omp parallel for schedule(static)
@@ -65,6 +66,7 @@ void gsr_omp_aprod2(const omp_system *S, const double *y, double *x)
 {
     const int64_t n = ncols(S), offAtt = NA * S->n_stars, offIns = offAtt + NAX * S->n_dof_att;
     const int64_t nShared = n - offAtt;
+    const int NP = NF + (int)S->n_glob;
     const int T = omp_get_max_threads();
     double *priv = (double *)calloc((size_t)T * (size_t)nShared, sizeof(double));
     int64_t *Nt = (int64_t *)malloc(sizeof(int64_t) * (size_t)(T + 1));
@@ -84,7 +86,7 @@ void gsr_omp_aprod2(const omp_system *S, const double *y, double *x)
             for (int a = 0; a < NAX; ++a)
                 for (int j = 0; j < NPA; ++j) p[a * S->n_dof_att + S->iatt[i] + j] += v[NA + a * NPA + j] * yi;
             for (int j = 0; j < NI; ++j) p[(offIns - offAtt) + S->ic[i * NI + j]] += v[NA + NATT + j] * yi;
-            p[nShared - 1] += v[NP - 1] * yi;
+            for (int g = 0; g < S->n_glob; ++g) p[nShared - S->n_glob + g] += v[NF + g] * yi;
         }
 #pragma omp barrier
 #pragma omp for schedule(static)

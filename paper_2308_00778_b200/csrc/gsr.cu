@@ -242,9 +242,9 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
         CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
         CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
         CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
-        // the fused kernel also gathers x: a 96 KB table leaves the rest of the SM's memory to L1 (measured at
-        // Medium: 0 / 3 k / 6 k / 12 k / 18 k / 24.5 k columns -> 22.3 / 22.5 / 22.8 / 22.4 / 22.7 / 24.4 ms per iteration)
-        h->nInsSmFused = std::min(h->nInsSm, 12288);
+        // the fused kernel also gathers x, which needs L1: the table takes 128 KB of the SM's 228 KB (measured at Medium,
+        // fused pass alone: 0 / 4 k / 8 k / 12 k / 16 k / 20 k columns -> 16.7 / 16.5 / 15.8 / 15.5 / 15.3 / 15.7 ms)
+        h->nInsSmFused = std::min(h->nInsSm, 16384);
         h->gridA2m = gridFor(h->nTiles, PRIV_THREADS / 32, h->smCount);
     }
     h->gridVec = gridFor(std::max(h->n, h->mTot), 256 * 4, h->smCount * 8);
@@ -954,6 +954,7 @@ int32_t gsr_path_info(const gsr_handle *h)
     if (h->instrSkewed) r |= GSR_PATH_INSTR_MATCH;
     if (h->texV && h->texPack) r |= GSR_PATH_TEX;
     if (h->ic16) r |= GSR_PATH_IC16;
+    if (canFuse(h) && h->useUT) r |= GSR_PATH_UT;
     return r;
 }
 

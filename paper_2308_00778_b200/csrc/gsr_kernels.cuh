@@ -5,6 +5,23 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <cstdio>
+
+// -DGSR_BOUNDS_CHECK (paper_2308_00778_b200.build.build(check=True) -> libgsr_check.so): every gather / scatter index
+// of the aprod kernels is checked against its section and the kernel traps on a violation.  compute-sanitizer is
+// closed on this pool; the parity tests are run against this build instead (profiles/r02_boundscheck.md).
+#ifdef GSR_BOUNDS_CHECK
+#define GSR_ASSERT(c)                                                                 \
+    do {                                                                              \
+        if (!(c)) {                                                                   \
+            printf("GSR_ASSERT failed: %s (%s:%d)\n", #c, __FILE__, __LINE__);        \
+            __trap();                                                                 \
+        }                                                                             \
+    } while (0)
+#else
+#define GSR_ASSERT(c) ((void)0)
+#endif
+
 namespace gsr {
 
 constexpr int N_ASTRO = 5, N_ATT = 12, N_INSTR = 6, N_PAR = 24;
@@ -186,6 +203,9 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
             const int64_t iatt = __ldcs(A.iatt + i);
             int32_t c[N_INSTR];
             load_ic<IC16>(A, tile, lane, c);
+            GSR_ASSERT(xa >= x && xa + N_ASTRO <= x + A.offAtt && iatt >= 0 && iatt + 4 <= A.nDof);
+#pragma unroll
+            for (int j = 0; j < N_INSTR; ++j) GSR_ASSERT(c[j] >= 0 && c[j] < A.nInstr);
             double sum = 0.0;
 #pragma unroll
             for (int k = 0; k < N_ASTRO; ++k) sum = fma(v[k], __ldg(xa + k), sum);
@@ -291,6 +311,9 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         // padded storage: the lanes past the last row read column 0 and a zero coefficient
         int32_t c[N_INSTR];
         load_ic<IC16>(A, tile, lane, c);
+        GSR_ASSERT(ia >= 0 && ia + N_ASTRO <= A.offAtt);
+#pragma unroll
+        for (int j = 0; j < N_INSTR; ++j) GSR_ASSERT(c[j] >= 0 && c[j] < A.nInstr);
         double yv = 0.0;
         if (FUSE) {
             if (valid) {
@@ -307,6 +330,7 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
                 double yOld = F.yrw[i];
                 if (FUSE_ATT) {
                     const int64_t iattRow = __ldcs(A.iatt + i);
+                    GSR_ASSERT(iattRow >= 0 && iattRow + 4 <= A.nDof);
                     const double *xp = F.xPack + 3 * iattRow;
 #pragma unroll
                     for (int j = 0; j < 4; ++j)
@@ -330,6 +354,7 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
 
         // ---- attitude + instrumental scatter (invalid lanes hold zeros and add nothing)
         if (ATT_RED && valid) {
+            GSR_ASSERT(A.iatt[i] >= 0 && A.iatt[i] + 4 <= A.nDof);
             double *xt = xAtt + A.iatt[i];
 #pragma unroll
             for (int a = 0; a < 3; ++a)
@@ -391,6 +416,7 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
 #pragma unroll
                 for (int k = 0; k < N_ASTRO; ++k) xa[k] = fma(cx, xa[k], s[k]);
             } else {
+                GSR_ASSERT(tile >= 0 && tile < nTiles);
                 double *c = (segStart == 0 ? carryFirst : carryLast) + tile * N_ASTRO;
 #pragma unroll
                 for (int k = 0; k < N_ASTRO; ++k) c[k] = s[k];
@@ -449,6 +475,7 @@ k_astro_fixup(MatView A, double *__restrict__ x, const double *__restrict__ coef
     const int64_t s = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
     if (s >= A.nStars) return;
     const int64_t r0 = A.rp[s], r1 = A.rp[s + 1];
+    GSR_ASSERT(r0 >= 0 && r0 <= r1 && r1 <= A.m);
     double *xa = x + s * N_ASTRO;
     if (r0 == r1) {
 #pragma unroll
@@ -511,6 +538,7 @@ k_aprod2_att(MatView A, const double *__restrict__ y, double *__restrict__ x,
         const bool valid = lane < nrows;
         const int64_t t = t0 + (valid ? lane : nrows - 1);
         const int32_t sv = __ldcs(A.sT + t);
+        GSR_ASSERT(sv >= 0 && int64_t(sv) + 4 <= A.nDof && (LINEAR || SQUARE || int64_t(A.permT[t]) < A.m));
         // The gathers below land anywhere in this block's slice of y.  Pull the NEXT block's slice
         // into L2 linearly while this block is processed (one 32-byte sector per 4 rows): first touches
         // that arrive together are not merged by L2 and would each go to DRAM (measured).
@@ -627,6 +655,7 @@ k_u_to_time(const double *__restrict__ u, const uint32_t *__restrict__ permT, in
     for (int64_t t = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; t < m; t += int64_t(gridDim.x) * blockDim.x) {
         if ((t & 3) == 0 && t + (int64_t(1) << ATT_BLOCK_BITS) < m)
             asm volatile("prefetch.global.L2 [%0];" ::"l"(u + t + (int64_t(1) << ATT_BLOCK_BITS)));
+        GSR_ASSERT(int64_t(permT[t]) < m);
         uT[t] = __ldg(u + __ldcs(permT + t));
     }
 }
@@ -658,8 +687,10 @@ k_con_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
     for (int64_t r = (int64_t(blockIdx.x) * blockDim.x + threadIdx.x) >> 5; r < A.nCon;
          r += (int64_t(gridDim.x) * blockDim.x) >> 5) {
         double sum = 0.0;
-        for (int64_t q = A.conRp[r] + lane; q < A.conRp[r + 1]; q += 32)
+        for (int64_t q = A.conRp[r] + lane; q < A.conRp[r + 1]; q += 32) {
+            GSR_ASSERT(A.conCol[q] >= 0 && A.conCol[q] < A.n);
             sum = fma(A.conVal[q], __ldg(x + A.conCol[q]), sum);
+        }
         sum = warp_sum(sum);
         if (lane == 0) {
             const double yi = fma(cy, y[A.m + r], cx * sum);
@@ -684,6 +715,7 @@ k_con_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         const double yv = SQUARE ? 1.0 : cy * y[A.m + r];
         for (int64_t q = A.conRp[r] + lane; q < A.conRp[r + 1]; q += 32) {
             const double v = A.conVal[q];
+            GSR_ASSERT(A.conCol[q] >= 0 && A.conCol[q] < A.n);
             atomicAdd(x + A.conCol[q], SQUARE ? v * v : v * yv);
         }
     }

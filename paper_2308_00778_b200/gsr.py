@@ -14,14 +14,15 @@ import numpy as np
 import torch
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_PKG, "libgsr.so")
+# GSR_LIBRARY selects another build of the same ABI (the bounds-checked libgsr_check.so); read by this binding only
+LIB_PATH = os.environ.get("GSR_LIBRARY") or os.path.join(_PKG, "libgsr.so")
 
 GSR_OK, GSR_EINVAL, GSR_EINDEX, GSR_ENOMEM, GSR_ECUDA, GSR_ESTATE = 0, -1, -2, -3, -4, -5
 TRACE_CAP = 4096
 # gsr_layout.flags (include/gsr.h)
 GSR_FLAG_NO_ATT_COPY, GSR_FLAG_NO_FUSE, GSR_FLAG_NO_TEX = 1, 2, 4
 # gsr_path_info bits
-GSR_PATH_ATT_COPY, GSR_PATH_FUSED, GSR_PATH_INSTR_MATCH, GSR_PATH_TEX, GSR_PATH_IC16 = 1, 2, 4, 8, 16
+GSR_PATH_ATT_COPY, GSR_PATH_FUSED, GSR_PATH_INSTR_MATCH, GSR_PATH_TEX, GSR_PATH_IC16, GSR_PATH_UT = 1, 2, 4, 8, 16, 32
 # gsr_time_aprod selectors (include/gsr_bench.h)
 GSR_TIME_APROD1_GROUP, GSR_TIME_APROD2_GROUP = 1, 2
 GSR_TIME_K_APROD1, GSR_TIME_K_APROD2_MAIN, GSR_TIME_K_APROD2_ATT, GSR_TIME_K_FUSED = 11, 12, 13, 21

@@ -77,10 +77,15 @@ class SynthConfig:
     n_con: int = 0                  # constraint rows
     con_nnz: int = 0                # distinct astro columns per constraint row
     seed: int = 0
+    n_glob: int = 1                 # global columns (1 in the paper's production layout; it also ran 5)
 
     @property
     def n(self) -> int:
-        return 5 * self.n_stars + 3 * self.n_dof_att + self.n_instr + 1
+        return 5 * self.n_stars + 3 * self.n_dof_att + self.n_instr + self.n_glob
+
+    @property
+    def n_par(self) -> int:         # stored coefficients per row: 5 + 12 + 6 + n_glob (24 in production)
+        return 23 + self.n_glob
 
 
 def tiny(seed=0):      # BASELINE.json configs[0]
@@ -161,7 +166,7 @@ def _distinct_draws(seed, stream, base_idx, n_choices, width, cdf=None):
 def generate_rows(cfg: SynthConfig, star0: int, star1: int, device="cpu", rowptr=None) -> dict:
     """Upload arrays for the rows of stars [star0, star1).
 
-    Returns dict(row0, values [r,24] f64, matrixIndexAstro [r] i64, matrixIndexAtt [r] i64,
+    Returns dict(row0, values [r,23+n_glob] f64, matrixIndexAstro [r] i64, matrixIndexAtt [r] i64,
     instrCol [r,6] i32, noise [r] f64).  Rows are sorted by star and by time within a star.
     """
     if rowptr is None:
@@ -189,8 +194,8 @@ def generate_rows(cfg: SynthConfig, star0: int, star1: int, device="cpu", rowptr
     iatt = torch.floor(t * (cfg.n_dof_att - 3)).to(torch.int64).clamp_(0, cfg.n_dof_att - 4)
     cdf = _zipf_cdf(cfg.n_instr, cfg.instr_zipf, device) if cfg.instr_zipf > 0 else None
     ic = _distinct_draws(cfg.seed, S_INSTR, rows, cfg.n_instr, 6, cdf).to(torch.int32)
-    k = torch.arange(N_PAR, dtype=torch.int64, device=device)
-    values = normal(cfg.seed, S_VAL, rows[:, None] * N_PAR + k[None, :])
+    k = torch.arange(cfg.n_par, dtype=torch.int64, device=device)
+    values = normal(cfg.seed, S_VAL, rows[:, None] * cfg.n_par + k[None, :])
     noise = normal(cfg.seed, S_NOISE, rows) * cfg.noise_sigma
     return dict(row0=row0, values=values, matrixIndexAstro=star * 5, matrixIndexAtt=iatt,
                 instrCol=ic, noise=noise)

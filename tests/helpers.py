@@ -14,14 +14,14 @@ def oracle_system(cfg, d=None):
     d = d or np_inputs(cfg)
     con = (d["con_rowptr"], d["con_col"], d["con_val"]) if cfg.n_con else (None, None, None)
     return oracle.OracleSystem(cfg.n_stars, cfg.n_dof_att, cfg.n_instr, d["values"],
-                               d["matrixIndexAstro"], d["matrixIndexAtt"], d["instrCol"], *con), d
+                               d["matrixIndexAstro"], d["matrixIndexAtt"], d["instrCol"], *con, n_glob=cfg.n_glob), d
 
 
 def dense(S):
     """Dense expansion of the oracle's stored system through its column map."""
     A = np.zeros((S.m_tot, S.n))
     for i in range(S.m):
-        for k in range(24):
+        for k in range(S.n_par):
             A[i, S.col(i, k)] += S.V[i, k]
     for r in range(S.n_con):
         for q in range(S.con_rowptr[r], S.con_rowptr[r + 1]):

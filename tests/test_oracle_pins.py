@@ -424,3 +424,36 @@ def test_omp_restatement_matches_the_oracle(threads):
     assert np.linalg.norm(r1.x - r2.x) <= 1e-10 * np.linalg.norm(r1.x)
     assert np.linalg.norm(r1.se - r2.se) <= 1e-9 * np.linalg.norm(r1.se)
     assert abs(r1.rnorm - r2.rnorm) <= 1e-10 * r1.rnorm
+
+
+# ----------------------------------------------------------------------------- N_Glob != 1
+@pytest.mark.parametrize("n_glob", [0, 2, 5])
+def test_global_section_of_any_width(n_glob):
+    """The paper's layout has N_Glob = 1 but it also ran 5 global parameters and allows none
+    (PAPER.md:78): row width 23 + n_glob, global columns at the end of x.  Pins: the structure (every row touches
+    every global column exactly once, in stored order), dense numpy products, adjoint identity, unit columns after
+    preconditioning, and the least-squares solution from numpy."""
+    cfg = dataclasses.replace(synth.mini(seed=11, n_stars=6, obs=14, n_dof_att=7, n_instr=6), n_glob=n_glob)
+    S, d = oracle_system(cfg)
+    assert S.V.shape == (84, 23 + n_glob) and S.n == 30 + 21 + 6 + n_glob
+    for i in (0, 17, 83):
+        assert [S.col(i, 23 + g) for g in range(n_glob)] == [S.n - n_glob + g for g in range(n_glob)]
+        assert S.col(i, 22) == 30 + 21 + d["instrCol"][i, 5]
+    A = dense(S)
+    rng = np.random.default_rng(n_glob)
+    x, y = rng.standard_normal(S.n), rng.standard_normal(S.m_tot)
+    y1, ab = S.aprod1(x, y, want_abs=True)
+    assert np.all(np.abs(y1 - (y + A @ x)) <= 1e-14 * ab)
+    x1, ab = S.aprod2(y, x, want_abs=True)
+    assert np.all(np.abs(x1 - (x + A.T @ y)) <= 1e-14 * ab)
+    assert abs(np.dot(A @ x, y) - np.dot(x, S.aprod2(y, np.zeros(S.n)))) <= 1e-12 * np.linalg.norm(A @ x) * np.linalg.norm(y)
+    b = make_b(S, d)
+    p = S.precondition()
+    np.testing.assert_allclose(np.linalg.norm(dense(S), axis=0), 1.0, rtol=1e-14)
+    np.testing.assert_allclose(p, 1.0 / np.linalg.norm(A, axis=0), rtol=1e-14)
+    r = S.lsqr(b, 500, 1e-15, 1e-15)
+    xls = np.linalg.lstsq(A, b, rcond=None)[0]
+    assert np.linalg.norm(r.x - xls) <= 1e-9 * np.linalg.norm(xls)
+    if n_glob:   # the OpenMP restatement follows
+        R = oracle.OmpRunner(S, 3)
+        assert np.linalg.norm(R.lsqr(b, 500, 1e-15, 1e-15).x - r.x) <= 1e-9 * np.linalg.norm(r.x)
