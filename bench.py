@@ -64,11 +64,17 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel-reps", type=int, default=20)
+    ap.add_argument("--skew-alpha", type=float, default=2.0,
+                    help="exponent of the skewed workload's obs-count law (2.0: literal, ~53 M rows; 1.47: ~150 M rows, DESIGN.md R18)")
+    ap.add_argument("--rerun", type=int, default=0,
+                    help="extra solves of the same system after the timed one; reports run-to-run max|dx| (atomics)")
     return ap.parse_args()
 
 
-def workload_cfg(name):
+def workload_cfg(name, skew_alpha=2.0):
     from paper_2308_00778_b200 import synth
+    if name == "skewed":
+        return synth.skewed(alpha=skew_alpha)
     return {"tiny": synth.tiny, "small": synth.small, "medium": synth.medium, "skewed": synth.skewed,
             "large": synth.large}[name]()
 
@@ -211,7 +217,7 @@ def main_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    cfg = workload_cfg(args.workload)
+    cfg = workload_cfg(args.workload, args.skew_alpha)
     steps = max(1, min(args.steps, 10))
     o = oracle_sample_run(cfg, steps, min(args.warmup, 1))
     blk = cpu_baseline_block(o)
@@ -257,7 +263,7 @@ def main_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    cfg = workload_cfg(args.workload)
+    cfg = workload_cfg(args.workload, args.skew_alpha)
     rp = synth.star_rowptr(cfg)
     m = int(rp[-1])
     G = gsr.Gsr(m, cfg.n_stars, cfg.n_dof_att, cfg.n_instr, cfg.n_con, cfg.n_con * cfg.con_nnz, device=local)
@@ -278,6 +284,15 @@ def main_ours(args):
     xt = synth.x_true(cfg, dev)
     x_err = float(torch.linalg.norm(r.x - xt) / torch.linalg.norm(xt))
     del xt
+    rerun = None
+    if args.rerun > 0:      # att / instr sums use floating-point atomics: how far do repeated solves of one system differ?
+        dmax = 0.0
+        for _ in range(args.rerun):
+            r2 = G.gsr_lsqr(args.steps, 0.0, 0.0)
+            dmax = max(dmax, float((r2.x - r.x).abs().max()))
+            del r2
+        rerun = {"solves": args.rerun + 1, "max_abs_dx": dmax, "max_abs_x": float(r.x.abs().max()),
+                 "what": "largest |x_run_k - x_run_0| over all unknowns after the same number of iterations"}
 
     # ---- per-kernel roofline: every kernel timed alone (CUDA events on the library's stream) against ITS OWN bytes
     peak, peak_src = peaks()
@@ -360,7 +375,9 @@ def main_ours(args):
             "config": {"workload": args.workload, "rows": m, "cols": G.n, "nnz_per_row": 24,
                        "matrix_gb": 232 * m / 1e9, "device_matrix_gb": (rb["k_aprod1"] - 16) * m / 1e9, "path_info": info, "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "inputs larger than L2" if 232 * m > 2.5e8 else "L2-resident (launch-bound config)",
-                       "x_rel_err_vs_planted": x_err, "setup_s": t_gen},
+                       "x_rel_err_vs_planted": x_err, "setup_s": t_gen,
+                       **({"skew_alpha": args.skew_alpha} if args.workload == "skewed" else {}),
+                       **({"run_to_run": rerun} if rerun else {})},
             "clocks": clk.summary(), "gpu_launches": int(r.kernel_launches), "roofline": roofline}
 
     # ---- end to end through the C ABI with HOST buffers: upload + precondition + K iterations + results

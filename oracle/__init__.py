@@ -42,6 +42,7 @@ class _Sys(C.Structure):
         ("n_instr", C.c_int64), ("n_con", C.c_int64), ("n_glob", C.c_int64),
         ("V", C.c_void_p), ("ia", C.c_void_p), ("iatt", C.c_void_p), ("ic", C.c_void_p),
         ("con_rowptr", C.c_void_p), ("con_col", C.c_void_p), ("con_val", C.c_void_p),
+        ("n_astro_par", C.c_int64), ("n_att_par", C.c_int64), ("n_instr_par", C.c_int64),
     ]
 
 
@@ -132,21 +133,29 @@ class LsqrResult:
 class OracleSystem:
     """Holds (private copies of) the upload-format arrays of one system.
 
-    values [m,23+n_glob] f64 row-major; matrixIndexAstro [m] i64 (= 5*star, non-decreasing);
-    matrixIndexAtt [m] i64 (axis-0 start); instrCol [m,6] i32; optional constraint rows
-    as CSR with absolute columns.  n_glob = 1 is the paper's production layout (24 per row).
+    values [m, n_par] f64 row-major with n_par = n_astro_par + n_att_par + n_instr_par + n_glob;
+    matrixIndexAstro [m] i64 (= n_astro_par*star, non-decreasing); matrixIndexAtt [m] i64 (axis-0 start);
+    instrCol [m, n_instr_par] i32; optional constraint rows as CSR with absolute columns.
+    5 / 12 / 6 / 1 is the paper's production layout (24 per row); a section of width 0 has no
+    columns and its index array is ignored (may be None).
     """
 
     def __init__(self, n_stars, n_dof_att, n_instr, values, matrixIndexAstro, matrixIndexAtt,
-                 instrCol, con_rowptr=None, con_col=None, con_val=None, n_glob=1):
+                 instrCol, con_rowptr=None, con_col=None, con_val=None, n_glob=1,
+                 n_astro_par=5, n_att_par=12, n_instr_par=6):
         self.lib = _load()
         self.n_glob = int(n_glob)
-        self.n_par = 23 + self.n_glob
+        self.n_astro_par, self.n_att_par, self.n_instr_par = int(n_astro_par), int(n_att_par), int(n_instr_par)
+        assert 0 <= self.n_astro_par <= 5 and self.n_att_par in (0, 12) and 0 <= self.n_instr_par <= 6 and self.n_glob >= 0
+        self.n_par = self.n_astro_par + self.n_att_par + self.n_instr_par + self.n_glob
+        assert self.n_par > 0
         self.V = np.array(values, dtype=np.float64, order="C", copy=True).reshape(-1, self.n_par)
         self.m = self.V.shape[0]
-        self.ia = np.array(matrixIndexAstro, dtype=np.int64, copy=True).reshape(-1)
-        self.iatt = np.array(matrixIndexAtt, dtype=np.int64, copy=True).reshape(-1)
-        self.ic = np.array(instrCol, dtype=np.int32, order="C", copy=True).reshape(-1, 6)
+        zeros = np.zeros(self.m, dtype=np.int64)
+        self.ia = np.array(matrixIndexAstro if self.n_astro_par else zeros, dtype=np.int64, copy=True).reshape(-1)
+        self.iatt = np.array(matrixIndexAtt if self.n_att_par else zeros, dtype=np.int64, copy=True).reshape(-1)
+        self.ic = (np.array(instrCol, dtype=np.int32, order="C", copy=True).reshape(-1, self.n_instr_par)
+                   if self.n_instr_par else np.zeros((self.m, 0), dtype=np.int32))
         assert self.ia.shape[0] == self.m and self.iatt.shape[0] == self.m and self.ic.shape[0] == self.m
         self.n_stars, self.n_dof_att, self.n_instr = int(n_stars), int(n_dof_att), int(n_instr)
         if con_rowptr is not None:
@@ -162,7 +171,8 @@ class OracleSystem:
         self.p = None
         self._s = _Sys(self.m, self.n_stars, self.n_dof_att, self.n_instr, self.n_con, self.n_glob,
                        _ptr(self.V), _ptr(self.ia), _ptr(self.iatt), _ptr(self.ic),
-                       _ptr(self.con_rowptr), _ptr(self.con_col), _ptr(self.con_val))
+                       _ptr(self.con_rowptr), _ptr(self.con_col), _ptr(self.con_val),
+                       self.n_astro_par, self.n_att_par, self.n_instr_par)
         self._sp = C.addressof(self._s)
         self.n = int(self.lib.gsr_oracle_ncols(self._sp))
         self.m_tot = self.m + self.n_con
@@ -217,6 +227,7 @@ class OmpRunner:
     threading.  For bench.py's all-core cpu_baseline; checked against the oracle in the tests."""
 
     def __init__(self, S: OracleSystem, threads: int = 0):
+        assert (S.n_astro_par, S.n_att_par, S.n_instr_par) == (5, 12, 6), "the threaded restatement covers the 5/12/6/n_glob layout"
         self.S = S
         self.lib = _load_omp()
         self.lib.gsr_omp_set_threads(int(threads) if threads > 0 else (os.cpu_count() or 1))

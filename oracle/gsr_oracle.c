@@ -27,14 +27,18 @@
  *
  * Matrix definition (PAPER.md:78-80 and the index expressions
  * of Algorithm 2).  Row i of A holds
- * N_par = 23 + nGlob stored coefficients V[i*N_par + k] in the section order
- *   [ 5 astrometric | 12 attitude = 3 axes x 4 | 6 instrumental | nGlob global ]
- * (nGlob = 1, N_par = 24 in the paper's production layout; the paper
- * also ran 5 global parameters, and allows 0) and coefficient k sits in column
- *   k <  5 : ia[i] + k                                   (ia[i] = 5*star(i))
- *   k < 17 : 5*nStars + a*nDofAtt + iatt[i] + j          a=(k-5)/4, j=(k-5)%4
- *   k < 23 : 5*nStars + 3*nDofAtt + ic[i*6 + (k-17)]
- *   k >= 23: 5*nStars + 3*nDofAtt + nInstr + (k-23)      (Alg. 2 "glob": x[j + offset])
+ * N_par = nAstro + nAtt + nInstrPar + nGlob stored coefficients V[i*N_par + k] in the section order
+ *   [ nAstro astrometric | nAtt attitude = 3 axes x 4 | nInstrPar instrumental | nGlob global ]
+ * with 0 <= nAstro <= 5, nAtt = 12 or 0, 0 <= nInstrPar <= 6, nGlob >= 0 ("0 <= N_Astro <= 5",
+ * "N_Att = 12", "0 <= N_Instr <= 6", N_Glob = 1 "or ... without computing a global part"; the paper also ran
+ * 5 global parameters, and its 40 / 100 / 300 GB datasets solve only some of the sections,
+ * PAPER.md:263).  The production layout is 5 / 12 / 6 / 1, N_par = 24.  A section of width 0 has no
+ * columns.  With kA = nAstro, kT = kA + nAtt, kI = kT + nInstrPar, coefficient k sits in column
+ *   k < kA : ia[i] + k                                   (ia[i] = nAstro*star(i))
+ *   k < kT : offAtt + a*nDofAtt + iatt[i] + j            a=(k-kA)/4, j=(k-kA)%4;  offAtt = nAstro*nStars
+ *   k < kI : offInstr + ic[i*nInstrPar + (k-kT)]         offInstr = offAtt + (nAtt ? 3*nDofAtt : 0)
+ *   else   : offGlob + (k-kI)                            offGlob = offInstr + (nInstrPar ? nInstr : 0)
+ *                                                        (Alg. 2 "glob": x[j + offset])
  * Constraint rows are generic sparse rows appended below
  * the observation rows, given as CSR (rowptr, col, val) with absolute columns.
  */
@@ -43,12 +47,8 @@
 #include <stdlib.h>
 #include <string.h>
 
-#define N_ASTRO 5
 #define N_AXES 3
 #define N_PAR_AXIS 4
-#define N_ATT (N_AXES * N_PAR_AXIS)
-#define N_INSTR 6
-#define N_FIXED (N_ASTRO + N_ATT + N_INSTR) /* 23; N_par = 23 + n_glob = 24 for n_glob = 1 */
 
 typedef struct {
     int64_t n_obs;      /* observation rows m                                  */
@@ -58,36 +58,42 @@ typedef struct {
     int64_t n_con;      /* constraint rows                                     */
     int64_t n_glob;     /* N_Glob global columns (1 in production)*/
     double *V;          /* [n_obs*N_par] row-major A_d           */
-    const int64_t *ia;  /* [n_obs]   M_i astro part: 5*star, non-decreasing    */
+    const int64_t *ia;  /* [n_obs]   M_i astro part: N_Astro*star, non-decreasing */
     const int64_t *iatt;/* [n_obs]   M_i attitude part: start s_i, axis 0      */
-    const int32_t *ic;  /* [n_obs*6] I_c instrumental columns                  */
+    const int32_t *ic;  /* [n_obs*N_Instr] I_c instrumental columns            */
     const int64_t *con_rowptr; /* [n_con+1]                                    */
     const int64_t *con_col;    /* [nnz] absolute columns                       */
     double *con_val;           /* [nnz]                                        */
+    int64_t n_astro_par; /* N_Astro, 0..5 coefficients (and unknowns) per star */
+    int64_t n_att_par;   /* N_Att, 12 (3 axes x 4) or 0                        */
+    int64_t n_instr_par; /* N_Instr, 0..6 coefficients per row                 */
 } gsr_oracle_system;
 
-int64_t gsr_oracle_ncols(const gsr_oracle_system *S)
-{
-    return N_ASTRO * S->n_stars + N_AXES * S->n_dof_att + S->n_instr + S->n_glob;
-}
+/* first column of the attitude, instrumental and global sections (a section of width 0 has no columns) */
+static int64_t off_att(const gsr_oracle_system *S) { return S->n_astro_par * S->n_stars; }
+static int64_t off_instr(const gsr_oracle_system *S) { return off_att(S) + (S->n_att_par ? N_AXES * S->n_dof_att : 0); }
+static int64_t off_glob(const gsr_oracle_system *S) { return off_instr(S) + (S->n_instr_par ? S->n_instr : 0); }
 
-static int npar(const gsr_oracle_system *S) { return N_FIXED + (int)S->n_glob; }
+int64_t gsr_oracle_ncols(const gsr_oracle_system *S) { return off_glob(S) + S->n_glob; }
+
+static int npar(const gsr_oracle_system *S)
+{
+    return (int)(S->n_astro_par + S->n_att_par + S->n_instr_par + S->n_glob);
+}
 
 /* Column of stored coefficient k of observation row i (see header). */
 int64_t gsr_oracle_col(const gsr_oracle_system *S, int64_t i, int k)
 {
-    const int64_t off_att = N_ASTRO * S->n_stars;
-    const int64_t off_instr = off_att + N_AXES * S->n_dof_att;
-    const int64_t off_glob = off_instr + S->n_instr;
-    if (k < N_ASTRO)
+    const int kA = (int)S->n_astro_par, kT = kA + (int)S->n_att_par, kI = kT + (int)S->n_instr_par;
+    if (k < kA)
         return S->ia[i] + k;
-    if (k < N_ASTRO + N_ATT) {
-        int a = (k - N_ASTRO) / N_PAR_AXIS, j = (k - N_ASTRO) % N_PAR_AXIS;
-        return off_att + (int64_t)a * S->n_dof_att + S->iatt[i] + j;
+    if (k < kT) {
+        int a = (k - kA) / N_PAR_AXIS, j = (k - kA) % N_PAR_AXIS;
+        return off_att(S) + (int64_t)a * S->n_dof_att + S->iatt[i] + j;
     }
-    if (k < N_ASTRO + N_ATT + N_INSTR)
-        return off_instr + S->ic[i * N_INSTR + (k - N_ASTRO - N_ATT)];
-    return off_glob + (k - N_FIXED);
+    if (k < kI)
+        return off_instr(S) + S->ic[i * S->n_instr_par + (k - kT)];
+    return off_glob(S) + (k - kI);
 }
 
 /*

@@ -22,7 +22,8 @@
 
 enum { NA = 5, NAX = 3, NPA = 4, NATT = 12, NI = 6, NF = 23 };   /* row width 23 + n_glob */
 
-/* same field order as gsr_oracle_system (oracle/__init__.py passes one ctypes struct to both) */
+/* same leading fields as gsr_oracle_system (oracle/__init__.py passes one ctypes struct to both; the section
+ * widths that follow there are 5 / 12 / 6 here, checked by the Python side) */
 typedef struct {
     int64_t n_obs, n_stars, n_dof_att, n_instr, n_con, n_glob;
     double *V;

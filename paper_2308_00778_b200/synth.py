@@ -78,14 +78,20 @@ class SynthConfig:
     con_nnz: int = 0                # distinct astro columns per constraint row
     seed: int = 0
     n_glob: int = 1                 # global columns (1 in the paper's production layout; it also ran 5)
+    # section widths (0 <= N_Astro <= 5, N_Att = 12 or no attitude part, 0 <= N_Instr <= 6);
+    # a section of width 0 has no columns (the paper's 40 / 100 / 300 GB datasets solve only some sections)
+    n_astro_par: int = 5
+    n_att_par: int = 12
+    n_instr_par: int = 6
 
     @property
     def n(self) -> int:
-        return 5 * self.n_stars + 3 * self.n_dof_att + self.n_instr + self.n_glob
+        return (self.n_astro_par * self.n_stars + (3 * self.n_dof_att if self.n_att_par else 0)
+                + (self.n_instr if self.n_instr_par else 0) + self.n_glob)
 
     @property
-    def n_par(self) -> int:         # stored coefficients per row: 5 + 12 + 6 + n_glob (24 in production)
-        return 23 + self.n_glob
+    def n_par(self) -> int:         # stored coefficients per row (24 in production)
+        return self.n_astro_par + self.n_att_par + self.n_instr_par + self.n_glob
 
 
 def tiny(seed=0):      # BASELINE.json configs[0]
@@ -166,8 +172,8 @@ def _distinct_draws(seed, stream, base_idx, n_choices, width, cdf=None):
 def generate_rows(cfg: SynthConfig, star0: int, star1: int, device="cpu", rowptr=None) -> dict:
     """Upload arrays for the rows of stars [star0, star1).
 
-    Returns dict(row0, values [r,23+n_glob] f64, matrixIndexAstro [r] i64, matrixIndexAtt [r] i64,
-    instrCol [r,6] i32, noise [r] f64).  Rows are sorted by star and by time within a star.
+    Returns dict(row0, values [r,n_par] f64, matrixIndexAstro [r] i64 (= n_astro_par*star), matrixIndexAtt [r] i64,
+    instrCol [r,n_instr_par] i32, noise [r] f64).  Rows are sorted by star and by time within a star.
     """
     if rowptr is None:
         rowptr = star_rowptr(cfg, device)
@@ -193,11 +199,14 @@ def generate_rows(cfg: SynthConfig, star0: int, star1: int, device="cpu", rowptr
         t = t.clamp_(0.0, 1.0 - 2.0 ** -53)
     iatt = torch.floor(t * (cfg.n_dof_att - 3)).to(torch.int64).clamp_(0, cfg.n_dof_att - 4)
     cdf = _zipf_cdf(cfg.n_instr, cfg.instr_zipf, device) if cfg.instr_zipf > 0 else None
-    ic = _distinct_draws(cfg.seed, S_INSTR, rows, cfg.n_instr, 6, cdf).to(torch.int32)
+    if cfg.n_instr_par > 0:
+        ic = _distinct_draws(cfg.seed, S_INSTR, rows, cfg.n_instr, cfg.n_instr_par, cdf).to(torch.int32)
+    else:
+        ic = torch.zeros((r, 0), dtype=torch.int32, device=device)
     k = torch.arange(cfg.n_par, dtype=torch.int64, device=device)
     values = normal(cfg.seed, S_VAL, rows[:, None] * cfg.n_par + k[None, :])
     noise = normal(cfg.seed, S_NOISE, rows) * cfg.noise_sigma
-    return dict(row0=row0, values=values, matrixIndexAstro=star * 5, matrixIndexAtt=iatt,
+    return dict(row0=row0, values=values, matrixIndexAstro=star * cfg.n_astro_par, matrixIndexAtt=iatt,
                 instrCol=ic, noise=noise)
 
 
@@ -212,7 +221,7 @@ def constraints(cfg: SynthConfig, device="cpu"):
                 torch.zeros(0, dtype=torch.int64, device=device),
                 torch.zeros(0, dtype=torch.float64, device=device))
     rows = torch.arange(cfg.n_con, dtype=torch.int64, device=device)
-    col = _distinct_draws(cfg.seed, S_CONCOL, rows, 5 * cfg.n_stars, cfg.con_nnz)
+    col = _distinct_draws(cfg.seed, S_CONCOL, rows, max(cfg.n_astro_par, 1) * cfg.n_stars, cfg.con_nnz)
     col = torch.sort(col, dim=1).values.reshape(-1)
     val = normal(cfg.seed, S_CONVAL, torch.arange(cfg.n_con * cfg.con_nnz, dtype=torch.int64, device=device))
     rowptr = torch.arange(cfg.n_con + 1, dtype=torch.int64, device=device) * cfg.con_nnz

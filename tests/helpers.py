@@ -14,7 +14,8 @@ def oracle_system(cfg, d=None):
     d = d or np_inputs(cfg)
     con = (d["con_rowptr"], d["con_col"], d["con_val"]) if cfg.n_con else (None, None, None)
     return oracle.OracleSystem(cfg.n_stars, cfg.n_dof_att, cfg.n_instr, d["values"],
-                               d["matrixIndexAstro"], d["matrixIndexAtt"], d["instrCol"], *con, n_glob=cfg.n_glob), d
+                               d["matrixIndexAstro"], d["matrixIndexAtt"], d["instrCol"], *con, n_glob=cfg.n_glob,
+                               n_astro_par=cfg.n_astro_par, n_att_par=cfg.n_att_par, n_instr_par=cfg.n_instr_par), d
 
 
 def dense(S):

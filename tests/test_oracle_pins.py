@@ -457,3 +457,95 @@ def test_global_section_of_any_width(n_glob):
     if n_glob:   # the OpenMP restatement follows
         R = oracle.OmpRunner(S, 3)
         assert np.linalg.norm(R.lsqr(b, 500, 1e-15, 1e-15).x - r.x) <= 1e-9 * np.linalg.norm(r.x)
+
+
+# ----------------------------------------------------------------------------- section widths other than 5/12/6/1 (NEXT-4)
+def test_hand_worked_variant_fixture():
+    """General column map (PAPER.md:78 widths; Alg. 2 index expressions) on a hand-worked 2/12/3/2 system
+    (tests/golden/hand_variant.txt): columns, aprod1 and aprod2 values derived by hand."""
+    rows, kv = [], {}
+    for line in open(os.path.join(GOLD, "hand_variant.txt")):
+        line = line.split("#")[0].strip()
+        if not line:
+            continue
+        tok = line.split()
+        if tok[0] == "row":
+            a, b_, c = line[3:].split("|")
+            ia, iatt = map(int, a.split())
+            rows.append((ia, iatt, list(map(int, b_.split())), c.strip()))
+        else:
+            kv[tok[0]] = [float(t) for t in tok[1:]]
+    w = {k: int(kv[k][0]) for k in ("n_astro_par", "n_att_par", "n_instr_par", "n_glob", "n_stars", "n_dof_att", "n_instr")}
+    npar = w["n_astro_par"] + w["n_att_par"] + w["n_instr_par"] + w["n_glob"]
+    assert npar == 19
+    rule = {"ones": lambda k: 1.0, "kplus1": lambda k: k + 1.0}
+    V = np.array([[rule[r[3]](k) for k in range(npar)] for r in rows])
+    S = oracle.OracleSystem(w["n_stars"], w["n_dof_att"], w["n_instr"], V, [r[0] for r in rows], [r[1] for r in rows],
+                            [r[2] for r in rows], n_glob=w["n_glob"], n_astro_par=w["n_astro_par"],
+                            n_att_par=w["n_att_par"], n_instr_par=w["n_instr_par"])
+    assert S.n == 25
+    assert [S.col(1, k) for k in range(npar)] == [int(c) for c in kv["cols1"]]
+    y, ab = S.aprod1(np.arange(1, 26, dtype=np.float64), np.array(kv["aprod1_yin"]), want_abs=True)
+    assert y.tolist() == kv["aprod1_yout"]
+    assert ab.tolist() == [100 + 253, 200 + 3407]      # all terms positive
+    assert S.aprod2(np.array(kv["aprod2_y"]), np.zeros(25)).tolist() == kv["aprod2_xout"]
+
+
+VARIANTS = [   # (n_astro_par, n_att_par, n_instr_par, n_glob): PAPER.md:78 ranges and the section subsets of PAPER.md:263
+    (0, 12, 6, 0),    # attitude + instrumental only (the paper's 40 and 300 GB datasets)
+    (5, 0, 0, 0),     # astrometric only (the 100 GB dataset)
+    (5, 12, 6, 0),    # astrometric + attitude + instrumental, no global part (the 350 GB dataset)
+    (3, 12, 4, 2),    # fewer astrometric / instrumental coefficients, two global parameters
+    (2, 0, 1, 5),     # no attitude part, five global parameters (PAPER.md:206)
+]
+
+
+@pytest.mark.parametrize("widths", VARIANTS)
+def test_section_width_variants(widths):
+    """Every layout the paper allows reduces to the same definition with other widths.  Pins: structure of each row
+    (block-diagonal astro part of N_Astro columns, 3 x 4 attitude columns N_DFA apart, instrument columns inside their
+    range, every global column once), dense numpy products with their |terms| bounds, adjoint identity, unit columns
+    after preconditioning, numpy's least-squares solution."""
+    na, nt, ni, ng = widths
+    cfg = dataclasses.replace(synth.mini(seed=5, n_stars=7, obs=16, n_dof_att=9, n_instr=7), n_glob=ng, n_astro_par=na,
+                              n_att_par=nt, n_instr_par=ni)
+    S, d = oracle_system(cfg)
+    m, ns, nd = S.m, cfg.n_stars, cfg.n_dof_att
+    off_att = na * ns
+    off_instr = off_att + (3 * nd if nt else 0)
+    off_glob = off_instr + (cfg.n_instr if ni else 0)
+    assert S.n == off_glob + ng == cfg.n and S.V.shape == (m, na + nt + ni + ng)
+    A = dense(S)
+    assert ((A[:m] != 0).sum(axis=1) == na + nt + ni + ng).all()
+    star = np.repeat(np.arange(ns), 16)
+    for i in range(m):
+        nz = np.nonzero(A[i])[0]
+        assert nz[:na].tolist() == list(range(na * star[i], na * star[i] + na))
+        if nt:
+            att = nz[na:na + 12].reshape(3, 4)
+            assert (np.diff(att, axis=1) == 1).all() and (np.diff(att[:, 0]) == nd).all()
+            assert off_att <= att[0, 0] and att[0, 3] < off_att + nd
+            assert att[0, 0] - off_att == d["matrixIndexAtt"][i]
+        if ni:
+            ins = nz[na + nt:na + nt + ni]
+            assert sorted(ins - off_instr) == sorted(d["instrCol"][i].tolist())
+        assert nz[na + nt + ni:].tolist() == list(range(off_glob, off_glob + ng))
+        # stored order: coefficient k of the row sits in the k-th column of the map, with the stored value
+        for k in range(S.n_par):
+            assert A[i, S.col(i, k)] == S.V[i, k]
+    rng = np.random.default_rng(sum(widths))
+    x, y = rng.standard_normal(S.n), rng.standard_normal(S.m_tot)
+    y1, ab = S.aprod1(x, y, want_abs=True)
+    np.testing.assert_allclose(ab, np.abs(y) + np.abs(A) @ np.abs(x), rtol=1e-13)
+    assert np.all(np.abs(y1 - (y + A @ x)) <= 1e-14 * ab)
+    x1, ab = S.aprod2(y, x, want_abs=True)
+    np.testing.assert_allclose(ab, np.abs(x) + np.abs(A).T @ np.abs(y), rtol=1e-13)
+    assert np.all(np.abs(x1 - (x + A.T @ y)) <= 1e-14 * ab)
+    assert abs(np.dot(A @ x, y) - np.dot(x, S.aprod2(y, np.zeros(S.n)))) <= 1e-12 * np.linalg.norm(A @ x) * np.linalg.norm(y)
+    b = make_b(S, d)
+    p = S.precondition()
+    np.testing.assert_allclose(np.linalg.norm(dense(S), axis=0), 1.0, rtol=1e-14)
+    np.testing.assert_allclose(p, 1.0 / np.linalg.norm(A, axis=0), rtol=1e-14)
+    r = S.lsqr(b, 800, 1e-15, 1e-15)
+    xls = np.linalg.lstsq(A, b, rcond=None)[0]
+    assert np.linalg.norm(r.x - xls) <= 1e-9 * np.linalg.norm(xls)
