@@ -16,6 +16,21 @@
  *     k = 23 : 5*n_stars + 3*n_dof_att + n_instr
  * (index expressions of Algorithm 2).
  *
+ * Model variants ("0 <= N_Astro <= 5", "0 <= N_Instr <= 6", N_Glob = 1 "or ... without
+ * computing a global part"; runs with 5 global parameters; datasets that
+ * solve only some of the sections).  gsr_layout carries the four section widths
+ *     n_astro_par 0..5 | n_att_par 12 or 0 | n_instr_par 0..6 | n_glob_par 0..GSR_MAX_GLOB
+ * and a row then stores N_par = their sum coefficients in the same section order.  A section of
+ * width 0 has no columns: with kA = n_astro_par, kT = kA + n_att_par, kI = kT + n_instr_par,
+ *     offAtt = n_astro_par*n_stars, offInstr = offAtt + (n_att_par ? 3*n_dof_att : 0),
+ *     offGlob = offInstr + (n_instr_par ? n_instr : 0), n = offGlob + n_glob_par,
+ *     k < kA : matrixIndexAstro[i] + k          (matrixIndexAstro[i] = n_astro_par*star(i))
+ *     k < kT : offAtt + a*n_dof_att + matrixIndexAtt[i] + j,  a=(k-kA)/4, j=(k-kA)%4
+ *     k < kI : offInstr + instrCol[n_instr_par*i + (k-kT)]
+ *     else   : offGlob + (k-kI)                 (Alg. 2 "glob")
+ * The production layout 5/12/6/1 runs the specialised kernels (fused iteration, attitude copy);
+ * every other layout runs one general pair of aprod kernels and the two-product iteration.
+ *
  * Conventions
  *  - every call returns a gsr_status (0 = OK, negative = error); nothing throws;
  *    gsr_last_error(h) gives a handle-owned, NUL-terminated description.
@@ -40,6 +55,7 @@ extern "C" {
 #define GSR_N_INSTR 6
 #define GSR_N_GLOB 1
 #define GSR_N_PAR 24
+#define GSR_MAX_GLOB 16 /* widest global section a layout may ask for */
 
 typedef enum {
     GSR_OK = 0,
@@ -50,17 +66,19 @@ typedef enum {
     GSR_ESTATE = -5  /* call order: e.g. aprod before upload, precondition twice       */
 } gsr_status;
 
-/* Sizes of one system.  Section widths are fixed at 5/12/6/1
- * (BASELINE north_star); the fields exist so that a mismatch is an error rather
- * than a silent misread. */
+/* Sizes of one system.  Section widths: 5/12/6/1 is the production
+ * layout (BASELINE north_star); see "Model variants" above for the others.  Widths outside
+ * their ranges are GSR_EINVAL. */
 typedef struct {
     int64_t n_obs;      /* observation rows m (>= 0)                                   */
-    int64_t n_stars;    /* N_Stars                                                     */
-    int64_t n_dof_att;  /* N_DFA, attitude degrees of freedom per axis (>= 4)          */
-    int64_t n_instr;    /* number of instrumental columns (>= 6)                       */
+    int64_t n_stars;    /* N_Stars (>= 1 when n_astro_par > 0)                         */
+    int64_t n_dof_att;  /* N_DFA, attitude degrees of freedom per axis (>= 4 when
+                           n_att_par > 0)                                              */
+    int64_t n_instr;    /* number of instrumental columns (>= n_instr_par)             */
     int64_t n_con;      /* constraint rows appended below the observations (>= 0)      */
     int64_t n_con_nnz;  /* non-zeros of the constraint rows                            */
-    int32_t n_astro_par, n_att_par, n_instr_par, n_glob_par; /* must be 5, 12, 6, 1    */
+    int32_t n_astro_par, n_att_par, n_instr_par, n_glob_par; /* 5, 12, 6, 1 in production;
+                           0..5, 12 or 0, 0..6, 0..GSR_MAX_GLOB in general             */
     int32_t device;     /* CUDA device ordinal                                         */
     uint32_t flags;     /* bitwise OR of GSR_FLAG_* (0 = default path)                 */
     void *stream;       /* cudaStream_t of the CALLER (e.g. torch's current stream), or
@@ -109,16 +127,18 @@ const char *gsr_last_error(const gsr_handle *h);
 /* After GSR_EINDEX: first offending observation row (or -1). */
 int64_t gsr_bad_row(const gsr_handle *h);
 
-/* n = 5*n_stars + 3*n_dof_att + n_instr + 1 and m_tot = n_obs + n_con. */
+/* n (5*n_stars + 3*n_dof_att + n_instr + 1 in production; see "Model variants") and
+ * m_tot = n_obs + n_con. */
 int64_t gsr_ncols(const gsr_handle *h);
 int64_t gsr_nrows(const gsr_handle *h);
 
 /* Copies the system to the device (A_d, M_i, I_c; Alg. 1 l.6-12).
- *   values           f64 [n_obs*24] row-major, section order as above
- *   matrixIndexAstro i64 [n_obs]   = 5*star(i), non-decreasing, in [0, 5*(n_stars-1)]
+ *   values           f64 [n_obs*N_par] row-major, section order as above (N_par = 24)
+ *   matrixIndexAstro i64 [n_obs]   = n_astro_par*star(i), non-decreasing (5*star(i) in production)
  *   matrixIndexAtt   i64 [n_obs]   = s_i in [0, n_dof_att-4] (axis-0 relative)
- *   instrCol         i32 [n_obs*6] in [0, n_instr)
+ *   instrCol         i32 [n_obs*n_instr_par] in [0, n_instr)
  *   b                f64 [n_obs+n_con] known terms
+ * The index array of a section of width 0 is ignored and may be NULL.
  * All host or device.  Validates the index contracts on the device (GSR_EINDEX,
  * gsr_bad_row) and derives the star row pointer.  Replaces any earlier upload,
  * clears the preconditioned state and DISCARDS the constraint rows (gsr_precondition
@@ -149,7 +169,7 @@ int32_t gsr_upload_constraints(gsr_handle *h, const int64_t *rowptr, const int64
                                const double *val);
 
 /* Derived layout, for bit-exact checks: i64 [n_stars+1], first row of each star.
- * out: host or device. */
+ * out: host or device.  GSR_ESTATE when the layout has no astrometric section. */
 int32_t gsr_get_star_rowptr(gsr_handle *h, int64_t *out);
 
 /* Column preconditioning (Alg. 1 l.2-3): p_j = 1/||A_:j||_2 over all
@@ -161,7 +181,7 @@ int32_t gsr_precondition(gsr_handle *h);
 int32_t gsr_get_colscale(gsr_handle *h, double *out);
 
 /* Device copy of the matrix values as they stand (scaled if preconditioned):
- * out f64 [n_obs*24], host or device; con_val_out f64 [n_con_nnz] or NULL. */
+ * out f64 [n_obs*N_par], host or device; con_val_out f64 [n_con_nnz] or NULL. */
 int32_t gsr_get_values(gsr_handle *h, double *out, double *con_val_out);
 
 /* aprod mode 1, Eq. 2, Algorithm 2:  y += A x  on the matrix as it

@@ -21,6 +21,8 @@ using namespace gsr;
 struct gsr_handle {
     gsr_layout L{};
     int64_t n = 0, mTot = 0, nTiles = 0;
+    int nA = N_ASTRO, nAtt = N_ATT, nI = N_INSTR, nG = 1, nPar = N_PAR;   // section widths
+    bool prod = true;   // 5/12/6/1: the specialised kernels; any other layout runs k_aprod1_gen / k_aprod2_gen
     cudaStream_t stream = nullptr;
     cudaStream_t userStream = nullptr;
     int smCount = 148;
@@ -104,9 +106,10 @@ MatView view(const gsr_handle *h)
     MatView A;
     A.V = h->V; A.star = h->star; A.iatt = h->iatt; A.ic = h->ic; A.ic16 = h->ic16; A.rp = h->rp; A.tw = h->tw;
     A.m = h->L.n_obs; A.nStars = h->L.n_stars; A.nDof = h->L.n_dof_att; A.nInstr = h->L.n_instr;
-    A.offAtt = 5 * h->L.n_stars;
-    A.offInstr = A.offAtt + 3 * h->L.n_dof_att;
-    A.offGlob = A.offInstr + h->L.n_instr;
+    A.nA = h->nA; A.nAtt = h->nAtt; A.nI = h->nI; A.nG = h->nG; A.nPar = h->nPar;
+    A.offAtt = int64_t(h->nA) * h->L.n_stars;                       // a section of width 0 has no columns
+    A.offInstr = A.offAtt + (h->nAtt ? 3 * h->L.n_dof_att : 0);
+    A.offGlob = A.offInstr + (h->nI ? h->L.n_instr : 0);
     A.n = h->n;
     A.conRp = h->conRp; A.conCol = h->conCol; A.conVal = h->conVal; A.nCon = h->L.n_con;
     A.attT = h->useAttT ? h->attT : nullptr; A.sT = h->sT; A.permT = h->permT;
@@ -198,16 +201,20 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     if (!h) return GSR_ENOMEM;
     *out = h;   // returned even on failure so that gsr_last_error works; caller destroys it
     h->L = *L;
-    if (L->n_astro_par != GSR_N_ASTRO || L->n_att_par != GSR_N_ATT || L->n_instr_par != GSR_N_INSTR ||
-        L->n_glob_par != GSR_N_GLOB)
-        return fail(h, GSR_EINVAL, "section widths must be 5/12/6/1 (got %d/%d/%d/%d)", L->n_astro_par,
-                    L->n_att_par, L->n_instr_par, L->n_glob_par);
-    if (L->n_obs < 0 || L->n_stars < 1 || L->n_dof_att < 4 || L->n_instr < 6 || L->n_con < 0 ||
-        L->n_con_nnz < 0 || (L->n_con == 0 && L->n_con_nnz != 0))
+    if (L->n_astro_par < 0 || L->n_astro_par > GSR_N_ASTRO || (L->n_att_par != GSR_N_ATT && L->n_att_par != 0) ||
+        L->n_instr_par < 0 || L->n_instr_par > GSR_N_INSTR || L->n_glob_par < 0 || L->n_glob_par > GSR_MAX_GLOB ||
+        L->n_astro_par + L->n_att_par + L->n_instr_par + L->n_glob_par < 1)
+        return fail(h, GSR_EINVAL, "section widths must be 0..5 / 12 or 0 / 0..6 / 0..%d with at least one coefficient per row "
+                    "(got %d/%d/%d/%d)", GSR_MAX_GLOB, L->n_astro_par, L->n_att_par, L->n_instr_par, L->n_glob_par);
+    h->nA = L->n_astro_par; h->nAtt = L->n_att_par; h->nI = L->n_instr_par; h->nG = L->n_glob_par;
+    h->nPar = h->nA + h->nAtt + h->nI + h->nG;
+    h->prod = h->nA == GSR_N_ASTRO && h->nAtt == GSR_N_ATT && h->nI == GSR_N_INSTR && h->nG == GSR_N_GLOB;
+    if (L->n_obs < 0 || L->n_stars < 0 || (h->nA > 0 && L->n_stars < 1) || (h->nAtt > 0 && L->n_dof_att < 4) ||
+        L->n_dof_att < 0 || L->n_instr < h->nI || L->n_con < 0 || L->n_con_nnz < 0 || (L->n_con == 0 && L->n_con_nnz != 0))
         return fail(h, GSR_EINVAL, "bad sizes");
     if (L->n_stars >= (int64_t(1) << TW_STAR_BITS) || L->n_dof_att >= (int64_t(1) << 31) || L->n_instr >= (int64_t(1) << 31))
         return fail(h, GSR_EINVAL, "n_stars must be below 2^29, n_dof_att and n_instr below 2^31 (packed row indices)");
-    h->n = 5 * L->n_stars + 3 * L->n_dof_att + L->n_instr + 1;
+    h->n = int64_t(h->nA) * L->n_stars + (h->nAtt ? 3 * L->n_dof_att : 0) + (h->nI ? L->n_instr : 0) + h->nG;
     h->mTot = L->n_obs + L->n_con;
     h->nTiles = (L->n_obs + TILE - 1) / TILE;
     h->userStream = static_cast<cudaStream_t>(L->stream);
@@ -223,8 +230,13 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(cudaEventCreateWithFlags(&h->evSlot[1], cudaEventDisableTiming));
 
     int occ1 = 1, occ2 = 1;
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, k_aprod1<true>, THREADS, 0));
-    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, k_aprod2<true, false, true>, THREADS, 0));
+    if (h->prod) {
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, k_aprod1<true>, THREADS, 0));
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, k_aprod2<true, false, true>, THREADS, 0));
+    } else {
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ1, k_aprod1_gen, THREADS, 0));
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ2, k_aprod2_gen<false>, THREADS, 0));
+    }
     h->gridA1 = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ1, 1));
     h->gridA2 = gridFor(h->nTiles, WARPS, h->smCount * std::max(occ2, 1));
     {   // main kernel without attitude: one CTA per SM with a private shared-memory table for the first
@@ -251,25 +263,26 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     h->gridCon = gridFor(L->n_con, 8, h->smCount * 8);
     // fix-up grid: one thread per star, then one per instrument column (replica fold), then gamma
     h->gridFix = int((L->n_stars + 255) / 256) + int((L->n_instr + 255) / 256) + 1;
+    if (!h->prod) h->gridFix = (h->nA > 0 ? int((L->n_stars + 255) / 256) : 0) + 1;   // k_fixup_gen: stars, then the global columns
     h->gridAtt = gridFor(h->nTiles, 8, h->smCount * 4);
     h->gridUT = gridFor(L->n_obs, 256, h->smCount * 4);
     // instrument replicas: spread the REDs of aprod2 over >= ~512k distinct addresses
-    h->nRep = int(std::max<int64_t>(1, std::min<int64_t>(128, (524288 + L->n_instr - 1) / L->n_instr)));
+    h->nRep = int(std::max<int64_t>(1, std::min<int64_t>(128, (524288 + L->n_instr - 1) / std::max<int64_t>(L->n_instr, 1))));
 
     const int64_t m = L->n_obs;
     // coefficients and instrument columns are stored tile-transposed and padded to whole tiles
-    CK(dalloc(&h->V, h->nTiles * TILE * N_PAR));
+    CK(dalloc(&h->V, h->nTiles * TILE * h->nPar));
     CK(dalloc(&h->star, m));   // scratch of the upload: freed by gsr_upload_finish, allocated again by the next upload
     CK(dalloc(&h->tw, h->nTiles));
     CK(dalloc(&h->iatt, m));
     // instrument columns: 2 bytes each when they fit, else 4
     const bool ic16 = L->n_instr <= 65536;
-    if (ic16) CK(dalloc(&h->ic16, h->nTiles * TILE * N_INSTR));
-    else CK(dalloc(&h->ic, h->nTiles * TILE * N_INSTR));
+    if (ic16) CK(dalloc(&h->ic16, h->nTiles * TILE * h->nI));
+    else CK(dalloc(&h->ic, h->nTiles * TILE * h->nI));
     if (h->nTiles > 0) {   // zero the padding rows of the last tile
-        CK(cudaMemset(h->V + (h->nTiles - 1) * TILE * N_PAR, 0, sizeof(double) * TILE * N_PAR));
-        if (ic16) CK(cudaMemset(h->ic16 + (h->nTiles - 1) * TILE * N_INSTR, 0, sizeof(uint16_t) * TILE * N_INSTR));
-        else CK(cudaMemset(h->ic + (h->nTiles - 1) * TILE * N_INSTR, 0, sizeof(int32_t) * TILE * N_INSTR));
+        CK(cudaMemset(h->V + (h->nTiles - 1) * TILE * h->nPar, 0, sizeof(double) * TILE * h->nPar));
+        if (ic16) CK(cudaMemset(h->ic16 + (h->nTiles - 1) * TILE * h->nI, 0, sizeof(uint16_t) * TILE * h->nI));
+        else CK(cudaMemset(h->ic + (h->nTiles - 1) * TILE * h->nI, 0, sizeof(int32_t) * TILE * h->nI));
     }
     CK(dalloc(&h->b, h->mTot));
     CK(dalloc(&h->rp, L->n_stars + 1));
@@ -279,7 +292,7 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(dalloc(&h->p, h->n));
     CK(dalloc(&h->carryFirst, h->nTiles * N_ASTRO));
     CK(dalloc(&h->carryLast, h->nTiles * N_ASTRO));
-    CK(dalloc(&h->globPartial, std::max(h->gridA2, h->gridA2m)));
+    CK(dalloc(&h->globPartial, int64_t(std::max(h->gridA2, h->gridA2m)) * std::max(h->nG, 1)));
     CK(dalloc(&h->sqPartialU, std::max(h->gridA1, h->gridA2m) + h->gridCon));
     CK(dalloc(&h->t, h->n));
     CK(dalloc(&h->coefRaw, 2));
@@ -313,7 +326,7 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
             td.readMode = cudaReadModeElementType;
             return cudaCreateTextureObject(t, &rd, &td, nullptr);
         };
-        const bool tex = !(L->flags & GSR_FLAG_NO_TEX);
+        const bool tex = !(L->flags & GSR_FLAG_NO_TEX) && h->prod;
         if (tex && h->n < (int64_t(1) << 27)) CK(mk(&h->texV, h->v, h->n));
         if (tex && 3 * L->n_dof_att < (int64_t(1) << 27)) CK(mk(&h->texPack, h->xPack, 3 * L->n_dof_att));
     }
@@ -323,7 +336,7 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
         CK(cudaMemGetInfo(&freeB, &totB));
         const size_t need = size_t(m) * (N_ATT * 8 + 4 + 4) + size_t(m) * 12 + (size_t(64) << 20);
         // GSR_FLAG_NO_ATT_COPY forces the low-memory path (attitude REDs in k_aprod2, two-product iteration)
-        if (m > 0 && m < (int64_t(1) << 32) && L->n_dof_att < (int64_t(1) << 31) &&
+        if (h->prod && m > 0 && m < (int64_t(1) << 32) && L->n_dof_att < (int64_t(1) << 31) &&
             freeB > need + (size_t(2) << 30) && !(L->flags & GSR_FLAG_NO_ATT_COPY)) {
             bool ok = dalloc(&h->attT, m * N_ATT) == cudaSuccess && dalloc(&h->sT, m) == cudaSuccess &&
                       dalloc(&h->permT, m) == cudaSuccess;
@@ -393,7 +406,11 @@ int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double
 {
     if (!h) return GSR_EINVAL;
     if (row0 < 0 || nrows < 0 || row0 + nrows > h->L.n_obs) return fail(h, GSR_EINVAL, "row range");
-    if (nrows > 0 && (!values || !ia || !iatt || !ic || !b)) return fail(h, GSR_EINVAL, "null array");
+    if (nrows > 0 && (!values || (h->nA > 0 && !ia) || (h->nAtt > 0 && !iatt) || (h->nI > 0 && !ic) || !b))
+        return fail(h, GSR_EINVAL, "null array");
+    if (h->nA == 0) ia = nullptr;      // the index array of an absent section is ignored
+    if (h->nAtt == 0) iatt = nullptr;
+    if (h->nI == 0) ic = nullptr;
     int rc = enter(h);
     if (rc) return rc;
     h->uploaded = false;
@@ -403,19 +420,19 @@ int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double
     const size_t r = size_t(nrows);
     CK(cudaMemcpyAsync(h->b + row0, b, r * sizeof(double), cudaMemcpyDefault, h->stream));
     {   // the two i64 index arrays -> 4-byte star / attitude start (device sources in place, host sources staged)
-        const bool devI = nrows > 0 && isDevicePtr(ia) && isDevicePtr(iatt);
+        const bool devI = nrows > 0 && (!ia || isDevicePtr(ia)) && (!iatt || isDevicePtr(iatt));
         if (nrows > 0 && !devI && !h->stageI) CK(dalloc(&h->stageI, 2 * STAGE_ROWS));
-        for (int64_t q0 = 0; q0 < nrows; q0 += STAGE_ROWS) {
+        for (int64_t q0 = 0; (ia || iatt) && q0 < nrows; q0 += STAGE_ROWS) {
             const int64_t cnt = std::min(STAGE_ROWS, nrows - q0);
-            const int64_t *sa = ia + q0, *st = iatt + q0;
+            const int64_t *sa = ia ? ia + q0 : nullptr, *st = iatt ? iatt + q0 : nullptr;
             if (!devI) {
-                CK(cudaMemcpyAsync(h->stageI, sa, size_t(cnt) * sizeof(int64_t), cudaMemcpyDefault, h->stream));
-                CK(cudaMemcpyAsync(h->stageI + STAGE_ROWS, st, size_t(cnt) * sizeof(int64_t), cudaMemcpyDefault, h->stream));
-                sa = h->stageI;
-                st = h->stageI + STAGE_ROWS;
+                if (sa) CK(cudaMemcpyAsync(h->stageI, sa, size_t(cnt) * sizeof(int64_t), cudaMemcpyDefault, h->stream));
+                if (st) CK(cudaMemcpyAsync(h->stageI + STAGE_ROWS, st, size_t(cnt) * sizeof(int64_t), cudaMemcpyDefault, h->stream));
+                if (sa) sa = h->stageI;
+                if (st) st = h->stageI + STAGE_ROWS;
             }
             k_ingest_index<<<gridFor(cnt, 256, h->smCount * 16), 256, 0, h->stream>>>(
-                cnt, sa, st, h->L.n_stars, h->L.n_dof_att, h->star + row0 + q0, h->iatt + row0 + q0);
+                cnt, sa, st, h->L.n_stars, h->L.n_dof_att, h->nA, h->star + row0 + q0, h->iatt + row0 + q0);
             CK(cudaGetLastError());
         }
     }
@@ -424,24 +441,24 @@ int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double
     MatView A = view(h);
     const unsigned long long noneI = ~0ull;
     CK(cudaMemcpyAsync(h->badDev, &noneI, sizeof(noneI), cudaMemcpyHostToDevice, h->stream));
-    const bool devV = nrows > 0 && isDevicePtr(values), devC = nrows > 0 && isDevicePtr(ic);
+    const bool devV = nrows > 0 && isDevicePtr(values), devC = nrows > 0 && (!ic || isDevicePtr(ic));
     if (nrows > 0 && (!devV || !devC) && !h->stageV) {
-        CK(dalloc(&h->stageV, STAGE_ROWS * N_PAR));
-        CK(dalloc(&h->stageC, STAGE_ROWS * N_INSTR));
+        CK(dalloc(&h->stageV, STAGE_ROWS * h->nPar));
+        CK(dalloc(&h->stageC, STAGE_ROWS * h->nI));
     }
     for (int64_t q0 = 0; q0 < nrows; q0 += STAGE_ROWS) {
         const int64_t cnt = std::min(STAGE_ROWS, nrows - q0);
-        const double *srcV = values + q0 * N_PAR;
-        const int32_t *srcC = ic + q0 * N_INSTR;
+        const double *srcV = values + q0 * h->nPar;
+        const int32_t *srcC = ic ? ic + q0 * h->nI : nullptr;
         if (!devV) {
-            CK(cudaMemcpyAsync(h->stageV, srcV, size_t(cnt) * N_PAR * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+            CK(cudaMemcpyAsync(h->stageV, srcV, size_t(cnt) * h->nPar * sizeof(double), cudaMemcpyHostToDevice, h->stream));
             srcV = h->stageV;
         }
         if (!devC) {
-            CK(cudaMemcpyAsync(h->stageC, srcC, size_t(cnt) * N_INSTR * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
+            CK(cudaMemcpyAsync(h->stageC, srcC, size_t(cnt) * h->nI * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
             srcC = h->stageC;
         }
-        k_ingest_rows<<<gridFor(cnt * (N_PAR + N_INSTR), 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(
+        k_ingest_rows<<<gridFor(cnt * (h->nPar + h->nI), 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(
             A, h->ic, h->ic16, row0 + q0, cnt, srcV, srcC, h->badDev);
         CK(cudaGetLastError());
     }
@@ -477,8 +494,10 @@ int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail)
         return fail(h, GSR_EINDEX, "index contract violated at observation row %lld", (long long)bad);
     }
     h->badRow = -1;
-    k_star_rowptr<<<int((h->L.n_stars + 1 + 255) / 256), 256, 0, h->stream>>>(h->star, A.m, A.nStars, h->rp);
-    if (A.m > 0) k_tile_words<<<gridFor(h->nTiles, 8, h->smCount * 16), 256, 0, h->stream>>>(h->star, A.m, h->tw);
+    if (h->nA > 0) {
+        k_star_rowptr<<<int((h->L.n_stars + 1 + 255) / 256), 256, 0, h->stream>>>(h->star, A.m, A.nStars, h->rp);
+        if (A.m > 0) k_tile_words<<<gridFor(h->nTiles, 8, h->smCount * 16), 256, 0, h->stream>>>(h->star, A.m, h->tw);
+    }
     CK(cudaGetLastError());
     k_fill<<<h->gridVec, 256, 0, h->stream>>>(h->p, h->n, 1.0);
     CK(cudaGetLastError());
@@ -489,8 +508,8 @@ int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail)
         unsigned int *cnt = nullptr;
         CK(dalloc(&cnt, h->L.n_instr + 1));
         CK(cudaMemsetAsync(cnt, 0, sizeof(unsigned int) * size_t(h->L.n_instr + 1), h->stream));
-        if (A.m > 0) {
-            k_instr_hist<<<gridFor(h->nTiles * TILE * N_INSTR, 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(A, cnt);
+        if (A.m > 0 && h->nI > 0) {
+            k_instr_hist<<<gridFor(h->nTiles * TILE * h->nI, 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(A, cnt);
             k_max_u32<<<gridFor(h->L.n_instr, 256, h->smCount), 256, 0, h->stream>>>(cnt, h->L.n_instr, cnt + h->L.n_instr);
         }
         unsigned int mx = 0;
@@ -498,7 +517,7 @@ int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail)
         if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
         cudaFree(cnt);
         CK(e);
-        const double mean = double(A.m) * N_INSTR / double(h->L.n_instr);
+        const double mean = double(A.m) * h->nI / double(std::max<int64_t>(h->L.n_instr, 1));
         h->instrSkewed = double(mx) > 64.0 * std::max(mean, 1.0);
         if (h->iterGraph) {   // the captured iteration names the kernel variant
             cudaGraphExecDestroy(h->iterGraph);
@@ -589,7 +608,8 @@ void launchAtt(gsr_handle *h, const MatView &A, const double *y, double *x, cons
 void launchAprod1(gsr_handle *h, const MatView &A, const double *x, double *y, const double *coef, double *sq,
                   const int *done)
 {
-    if (h->ic16) k_aprod1<true><<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done, h->xPack);
+    if (!h->prod) k_aprod1_gen<<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done);
+    else if (h->ic16) k_aprod1<true><<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done, h->xPack);
     else k_aprod1<false><<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done, h->xPack);
 }
 
@@ -597,7 +617,10 @@ void launchAprod1(gsr_handle *h, const MatView &A, const double *x, double *y, c
 template <bool SQUARE>
 void launchAprod2Red(gsr_handle *h, const MatView &A, const double *y, double *x, const double *coef, const int *done)
 {
-    if (h->ic16)
+    if (!h->prod)
+        k_aprod2_gen<SQUARE><<<h->gridA2, THREADS, 0, h->stream>>>(A, y, x, coef, h->carryFirst, h->carryLast,
+                                                                  h->globPartial, done);
+    else if (h->ic16)
         k_aprod2<true, SQUARE, true><<<h->gridA2, THREADS, 0, h->stream>>>(A, y, x, coef, h->carryFirst, h->carryLast,
                                                                           h->globPartial, done);
     else
@@ -630,8 +653,10 @@ int enqueueAprod1(gsr_handle *h, const double *x, double *y, const double *coef,
 {
     MatView A = view(h);
     int nk = 1, np = h->gridA1;
-    k_pack_att<<<h->gridVec, 256, 0, h->stream>>>(A, x, h->xPack, done);
-    ++nk;
+    if (h->prod) {   // the specialised kernel gathers the attitude unknowns from their axis-interleaved copy
+        k_pack_att<<<h->gridVec, 256, 0, h->stream>>>(A, x, h->xPack, done);
+        ++nk;
+    }
     launchAprod1(h, A, x, y, coef, sqPartial, done);
     if (A.nCon > 0) {
         k_con_aprod1<<<h->gridCon, 256, 0, h->stream>>>(A, x, y, coef, sqPartial ? sqPartial + h->gridA1 : nullptr, done);
@@ -649,8 +674,8 @@ int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef,
 {
     MatView A = view(h);
     int nk = 1;
-    k_pre_aprod2<<<h->gridVec, 256, 0, h->stream>>>(x, A.offAtt, A.n, coef, h->insRep, int64_t(h->nRep) * A.nInstr,
-                                                    prescale ? 1 : 0, done);
+    k_pre_aprod2<<<h->gridVec, 256, 0, h->stream>>>(x, A.offAtt, A.n, coef, h->insRep,
+                                                    h->prod ? int64_t(h->nRep) * A.nInstr : 0, prescale ? 1 : 0, done);
     // attitude section: segmented reduction on the time-ordered copy when there is one; the
     // preconditioner pass (SQUARE) and the low-memory fallback scatter it with REDs in k_aprod2
     const bool attRed = SQUARE || !h->useAttT;
@@ -661,8 +686,11 @@ int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef,
         launchAprod2Main<false>(h, A, y, x, coef, done, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0});
         ++nk;
     }
-    k_astro_fixup<<<h->gridFix, 256, 0, h->stream>>>(A, x, coef, h->carryFirst, h->carryLast, h->globPartial,
-                                                     attRed ? h->gridA2 : h->gridA2m, done);
+    if (h->prod)
+        k_astro_fixup<<<h->gridFix, 256, 0, h->stream>>>(A, x, coef, h->carryFirst, h->carryLast, h->globPartial,
+                                                         attRed ? h->gridA2 : h->gridA2m, done);
+    else
+        k_fixup_gen<<<h->gridFix, 256, 0, h->stream>>>(A, x, coef, h->carryFirst, h->carryLast, h->globPartial, h->gridA2, done);
     nk += 2;
     if (A.nCon > 0) {
         k_con_aprod2<SQUARE><<<h->gridCon, 256, 0, h->stream>>>(A, y, x, coef, done);
@@ -676,7 +704,7 @@ int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef,
 // GSR_FLAG_NO_FUSE (gsr_layout.flags) selects the two-product form.
 bool canFuse(const gsr_handle *h)
 {
-    return !(h->L.flags & GSR_FLAG_NO_FUSE) && h->useAttT && h->L.n_obs > 0;
+    return h->prod && !(h->L.flags & GSR_FLAG_NO_FUSE) && h->useAttT && h->L.n_obs > 0;
 }
 
 int enqueueIterationFused(gsr_handle *h)
@@ -741,6 +769,7 @@ int32_t gsr_get_star_rowptr(gsr_handle *h, int64_t *out)
 {
     if (!h || !out) return GSR_EINVAL;
     if (!h->uploaded) return fail(h, GSR_ESTATE, "no system uploaded");
+    if (h->nA == 0) return fail(h, GSR_ESTATE, "layout has no astrometric section: no star row pointer");
     int rc = enter(h);
     if (rc) return rc;
     CK(cudaMemcpyAsync(out, h->rp, size_t(h->L.n_stars + 1) * sizeof(int64_t), cudaMemcpyDefault, h->stream));
@@ -769,16 +798,16 @@ int32_t gsr_get_values(gsr_handle *h, double *out, double *con_val_out)
         const int64_t m = h->L.n_obs;
         const bool devOut = isDevicePtr(out);
         if (m > 0 && !devOut && !h->stageV) {
-            CK(dalloc(&h->stageV, STAGE_ROWS * N_PAR));
-            CK(dalloc(&h->stageC, STAGE_ROWS * N_INSTR));
+            CK(dalloc(&h->stageV, STAGE_ROWS * h->nPar));
+            CK(dalloc(&h->stageC, STAGE_ROWS * h->nI));
         }
         for (int64_t q0 = 0; q0 < m; q0 += STAGE_ROWS) {
             const int64_t cnt = std::min(STAGE_ROWS, m - q0);
-            double *dst = devOut ? out + q0 * N_PAR : h->stageV;
-            k_export_rows<<<gridFor(cnt * N_PAR, 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(A, q0, cnt, dst);
+            double *dst = devOut ? out + q0 * h->nPar : h->stageV;
+            k_export_rows<<<gridFor(cnt * h->nPar, 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(A, q0, cnt, dst);
             CK(cudaGetLastError());
             if (!devOut)
-                CK(cudaMemcpyAsync(out + q0 * N_PAR, h->stageV, size_t(cnt) * N_PAR * sizeof(double),
+                CK(cudaMemcpyAsync(out + q0 * h->nPar, h->stageV, size_t(cnt) * h->nPar * sizeof(double),
                                    cudaMemcpyDeviceToHost, h->stream));
         }
     }
@@ -804,7 +833,7 @@ int32_t gsr_precondition(gsr_handle *h)
     enqueueAprod2<true>(h, nullptr, h->p, h->coefOne, nullptr, false);
     CK(cudaGetLastError());
     k_colscale<<<h->gridVec, 256, 0, h->stream>>>(h->p, h->n);
-    k_scale_values<<<gridFor(h->nTiles * TILE * N_PAR, 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(A, h->p);
+    k_scale_values<<<gridFor(h->nTiles * TILE * h->nPar, 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(A, h->p);
     if (A.nCon > 0)
         k_scale_con_values<<<gridFor(h->L.n_con_nnz, 256, h->smCount * 16), 256, 0, h->stream>>>(A, h->L.n_con_nnz, h->p);
     if (h->useAttT)   // the time-ordered copy takes the same factors
@@ -1000,7 +1029,7 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
     // bounded operands: u = b, v = 1e-3; coefficients 0.5 keep repeated products finite
     CK(cudaMemcpyAsync(h->u, h->b, size_t(h->mTot) * sizeof(double), cudaMemcpyDeviceToDevice, st));
     k_fill<<<h->gridVec, 256, 0, st>>>(h->v, h->n, 1e-3);
-    k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, nullptr);   // operand of k_aprod1 / the fused pass timed alone
+    if (h->prod) k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, nullptr);   // operand of k_aprod1 / the fused pass timed alone
     k_pre_aprod2<<<h->gridVec, 256, 0, st>>>(h->t, 0, A.n, h->coefRaw, h->insRep, int64_t(h->nRep) * A.nInstr, 2, nullptr);
     auto once = [&]() {
         if (which == GSR_TIME_APROD1_GROUP) enqueueAprod1(h, h->v, h->u, h->coefTime, h->sqPartialU, nullptr, nullptr);

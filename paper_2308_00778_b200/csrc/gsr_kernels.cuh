@@ -35,8 +35,10 @@ constexpr int ATT_BLOCK_BITS = 21;   // rows per block of the time-ordered attit
 // coefficients with one coalesced 8-byte load per warp instruction (256 B, two lines) and no
 // shared-memory transposition.  instrCol likewise: ic[(tile*6 + j)*32 + lane].  Storage is padded
 // to whole tiles (zero coefficients, column 0).  The upload format stays row-major.
-__host__ __device__ __forceinline__ int64_t vpos(int64_t i, int k) { return ((i >> 5) * N_PAR + k) * TILE + (i & 31); }
-__host__ __device__ __forceinline__ int64_t cpos(int64_t i, int j) { return ((i >> 5) * N_INSTR + j) * TILE + (i & 31); }
+// Other section widths (model variants): the same layout with nPar coefficients / nI columns per row.
+__host__ __device__ __forceinline__ int64_t vpos(int64_t i, int k, int nPar = N_PAR) { return ((i >> 5) * nPar + k) * TILE + (i & 31); }
+__host__ __device__ __forceinline__ int64_t cpos(int64_t i, int j, int nI = N_INSTR) { return ((i >> 5) * nI + j) * TILE + (i & 31); }
+constexpr int MAX_GLOB = 16;      // widest global section (GSR_MAX_GLOB in gsr.h)
 
 // Device view of the uploaded system (A_d, M_i, I_c) in upload layout.
 struct MatView {
@@ -54,6 +56,9 @@ struct MatView {
     const int64_t *rp;     // [nStars+1] derived star row pointer
     int64_t m, nStars, nDof, nInstr;
     int64_t offAtt, offInstr, offGlob, n;
+    // section widths: 5 / 12 / 6 / 1 in production (the kernels specialised for it use the constants above);
+    // a section of width 0 has no columns.  nPar = nA + nAtt + nI + nG coefficients per stored row.
+    int nA, nAtt, nI, nG, nPar;
     // constraint rows (CSR, absolute columns)
     const int64_t *conRp, *conCol;
     double *conVal;
@@ -672,6 +677,182 @@ __global__ void k_sort_keys(const int32_t *__restrict__ iatt, int64_t i0, int64_
 }
 
 // ---------------------------------------------------------------------------------------
+// Model variants.  PAPER.md:78 allows 0 <= N_Astro <= 5 astrometric and 0 <= N_Instr <= 6
+// instrumental coefficients per row and runs with or without the global part; the paper also ran 5 global
+// parameters, and its 40 / 100 / 300 GB datasets solve only some of the sections.
+// These two kernels compute the same products (Eq. 2-3, Alg. 2-3) for any such layout: the section widths are
+// read from MatView at run time, every coefficient is loaded where it is used (coalesced, tile-transposed storage
+// of width nPar) and nothing is kept in per-thread arrays.  The 5/12/6/1 production layout keeps its specialised
+// kernels above.  aprod2: astro by the same segmented scan (no atomics, carries for stars cut by a tile edge),
+// attitude and instrumental by RED.ADD.F64, every global column by warp sum -> per-warp shared-memory
+// accumulator -> CTA partial -> k_fixup_gen (fixed order).
+// ---------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(THREADS)
+k_aprod1_gen(MatView A, const double *__restrict__ x, double *__restrict__ y, const double *__restrict__ coef,
+             double *__restrict__ sqPartial, const int *done)
+{
+    __shared__ double red[32];
+    if (done && *done) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const double cx = coef[0], cy = coef[1];
+    const int64_t nTiles = (A.m + TILE - 1) / TILE;
+    const int kT = A.nA + A.nAtt, kI = kT + A.nI;
+    double sq = 0.0;
+    for (int64_t tile = int64_t(blockIdx.x) * WARPS + warp; tile < nTiles; tile += int64_t(gridDim.x) * WARPS) {
+        const int64_t r0 = tile * TILE;
+        const int nrows = int(min(int64_t(TILE), A.m - r0));
+        if (lane < nrows) {
+            const int64_t i = r0 + lane;
+            const double *g = A.V + tile * (int64_t(A.nPar) * TILE) + lane;
+            double sum = 0.0;
+            if (A.nA > 0) {
+                const double *xa = x + A.nA * star_of(A, __ldg(A.tw + tile), i, lane);
+                GSR_ASSERT(xa >= x && xa + A.nA <= x + A.offAtt);
+                for (int k = 0; k < A.nA; ++k) sum = fma(__ldcs(g + k * TILE), __ldg(xa + k), sum);
+            }
+            if (A.nAtt > 0) {
+                const int64_t s = __ldcs(A.iatt + i);
+                GSR_ASSERT(s >= 0 && s + 4 <= A.nDof);
+                const double *xt = x + A.offAtt + s;
+#pragma unroll
+                for (int a = 0; a < 3; ++a)
+#pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        sum = fma(__ldcs(g + (A.nA + 4 * a + j) * TILE), __ldg(xt + a * A.nDof + j), sum);
+            }
+            for (int j = 0; j < A.nI; ++j) {
+                const int32_t c = ic_at(A, (tile * A.nI + j) * TILE + lane);
+                GSR_ASSERT(c >= 0 && c < A.nInstr);
+                sum = fma(__ldcs(g + (kT + j) * TILE), __ldg(x + A.offInstr + c), sum);
+            }
+            for (int q = 0; q < A.nG; ++q) sum = fma(__ldcs(g + (kI + q) * TILE), __ldg(x + A.offGlob + q), sum);
+            const double yi = fma(cy, y[i], cx * sum);
+            y[i] = yi;
+            sq = fma(yi, yi, sq);
+        }
+    }
+    const double b = block_sum(sq, red);
+    if (threadIdx.x == 0 && sqPartial) sqPartial[blockIdx.x] = b;
+}
+
+// x <- cx*x + cy*(A^T y); the attitude / instrumental / global sections of x were multiplied by cx beforehand
+// (k_pre_aprod2).  globPartial[q*gridDim.x + blockIdx.x]: this CTA's share of global column q.
+template <bool SQUARE>
+__global__ void __launch_bounds__(THREADS)
+k_aprod2_gen(MatView A, const double *__restrict__ y, double *__restrict__ x, const double *__restrict__ coef,
+             double *__restrict__ carryFirst, double *__restrict__ carryLast, double *__restrict__ globPartial,
+             const int *done)
+{
+    __shared__ double gAcc[WARPS][MAX_GLOB];
+    if (done && *done) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const double cx = coef[0], cy = coef[1];
+    const int64_t nTiles = (A.m + TILE - 1) / TILE;
+    const int kT = A.nA + A.nAtt, kI = kT + A.nI;
+    if (lane < MAX_GLOB) gAcc[warp][lane] = 0.0;
+    __syncwarp();
+    for (int64_t tile = int64_t(blockIdx.x) * WARPS + warp; tile < nTiles; tile += int64_t(gridDim.x) * WARPS) {
+        const int64_t r0 = tile * TILE;
+        const int nrows = int(min(int64_t(TILE), A.m - r0));
+        const bool valid = lane < nrows;
+        const int ln = valid ? lane : nrows - 1;
+        const int64_t i = r0 + ln;
+        const double *g = A.V + tile * (int64_t(A.nPar) * TILE) + ln;
+        const double yv = valid ? (SQUARE ? 1.0 : cy * y[i]) : 0.0;     // lanes past the last row add zeros
+        if (A.nA > 0) {   // ---- astro: segmented scan by star, as in k_aprod2
+            const unsigned long long tw = __ldg(A.tw + tile);
+            const int64_t ia = A.nA * star_of(A, tw, i, ln);
+            GSR_ASSERT(ia >= 0 && ia + A.nA <= A.offAtt);
+            const unsigned heads = uint32_t(tw) | 1u;
+            const bool tail = valid && ((lane == nrows - 1) || ((heads >> 1) >> lane) & 1u);
+            const int segStart = 31 - __clz(heads & (0xffffffffu >> (31 - lane)));
+            const int dist = lane - segStart;
+            bool cut = false;
+            if (segStart == 0) cut = !(uint32_t(tw) & 1u);
+            if (lane == nrows - 1) cut = cut || ((tw >> 61) & 1ull);
+            for (int k = 0; k < A.nA; ++k) {
+                const double a = __ldcs(g + k * TILE);
+                double s = SQUARE ? a * a * yv : a * yv;
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const double t = __shfl_up_sync(0xffffffffu, s, d);
+                    if (dist >= d) s += t;
+                }
+                if (tail) {
+                    if (!cut) x[ia + k] = fma(cx, x[ia + k], s);
+                    else (segStart == 0 ? carryFirst : carryLast)[tile * N_ASTRO + k] = s;
+                }
+            }
+        }
+        if (A.nAtt > 0 && valid) {   // ---- attitude
+            const int64_t s = __ldcs(A.iatt + i);
+            GSR_ASSERT(s >= 0 && s + 4 <= A.nDof);
+            double *xt = x + A.offAtt + s;
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const double v = __ldcs(g + (A.nA + 4 * a + j) * TILE);
+                    atomicAdd(xt + a * A.nDof + j, SQUARE ? v * v * yv : v * yv);
+                }
+        }
+        if (valid)   // ---- instrumental
+            for (int j = 0; j < A.nI; ++j) {
+                const int32_t c = ic_at(A, (tile * A.nI + j) * TILE + lane);
+                GSR_ASSERT(c >= 0 && c < A.nInstr);
+                const double v = __ldcs(g + (kT + j) * TILE);
+                atomicAdd(x + A.offInstr + c, SQUARE ? v * v * yv : v * yv);
+            }
+        for (int q = 0; q < A.nG; ++q) {   // ---- global columns: fixed-order warp sum into this warp's accumulator
+            const double v = __ldcs(g + (kI + q) * TILE);
+            const double t = warp_sum(SQUARE ? v * v * yv : v * yv);
+            if (lane == 0) gAcc[warp][q] += t;
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x < A.nG) {
+        double t = 0.0;
+        for (int w = 0; w < WARPS; ++w) t += gAcc[w][threadIdx.x];
+        globPartial[int64_t(threadIdx.x) * gridDim.x + blockIdx.x] = t;
+    }
+}
+
+// Finishes the astro section (stars cut by tile edges, stars without rows) and the global columns of k_aprod2_gen.
+__global__ void __launch_bounds__(256)
+k_fixup_gen(MatView A, double *__restrict__ x, const double *__restrict__ coef, const double *__restrict__ carryFirst,
+            const double *__restrict__ carryLast, const double *__restrict__ globPartial, int nGlobPartial, const int *done)
+{
+    __shared__ double red[32];
+    if (done && *done) return;
+    const double cx = coef[0];
+    if (blockIdx.x == gridDim.x - 1) {
+        for (int q = 0; q < A.nG; ++q) {
+            double g = 0.0;
+            for (int p = threadIdx.x; p < nGlobPartial; p += blockDim.x) g += globPartial[int64_t(q) * nGlobPartial + p];
+            g = block_sum(g, red);
+            if (threadIdx.x == 0) x[A.offGlob + q] += g;   // section already scaled by cx
+        }
+        return;
+    }
+    const int64_t s = int64_t(blockIdx.x) * blockDim.x + threadIdx.x;
+    if (s >= A.nStars) return;
+    const int64_t r0 = A.rp[s], r1 = A.rp[s + 1];
+    double *xa = x + s * A.nA;
+    if (r0 == r1) {
+        for (int k = 0; k < A.nA; ++k) xa[k] *= cx;
+        return;
+    }
+    const int64_t t0 = r0 / TILE, t1 = (r1 - 1) / TILE;
+    if (t0 == t1) return;   // stored by k_aprod2_gen
+    for (int k = 0; k < A.nA; ++k) {
+        double acc = 0.0;
+        for (int64_t t = t0; t <= t1; ++t)
+            acc += ((t == t0 && r0 != t * TILE) ? carryLast : carryFirst)[t * N_ASTRO + k];
+        xa[k] = fma(cx, xa[k], acc);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
 // Constraint rows ("Constraints kernels"): CSR tail below the
 // observation rows.  aprod1: one warp per row; aprod2: one thread per non-zero (RED).
 // ---------------------------------------------------------------------------------------
@@ -910,11 +1091,10 @@ __global__ void k_validate(MatView A, unsigned long long *badRow)
          i += int64_t(gridDim.x) * blockDim.x) {
         // k_ingest_index stored -1 for a matrixIndexAstro that is not 5*star with star in [0, nStars) and for a
         // matrixIndexAtt outside [0, nDof-4]
-        bool bad = A.star[i] < 0 || A.iatt[i] < 0;
-        if (i > 0) bad = bad || A.star[i - 1] > A.star[i];
-#pragma unroll
-        for (int j = 0; j < N_INSTR; ++j) {
-            const int32_t c = ic_at(A, cpos(i, j));
+        bool bad = (A.nA > 0 && A.star[i] < 0) || (A.nAtt > 0 && A.iatt[i] < 0);
+        if (A.nA > 0 && i > 0) bad = bad || A.star[i - 1] > A.star[i];
+        for (int j = 0; j < A.nI; ++j) {
+            const int32_t c = ic_at(A, cpos(i, j, A.nI));
             bad = bad || c < 0 || c >= A.nInstr;
         }
         if (bad) atomicMin(badRow, (unsigned long long)i);
@@ -962,14 +1142,20 @@ __global__ void k_tile_words(const int32_t *__restrict__ star, int64_t m, unsign
 
 // Upload: matrixIndexAstro / matrixIndexAtt (i64, "M_i") -> 4-byte star and attitude start;
 // a value that breaks its contract becomes -1 and is reported by k_validate.
+// nA: astrometric unknowns per star (matrixIndexAstro = nA*star); a section that is absent passes a null array.
 __global__ void k_ingest_index(int64_t cnt, const int64_t *__restrict__ ia, const int64_t *__restrict__ iatt,
-                               int64_t nStars, int64_t nDof, int32_t *__restrict__ star, int32_t *__restrict__ att)
+                               int64_t nStars, int64_t nDof, int nA, int32_t *__restrict__ star, int32_t *__restrict__ att)
 {
     for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < cnt;
          q += int64_t(gridDim.x) * blockDim.x) {
-        const int64_t a = ia[q], s = iatt[q];
-        star[q] = (a >= 0 && a % 5 == 0 && a / 5 < nStars) ? int32_t(a / 5) : -1;
-        att[q] = (s >= 0 && s <= nDof - 4) ? int32_t(s) : -1;
+        if (ia) {
+            const int64_t a = ia[q];
+            star[q] = (a >= 0 && a % nA == 0 && a / nA < nStars) ? int32_t(a / nA) : -1;
+        }
+        if (iatt) {
+            const int64_t s = iatt[q];
+            att[q] = (s >= 0 && s <= nDof - 4) ? int32_t(s) : -1;
+        }
     }
 }
 
@@ -1003,20 +1189,21 @@ __global__ void k_colscale(double *__restrict__ p, int64_t n)
 // One thread per stored coefficient (coalesced over A_d).
 __global__ void k_scale_values(MatView A, const double *__restrict__ p)
 {
-    const int64_t total = ((A.m + TILE - 1) / TILE) * (N_PAR * TILE);
+    const int64_t total = ((A.m + TILE - 1) / TILE) * (int64_t(A.nPar) * TILE);
+    const int kT = A.nA + A.nAtt, kI = kT + A.nI;
     for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < total;
          e += int64_t(gridDim.x) * blockDim.x) {
-        // e = (tile*24 + k)*32 + lane
+        // e = (tile*nPar + k)*32 + lane
         const int64_t tk = e >> 5;
-        const int64_t tile = tk / N_PAR;
-        const int k = int(tk - tile * N_PAR);
+        const int64_t tile = tk / A.nPar;
+        const int k = int(tk - tile * A.nPar);
         const int64_t i = tile * TILE + (e & 31);
         if (i >= A.m) continue;
         int64_t c;
-        if (k < N_ASTRO) c = 5 * star_of(A, A.tw[tile], i, int(e & 31)) + k;
-        else if (k < N_ASTRO + N_ATT) c = A.offAtt + ((k - N_ASTRO) >> 2) * A.nDof + A.iatt[i] + ((k - N_ASTRO) & 3);
-        else if (k < N_PAR - 1) c = A.offInstr + ic_at(A, cpos(i, k - N_ASTRO - N_ATT));
-        else c = A.offGlob;
+        if (k < A.nA) c = A.nA * star_of(A, A.tw[tile], i, int(e & 31)) + k;
+        else if (k < kT) c = A.offAtt + ((k - A.nA) >> 2) * A.nDof + A.iatt[i] + ((k - A.nA) & 3);
+        else if (k < kI) c = A.offInstr + ic_at(A, cpos(i, k - kT, A.nI));
+        else c = A.offGlob + (k - kI);
         A.V[e] = A.V[e] * p[c];
     }
 }
@@ -1037,34 +1224,34 @@ __global__ void k_ingest_rows(MatView A, int32_t *__restrict__ icDev, uint16_t *
                               const double *__restrict__ values, const int32_t *__restrict__ ic,
                               unsigned long long *badRow)
 {
-    const int64_t nV = cnt * N_PAR, nC = cnt * N_INSTR;
+    const int64_t nV = cnt * A.nPar, nC = cnt * A.nI;
     for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < nV + nC;
          e += int64_t(gridDim.x) * blockDim.x) {
         if (e < nV) {
-            const int64_t r = e / N_PAR;
-            A.V[vpos(row0 + r, int(e - r * N_PAR))] = values[e];
+            const int64_t r = e / A.nPar;
+            A.V[vpos(row0 + r, int(e - r * A.nPar), A.nPar)] = values[e];
         } else {
-            const int64_t f = e - nV, r = f / N_INSTR;
+            const int64_t f = e - nV, r = f / A.nI;
             const int32_t c = ic[f];
             if (ic16Dev) {
                 const bool ok = c >= 0 && c < A.nInstr;
-                ic16Dev[cpos(row0 + r, int(f - r * N_INSTR))] = ok ? uint16_t(c) : uint16_t(0);
+                ic16Dev[cpos(row0 + r, int(f - r * A.nI), A.nI)] = ok ? uint16_t(c) : uint16_t(0);
                 if (!ok) atomicMin(badRow, (unsigned long long)(row0 + r));
             } else {
-                icDev[cpos(row0 + r, int(f - r * N_INSTR))] = c;
+                icDev[cpos(row0 + r, int(f - r * A.nI), A.nI)] = c;
             }
         }
     }
 }
 
-// out[(i - row0)*24 + k] = V(i, k) for rows [row0, row0+cnt): the row-major view for gsr_get_values.
+// out[(i - row0)*nPar + k] = V(i, k) for rows [row0, row0+cnt): the row-major view for gsr_get_values.
 __global__ void k_export_rows(MatView A, int64_t row0, int64_t cnt, double *__restrict__ out)
 {
-    const int64_t nV = cnt * N_PAR;
+    const int64_t nV = cnt * A.nPar;
     for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < nV;
          e += int64_t(gridDim.x) * blockDim.x) {
-        const int64_t r = e / N_PAR;
-        out[e] = A.V[vpos(row0 + r, int(e - r * N_PAR))];
+        const int64_t r = e / A.nPar;
+        out[e] = A.V[vpos(row0 + r, int(e - r * A.nPar), A.nPar)];
     }
 }
 
@@ -1072,10 +1259,10 @@ __global__ void k_export_rows(MatView A, int64_t row0, int64_t cnt, double *__re
 // the largest count against the mean decides whether aprod2 pre-sums equal columns inside a warp.
 __global__ void k_instr_hist(MatView A, unsigned int *__restrict__ cnt)
 {
-    const int64_t total = ((A.m + TILE - 1) / TILE) * (N_INSTR * TILE);
+    const int64_t total = ((A.m + TILE - 1) / TILE) * (int64_t(A.nI) * TILE);
     for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < total;
          e += int64_t(gridDim.x) * blockDim.x) {
-        const int64_t i = (e / (N_INSTR * TILE)) * TILE + (e & 31);
+        const int64_t i = (e / (A.nI * TILE)) * TILE + (e & 31);
         if (i < A.m) atomicAdd(cnt + ic_at(A, e), 1u);
     }
 }

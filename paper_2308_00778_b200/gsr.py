@@ -150,13 +150,14 @@ class Gsr:
     """One system on one GPU.  Methods mirror the C entry points one to one."""
 
     def __init__(self, n_obs, n_stars, n_dof_att, n_instr, n_con=0, n_con_nnz=0, device=0, stream=None, flags=0,
-                 n_glob=1):
+                 n_glob=1, n_astro_par=5, n_att_par=12, n_instr_par=6):
         self.lib = load_library()
         self._h = C.c_void_p()
         if stream is None and torch.cuda.is_available():
             stream = torch.cuda.current_stream(device).cuda_stream
-        L = _Layout(n_obs, n_stars, n_dof_att, n_instr, n_con, n_con_nnz, 5, 12, 6, n_glob, device, flags,
-                    stream or None)
+        L = _Layout(n_obs, n_stars, n_dof_att, n_instr, n_con, n_con_nnz, n_astro_par, n_att_par, n_instr_par, n_glob,
+                    device, flags, stream or None)
+        self.n_par = n_astro_par + n_att_par + n_instr_par + n_glob
         rc = self.lib.gsr_create(C.byref(L), C.byref(self._h))
         if rc != GSR_OK:
             msg = self.lib.gsr_last_error(self._h).decode() if self._h else "gsr_create failed"
@@ -227,7 +228,7 @@ class Gsr:
         return out
 
     def gsr_get_values(self):
-        out = torch.empty((self.n_obs, 24), dtype=torch.float64, device=self.device)
+        out = torch.empty((self.n_obs, self.n_par), dtype=torch.float64, device=self.device)
         con = torch.empty(self.n_con_nnz, dtype=torch.float64, device=self.device) if self.n_con_nnz else None
         self._ck(self.lib.gsr_get_values(self._h, out.data_ptr(), None if con is None else con.data_ptr()))
         return out, con

@@ -4,6 +4,8 @@ Tolerances (BASELINE north_star): index/layout arrays bit-exact; every aprod out
 1e-12 * sum|terms|; LSQR x after a fixed iteration count within 1e-9 relative L2, same istop,
 itn within +-2.
 """
+import dataclasses
+
 import numpy as np
 import pytest
 import torch
@@ -30,9 +32,13 @@ def dev(a):
 
 def make_gpu(S, d, b, upload_constraints=True, flags=0):
     gsr = gsr_mod()
-    G = gsr.Gsr(S.m, S.n_stars, S.n_dof_att, S.n_instr, S.n_con, len(S.con_col), flags=flags)
-    G.gsr_upload(np.ascontiguousarray(d["values"]), np.ascontiguousarray(d["matrixIndexAstro"]),
-                 np.ascontiguousarray(d["matrixIndexAtt"]), np.ascontiguousarray(d["instrCol"]), b)
+    G = gsr.Gsr(S.m, S.n_stars, S.n_dof_att, S.n_instr, S.n_con, len(S.con_col), flags=flags, n_glob=S.n_glob,
+                n_astro_par=S.n_astro_par, n_att_par=S.n_att_par, n_instr_par=S.n_instr_par)
+    # the index array of a section the layout does not have is not passed at all
+    G.gsr_upload(np.ascontiguousarray(d["values"]),
+                 np.ascontiguousarray(d["matrixIndexAstro"]) if S.n_astro_par else None,
+                 np.ascontiguousarray(d["matrixIndexAtt"]) if S.n_att_par else None,
+                 np.ascontiguousarray(d["instrCol"]) if S.n_instr_par else None, b)
     if S.n_con and upload_constraints:
         G.gsr_upload_constraints(S.con_rowptr, S.con_col, S.con_val)
     return G
@@ -610,3 +616,89 @@ def test_fallback_paths(flag, case):
         if flag != "NO_TEX":
             with pytest.raises(gsr.GsrError):
                 G.gsr_time_aprod(gsr.GSR_TIME_K_FUSED, 1)
+
+
+# ----------------------------------------------------------------------------- model variants
+VARIANT_LAYOUTS = [   # (n_astro_par, n_att_par, n_instr_par, n_glob)
+    (0, 12, 6, 0),    # attitude + instrumental only (the paper's 40 / 300 GB datasets)
+    (5, 0, 0, 0),     # astrometric only (100 GB dataset)
+    (5, 12, 6, 0),    # no global part (350 GB dataset; "so far ... we have run without computing a global part")
+    (5, 12, 6, 5),    # five global parameters
+    (3, 12, 4, 2),
+    (2, 0, 1, 16),    # widest global section the library takes
+]
+
+
+def variant_cfg(widths, shape):
+    na, nt, ni, ng = widths
+    base = {"ragged": synth.mini(seed=21, n_stars=37, obs=23, n_dof_att=64, n_instr=10),                 # 851 rows
+            "powerlaw": synth.SynthConfig("plv", 400, 300, 50, obs_powerlaw=(2.0, 8, 200), att_bursts=(5, 1e-2, 0.9),
+                                          instr_zipf=1.1, seed=22),                                       # stars cut by tile edges
+            "multi_cta": synth.SynthConfig("mc", 3_000, 2_000, 70_000, obs_per_star=41, seed=23)}[shape]  # 123,000 rows, 4-byte columns
+    return dataclasses.replace(base, n_astro_par=na, n_att_par=nt, n_instr_par=ni, n_glob=ng)
+
+
+@pytest.mark.parametrize("shape", ["ragged", "powerlaw", "multi_cta"])
+@pytest.mark.parametrize("widths", VARIANT_LAYOUTS)
+def test_model_variants_aprod_and_precondition(widths, shape):
+    """Layouts other than 5/12/6/1 (general kernels k_aprod1_gen / k_aprod2_gen): sizes, star row pointer, both products
+    element by element, the preconditioner and the scaled coefficients against the oracle."""
+    cfg = variant_cfg(widths, shape)
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    with make_gpu(S, d, b) as G:
+        assert G.n == S.n == cfg.n and G.m_tot == S.m_tot
+        assert not (G.gsr_path_info() & (gsr_mod().GSR_PATH_FUSED | gsr_mod().GSR_PATH_ATT_COPY))
+        if widths[0]:
+            rp = G.gsr_get_star_rowptr().cpu().numpy()
+            assert np.array_equal(rp, d["rowptr"])
+        else:
+            with pytest.raises(gsr_mod().GsrError):
+                G.gsr_get_star_rowptr()
+        check_aprods(S, G, seed=3)
+        G.gsr_precondition()
+        po = S.precondition()
+        np.testing.assert_allclose(G.gsr_get_colscale().cpu().numpy(), po, rtol=P_TOL, atol=0)
+        V, _ = G.gsr_get_values()
+        assert V.shape == S.V.shape
+        np.testing.assert_allclose(V.cpu().numpy(), S.V, rtol=P_TOL, atol=0)
+        check_aprods_scaled(S, G)
+
+
+@pytest.mark.parametrize("widths", VARIANT_LAYOUTS)
+def test_model_variants_lsqr(widths):
+    cfg = variant_cfg(widths, "ragged")
+    S, d, G, r, ro = lsqr_both(cfg, 25, 0.0, 0.0)
+    with G:
+        assert (r.istop, r.itn) == (ro.istop, ro.itn) == (7, 25)
+        assert rel(r.x.cpu().numpy(), ro.x) <= X_TOL
+        assert rel(r.se.cpu().numpy(), ro.se) <= 1e-8
+        for a, bb in ((r.rnorm, ro.rnorm), (r.anorm, ro.anorm), (r.acond, ro.acond), (r.xnorm, ro.xnorm)):
+            assert abs(a - bb) <= 1e-9 * abs(bb)
+    # to convergence: same stop code, itn within 2
+    S, d, G, r, ro = lsqr_both(cfg, 400, 1e-12, 1e-12)
+    with G:
+        assert r.istop == ro.istop and abs(r.itn - ro.itn) <= 2, (r.istop, r.itn, ro.istop, ro.itn)
+        assert rel(r.x.cpu().numpy(), ro.x) <= 1e-8
+
+
+def test_model_variants_global_columns_bit_reproducible():
+    """Every global column is reduced in a fixed order (warp -> CTA -> one block), as gamma is in production."""
+    cfg = variant_cfg((3, 12, 4, 5), "multi_cta")
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    with make_gpu(S, d, b) as G:
+        y = torch.from_numpy(np.random.default_rng(0).standard_normal(S.m_tot)).cuda()
+        outs = [G.gsr_aprod2(y, torch.zeros(S.n, dtype=torch.float64, device="cuda")).cpu().numpy() for _ in range(3)]
+        na = 3 * cfg.n_stars
+        for o in outs[1:]:
+            assert np.array_equal(o[:na], outs[0][:na])
+            assert np.array_equal(o[-5:], outs[0][-5:])
+
+
+def test_layout_width_validation():
+    gsr = gsr_mod()
+    for bad in ((6, 12, 6, 1), (5, 8, 6, 1), (5, 12, 7, 1), (5, 12, 6, 17), (0, 0, 0, 0), (-1, 12, 6, 1)):
+        with pytest.raises(gsr.GsrError) as e:
+            gsr.Gsr(10, 2, 8, 8, n_astro_par=bad[0], n_att_par=bad[1], n_instr_par=bad[2], n_glob=bad[3])
+        assert e.value.code == gsr.GSR_EINVAL
