@@ -52,6 +52,8 @@ def kernel_row_bytes(path_info, gsr):
         "k_aprod2_att_linear": 96 + 4 + 8,                       # attT + start + uT
         "k_u_to_time": 4 + 8 + 8,                                # permutation + gathered u + uT written
         "k_aprod2_fused": 192 + ic + 4 + star + 8 + 8,           # whole row ONCE, u read + written
+        "k_aprod2_noins": 40 + 8 + star + 8,                     # astro + gamma coefficients only (instr by k_ins_scatter)
+        "k_ins_scatter": 6 * (8 + 4) + 8,                        # column-ordered copy: value + (column, row) word; u staged once
     }
 
 
@@ -330,7 +332,14 @@ def main_ours(args):
     ms1 = timed_kernel(gsr.GSR_TIME_K_APROD1)
     k["k_aprod1"] = entry(ms1, rb["k_aprod1"])
     ms2 = timed_kernel(gsr.GSR_TIME_K_APROD2_MAIN)
-    k["k_aprod2"] = entry(ms2, rb["k_aprod2"] if att_copy else rb["k_aprod2_redatt"], 8 * G.n)
+    ins_copy = bool(info & gsr.GSR_PATH_INS_COPY)
+    k["k_aprod2"] = entry(ms2, (rb["k_aprod2_noins"] if ins_copy else rb["k_aprod2"]) if att_copy else rb["k_aprod2_redatt"], 8 * G.n)
+    if ins_copy:
+        k["k_aprod2"]["form"] = "astro + gamma only; the instrumental section runs in k_ins_scatter"
+        k["k_ins_scatter"] = entry(timed_kernel(gsr.GSR_TIME_K_INS_SCATTER), rb["k_ins_scatter"])
+    msut = timed_kernel(gsr.GSR_TIME_K_U_TO_TIME) if (info & gsr.GSR_PATH_UT) else None
+    if msut is not None:
+        k["k_u_to_time"] = entry(msut, rb["k_u_to_time"])
     ms2a = timed_kernel(gsr.GSR_TIME_K_APROD2_ATT) if att_copy else None
     att_linear = bool(info & gsr.GSR_PATH_UT)
     if ms2a is not None:
@@ -341,8 +350,8 @@ def main_ours(args):
         k["k_aprod2_fused"] = entry(msf, rb["k_aprod2_fused"])
     ms1g = G.gsr_time_aprod(gsr.GSR_TIME_APROD1_GROUP, reps)
     ms2g = G.gsr_time_aprod(gsr.GSR_TIME_APROD2_GROUP, reps)
-    in_step = ["k_aprod2_fused", "k_aprod2_att"] if msf is not None else \
-              ["k_aprod1", "k_aprod2"] + (["k_aprod2_att"] if ms2a is not None else [])
+    in_step = ["k_aprod2_fused", "k_aprod2_att"] + (["k_ins_scatter"] if ins_copy else []) + (["k_u_to_time"] if msut is not None else []) \
+        if msf is not None else ["k_aprod1", "k_aprod2"] + (["k_aprod2_att"] if ms2a is not None else []) + (["k_ins_scatter"] if ins_copy else [])
     dom = max(in_step, key=lambda n: k[n]["ms"])
     # north-star figures on the METHOD's bytes (two products of 248 + 240 B/row)
     gb1 = ROW_BYTES_APROD1 * m / 1e9
@@ -351,8 +360,10 @@ def main_ours(args):
     # bytes the timed step actually has to stream with the device layout
     if msf is not None:
         moved = rb["k_aprod2_fused"] + (rb["k_aprod2_att_linear"] + rb["k_u_to_time"] if att_linear else rb["k_aprod2_att"])
+        moved += rb["k_ins_scatter"] if ins_copy else 0
     else:
-        moved = rb["k_aprod1"] + (rb["k_aprod2"] + rb["k_aprod2_att"] if att_copy else rb["k_aprod2_redatt"])
+        moved = rb["k_aprod1"] + ((rb["k_aprod2_noins"] + rb["k_ins_scatter"] if ins_copy else rb["k_aprod2"]) + rb["k_aprod2_att"]
+                                  if att_copy else rb["k_aprod2_redatt"])
     moved_gb = (moved * m + 12 * 8 * G.n) / 1e9
     traffic, traffic_src = None, None      # ncu-measured DRAM bytes per launch of the dominant kernel
     tpath = os.path.join(ROOT, "profiles", "r02_traffic.csv")

@@ -99,6 +99,13 @@ typedef struct {
 #define GSR_FLAG_NO_FUSE 2u     /* gsr_lsqr runs the two-product iteration (aprod1,
                                    then aprod2, as Alg. 1 l.17-25) instead of the
                                    fused single pass over A                            */
+#define GSR_FLAG_INS_COPY 8u    /* build a column-ordered copy of the instrumental section
+                                   (+72 B/row of HBM) and sum that section of A^T y on it
+                                   without atomics (k_ins_scatter): bit-reproducible, but
+                                   measured SLOWER than the default shared-memory / global
+                                   atomics (Medium: 23.6 vs 21.3 ms per iteration), hence
+                                   opt-in.  Needs the attitude copy, n_instr <= 65536 and
+                                   unskewed columns; silently not built otherwise           */
 #define GSR_FLAG_NO_TEX 4u      /* fused pass: gather the unknowns with plain loads
                                    instead of texture fetches (the path taken anyway
                                    when n >= 2^27 texels)                              */
@@ -225,6 +232,9 @@ int32_t gsr_get_trace(gsr_handle *h, double *out, int64_t max_itn, int64_t *n_wr
 #define GSR_PATH_TEX 8
 #define GSR_PATH_IC16 16
 #define GSR_PATH_UT 32
+#define GSR_PATH_INS_COPY 64 /* column-ordered copy of the instrumental section in use
+                                (GSR_FLAG_INS_COPY): that section of A^T y is summed without
+                                atomics and is bit-reproducible                               */
 int32_t gsr_path_info(const gsr_handle *h);
 
 /* Device time of the last gsr_lsqr's iteration loop in milliseconds (CUDA events on

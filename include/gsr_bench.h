@@ -19,6 +19,8 @@ typedef enum {
     GSR_TIME_K_APROD1 = 11,     /* k_aprod1 alone                                                       */
     GSR_TIME_K_APROD2_MAIN = 12,/* k_aprod2 (astro / instr / gamma scatter) alone                       */
     GSR_TIME_K_APROD2_ATT = 13, /* k_aprod2_att alone (GSR_ESTATE without the attitude copy)            */
+    GSR_TIME_K_INS_SCATTER = 14,/* k_ins_scatter alone (GSR_ESTATE without the instrument copy)         */
+    GSR_TIME_K_U_TO_TIME = 15,  /* k_u_to_time alone (GSR_ESTATE when u is not kept in block-time order) */
     GSR_TIME_K_FUSED = 21       /* the fused pass of gsr_lsqr alone: aprod1 + the astro/instr/gamma
                                    scatter of aprod2 on one read of A (GSR_ESTATE if not in use)        */
 } gsr_time_which;

@@ -55,6 +55,13 @@ struct gsr_handle {
     int nRep = 1, gridAtt = 1, perIter = 0, nInsSm = 0;
     bool useAttT = false;
     bool instrSkewed = false;   // some instrument column holds > 64x the mean number of coefficients
+    // column-ordered copy of the instrumental section (k_ins_scatter): +72 B/row; built by gsr_upload_finish when it fits
+    double *insVal = nullptr;
+    uint32_t *insMeta = nullptr;
+    int64_t *insPtr = nullptr;
+    int insNB = 1, insW = 1, insNG = 1;   // column buckets, columns per bucket, CTAs per bucket
+    bool useInsT = false;
+    bool fusedNoPriv = false;   // bench knob: fused pass without the shared-memory instrument table (REDs only), 256 threads x 2 CTAs per SM
     Scalars *S = nullptr;
     Scalars *hostS = nullptr;           // pinned, 2 slots
     unsigned long long *badDev = nullptr;
@@ -113,7 +120,9 @@ MatView view(const gsr_handle *h)
     A.n = h->n;
     A.conRp = h->conRp; A.conCol = h->conCol; A.conVal = h->conVal; A.nCon = h->L.n_con;
     A.attT = h->useAttT ? h->attT : nullptr; A.sT = h->sT; A.permT = h->permT;
-    A.insRep = h->insRep; A.nRep = h->nRep; A.nInsSm = h->nInsSm;
+    A.insRep = h->insRep; A.nRep = h->useInsT ? h->insNG : h->nRep; A.nInsSm = h->nInsSm;
+    A.insVal = h->useInsT ? h->insVal : nullptr; A.insMeta = h->insMeta; A.insPtr = h->insPtr;
+    A.insNB = h->insNB; A.insW = h->insW;
     return A;
 }
 
@@ -184,6 +193,73 @@ int buildAttT(gsr_handle *h)
         cudaGetLastError();
         return fail(h, e == cudaErrorMemoryAllocation ? GSR_ENOMEM : GSR_ECUDA, "time-ordered attitude copy: %s",
                     cudaGetErrorString(e));
+    }
+    return GSR_OK;
+}
+
+
+// Column-ordered copy of the instrumental section (setup; see k_ins_scatter).  Opt-in
+// (GSR_FLAG_INS_COPY: it makes that section bit-reproducible but the iteration slower); taken when the layout
+// is the production one with the attitude copy and 2-byte columns, the columns are not skewed (the MATCH path serves
+// those), and it fits beside everything else with 2 GB to spare.  Rows are sorted
+// in slabs of 2^22 (cub keys-only radix sort: a library primitive used once per upload).
+int buildInsT(gsr_handle *h)
+{
+    const int64_t m = h->L.n_obs;
+    for (void *q : {(void *)h->insVal, (void *)h->insMeta, (void *)h->insPtr})
+        if (q) cudaFree(q);
+    h->insVal = nullptr; h->insMeta = nullptr; h->insPtr = nullptr;
+    h->useInsT = false;
+    if (!h->prod || !h->useAttT || !h->ic16 || h->instrSkewed || !(h->L.flags & GSR_FLAG_INS_COPY) || m <= 0)
+        return GSR_OK;
+    const int64_t slabRows = int64_t(1) << 22, nBlocks = (m + INS_BLOCK - 1) >> INS_ROW_BITS;
+    const int64_t slabE = std::min(m, slabRows) * N_INSTR;
+    size_t freeB = 0, totB = 0;
+    CK(cudaMemGetInfo(&freeB, &totB));
+    const size_t need = size_t(m) * N_INSTR * 12 + size_t(nBlocks * h->insNB * INS_WARPS + 1) * 8 + size_t(slabE) * 24 + (size_t(64) << 20);
+    if (freeB < need + (size_t(2) << 30)) return GSR_OK;
+    unsigned long long *keyIn = nullptr, *keyOut = nullptr;
+    void *tmp = nullptr;
+    size_t tmpBytes = 0;
+    int endBit = INS_KEY_BLOCK;
+    while (endBit < 64 && (int64_t(1) << (endBit - INS_KEY_BLOCK)) <= nBlocks) ++endBit;
+    cudaError_t e = cub::DeviceRadixSort::SortKeys(nullptr, tmpBytes, keyIn, keyOut, slabE, 0, endBit, h->stream);
+    if (e == cudaSuccess) e = dalloc(&h->insVal, m * N_INSTR);
+    if (e == cudaSuccess) e = dalloc(&h->insMeta, m * N_INSTR);
+    if (e == cudaSuccess) e = dalloc(&h->insPtr, nBlocks * h->insNB * INS_WARPS + 1);
+    if (e == cudaSuccess) e = dalloc(&keyIn, slabE);
+    if (e == cudaSuccess) e = dalloc(&keyOut, slabE);
+    if (e == cudaSuccess) e = cudaMalloc(&tmp, std::max<size_t>(tmpBytes, 16));
+    h->useInsT = e == cudaSuccess;   // view() hands the copy to the kernels below
+    MatView A = view(h);
+    for (int64_t r0 = 0; e == cudaSuccess && r0 < m; r0 += slabRows) {
+        const int64_t cnt = std::min(slabRows, m - r0);
+        k_ins_keys<<<gridFor(cnt * N_INSTR, 256, h->smCount * 16), 256, 0, h->stream>>>(A, r0, cnt, keyIn);
+        e = cub::DeviceRadixSort::SortKeys(tmp, tmpBytes, keyIn, keyOut, cnt * N_INSTR, 0, endBit, h->stream);
+        if (e == cudaSuccess) {
+            k_ins_fill<<<gridFor(cnt * N_INSTR, 256, h->smCount * 16), 256, 0, h->stream>>>(A, r0 * N_INSTR, cnt * N_INSTR, keyOut,
+                                                                                         h->insMeta);
+            e = cudaGetLastError();
+        }
+    }
+    if (e == cudaSuccess) {
+        k_ins_ptr<<<gridFor(nBlocks * h->insNB * INS_WARPS + 1, 256, h->smCount * 16), 256, 0, h->stream>>>(A, h->insPtr);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
+    if (keyIn) cudaFree(keyIn);
+    if (keyOut) cudaFree(keyOut);
+    if (tmp) cudaFree(tmp);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        h->useInsT = false;
+        if (e == cudaErrorMemoryAllocation) {   // the copy is optional: go on without it
+            for (void *q : {(void *)h->insVal, (void *)h->insMeta, (void *)h->insPtr})
+                if (q) cudaFree(q);
+            h->insVal = nullptr; h->insMeta = nullptr; h->insPtr = nullptr;
+            return GSR_OK;
+        }
+        return fail(h, GSR_ECUDA, "column-ordered instrument copy: %s", cudaGetErrorString(e));
     }
     return GSR_OK;
 }
@@ -293,7 +369,7 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(dalloc(&h->carryFirst, h->nTiles * N_ASTRO));
     CK(dalloc(&h->carryLast, h->nTiles * N_ASTRO));
     CK(dalloc(&h->globPartial, int64_t(std::max(h->gridA2, h->gridA2m)) * std::max(h->nG, 1)));
-    CK(dalloc(&h->sqPartialU, std::max(h->gridA1, h->gridA2m) + h->gridCon));
+    CK(dalloc(&h->sqPartialU, std::max(std::max(h->gridA1, h->gridA2m), h->gridA2) + h->gridCon));
     CK(dalloc(&h->t, h->n));
     CK(dalloc(&h->coefRaw, 2));
     CK(dalloc(&h->sqPartialV, h->gridVec));
@@ -305,7 +381,14 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(dalloc(&h->S, 1));
     CK(dalloc(&h->badDev, 1));
     h->nRepAlloc = h->nRep;
-    CK(dalloc(&h->insRep, int64_t(h->nRep) * L->n_instr));
+    // k_ins_scatter: buckets of <= INS_BUCKET_MAX columns, two CTAs per SM shared out over the buckets; every CTA owns a
+    // slice of insRep
+    h->insNB = int(std::max<int64_t>(1, (L->n_instr + INS_BUCKET_MAX - 1) / INS_BUCKET_MAX));
+    h->insW = int(std::max<int64_t>(1, (L->n_instr + int64_t(h->insNB) * INS_WARPS - 1) / (int64_t(h->insNB) * INS_WARPS))) * INS_WARPS;
+    h->insNG = std::max(1, h->smCount / h->insNB);
+    CK(cudaFuncSetAttribute(k_ins_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                            int((h->insW + 2 * INS_BLOCK) * sizeof(double))));
+    CK(dalloc(&h->insRep, int64_t(std::max(h->nRep, h->insNG)) * L->n_instr));
     CK(dalloc(&h->u, h->mTot));
     CK(dalloc(&h->v, h->n));
     CK(dalloc(&h->w, h->n));
@@ -382,7 +465,7 @@ int32_t gsr_destroy(gsr_handle *h)
     void *ptrs[] = {h->V, h->b, h->conVal, h->p, h->star, h->iatt, h->stageI, h->rp, h->conRp, h->conCol, h->ic, h->ic16, h->tw,
                     h->u, h->v, h->w, h->z, h->var, h->carryFirst, h->carryLast, h->globPartial,
                     h->sqPartialU, h->sqPartialV, h->ddPartial, h->coefOne, h->coefTime, h->trace,
-                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC, h->xPack, h->t, h->coefRaw, h->uT};
+                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC, h->xPack, h->t, h->coefRaw, h->uT, h->insVal, h->insMeta, h->insPtr};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (h->hostS) cudaFreeHost(h->hostS);
@@ -519,6 +602,8 @@ int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail)
         CK(e);
         const double mean = double(A.m) * h->nI / double(std::max<int64_t>(h->L.n_instr, 1));
         h->instrSkewed = double(mx) > 64.0 * std::max(mean, 1.0);
+        int rcI = buildInsT(h);
+        if (rcI) return rcI;
         if (h->iterGraph) {   // the captured iteration names the kernel variant
             cudaGraphExecDestroy(h->iterGraph);
             h->iterGraph = nullptr;
@@ -636,6 +721,11 @@ void launchAprod2Main(gsr_handle *h, const MatView &A, const double *y, double *
     const size_t sm = size_t(A.nInsSm) * sizeof(double);
     const int g = h->gridA2m;
     cudaStream_t st = h->stream;
+    if (FUSE && h->fusedNoPriv && h->ic16 && !h->instrSkewed) {
+        k_aprod2<true, false, false, false, false, FUSE, FUSE, true><<<h->gridA2, THREADS, 0, st>>>(
+            A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done, F);
+        return;
+    }
 #define GSR_A2M(IC, MA)                                                                                          \
     k_aprod2<IC, false, false, true, MA, FUSE, FUSE><<<g, PRIV_THREADS, sm, st>>>(A, y, x, coef, h->carryFirst,    \
                                                                                  h->carryLast, h->globPartial, done, F)
@@ -645,6 +735,22 @@ void launchAprod2Main(gsr_handle *h, const MatView &A, const double *y, double *
         if (h->instrSkewed) GSR_A2M(false, true); else GSR_A2M(false, false);
     }
 #undef GSR_A2M
+}
+
+// astro / gamma (FUSE: and the whole of aprod1) with the instrumental section left to k_ins_scatter: no shared-memory
+// table, two CTAs of 256 threads per SM (grid gridA2)
+template <bool FUSE>
+void launchAprod2NoIns(gsr_handle *h, const MatView &A, const double *y, double *x, const double *coef, const int *done,
+                       const FuseArgs &F)
+{
+    k_aprod2<true, false, false, false, false, FUSE, FUSE, false><<<h->gridA2, THREADS, 0, h->stream>>>(
+        A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done, F);
+}
+
+// instrumental section of A^T y on the column-ordered copy; every CTA leaves its accumulators in its slice of insRep
+void launchInsScatter(gsr_handle *h, const MatView &A, const double *y, const double *coef, const int *done)
+{
+    k_ins_scatter<<<h->insNB * h->insNG, INS_THREADS, size_t(h->insW + 2 * INS_BLOCK) * sizeof(double), h->stream>>>(A, y, coef, done);
 }
 
 // y <- cy*y + cx*(A x); partials of sum y^2 go to sqPartial (or nowhere).  Returns #kernels.
@@ -674,13 +780,20 @@ int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef,
 {
     MatView A = view(h);
     int nk = 1;
+    const bool attRed = SQUARE || !h->useAttT;
+    const bool insT = !attRed && h->useInsT;   // instrumental section by k_ins_scatter (which fills insRep itself)
     k_pre_aprod2<<<h->gridVec, 256, 0, h->stream>>>(x, A.offAtt, A.n, coef, h->insRep,
-                                                    h->prod ? int64_t(h->nRep) * A.nInstr : 0, prescale ? 1 : 0, done);
+                                                    h->prod && !insT ? int64_t(h->nRep) * A.nInstr : 0, prescale ? 1 : 0, done);
     // attitude section: segmented reduction on the time-ordered copy when there is one; the
     // preconditioner pass (SQUARE) and the low-memory fallback scatter it with REDs in k_aprod2
-    const bool attRed = SQUARE || !h->useAttT;
     if (attRed) {
+        if (h->useInsT) A.nRep = h->nRep;   // this pass adds the instrumental section to the nRep replicas
         launchAprod2Red<SQUARE>(h, A, y, x, coef, done);
+    } else if (insT) {
+        launchAtt(h, A, y, x, coef, done);
+        launchAprod2NoIns<false>(h, A, y, x, coef, done, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0});
+        launchInsScatter(h, A, y, coef, done);
+        nk += 2;
     } else {
         launchAtt(h, A, y, x, coef, done);
         launchAprod2Main<false>(h, A, y, x, coef, done, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0});
@@ -688,7 +801,7 @@ int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef,
     }
     if (h->prod)
         k_astro_fixup<<<h->gridFix, 256, 0, h->stream>>>(A, x, coef, h->carryFirst, h->carryLast, h->globPartial,
-                                                         attRed ? h->gridA2 : h->gridA2m, done);
+                                                         attRed || insT ? h->gridA2 : h->gridA2m, done);
     else
         k_fixup_gen<<<h->gridFix, 256, 0, h->stream>>>(A, x, coef, h->carryFirst, h->carryLast, h->globPartial, h->gridA2, done);
     nk += 2;
@@ -717,12 +830,15 @@ int enqueueIterationFused(gsr_handle *h)
     k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, done);
     // t <- 0 (and the instrument replicas); then one star-ordered pass over A: u^ <- a1_cy*u^ + a1_cx*(A v^), sum u^2,
     // and the astro / instr / gamma sections of t = A^T u^ (unscaled)
-    k_pre_aprod2<<<h->gridVec, 256, 0, st>>>(h->t, 0, A.n, h->coefRaw, h->insRep, int64_t(h->nRep) * A.nInstr, 2, done);
+    const bool insT = h->useInsT;   // instrumental section of A^T u^ by k_ins_scatter, after u^ is complete
+    k_pre_aprod2<<<h->gridVec, 256, 0, st>>>(h->t, 0, A.n, h->coefRaw, h->insRep, insT ? 0 : int64_t(h->nRep) * A.nInstr, 2, done);
     FuseArgs F{h->v, h->u, &S->a1_cx, h->sqPartialU, h->xPack, h->texV, h->texPack};
-    launchAprod2Main<true>(h, A, h->u, h->t, h->coefRaw, done, F);
-    int nk = 10, npU = h->gridA2m;
+    if (insT) launchAprod2NoIns<true>(h, A, h->u, h->t, h->coefRaw, done, F);
+    else launchAprod2Main<true>(h, A, h->u, h->t, h->coefRaw, done, F);
+    const int gridMain = insT || (h->fusedNoPriv && h->ic16 && !h->instrSkewed) ? h->gridA2 : h->gridA2m;
+    int nk = insT ? 11 : 10, npU = gridMain;
     if (A.nCon > 0) {   // constraint rows: their part of u^ and of sum u^2, then (below) of t
-        k_con_aprod1<<<h->gridCon, 256, 0, st>>>(A, h->v, h->u, &S->a1_cx, h->sqPartialU + h->gridA2m, done);
+        k_con_aprod1<<<h->gridCon, 256, 0, st>>>(A, h->v, h->u, &S->a1_cx, h->sqPartialU + gridMain, done);
         npU += h->gridCon;
         nk += 2;
     }
@@ -732,8 +848,9 @@ int enqueueIterationFused(gsr_handle *h)
         launchAtt(h, A, h->uT, h->t, h->coefRaw, done, true);
         ++nk;
     } else launchAtt(h, A, h->u, h->t, h->coefRaw, done);
+    if (insT) launchInsScatter(h, A, h->u, h->coefRaw, done);
     k_astro_fixup<<<h->gridFix, 256, 0, st>>>(A, h->t, h->coefRaw, h->carryFirst, h->carryLast, h->globPartial,
-                                              h->gridA2m, done);
+                                              gridMain, done);
     // after the fix-up: it overwrites the astro entries of stars cut by a tile edge
     if (A.nCon > 0) k_con_aprod2<false><<<h->gridCon, 256, 0, st>>>(A, h->u, h->t, h->coefRaw, done);
     // v^ <- a2_cx*v^ + a2_cy*t  (= A^T u - beta v with the lazy scales), sum v^2
@@ -838,6 +955,8 @@ int32_t gsr_precondition(gsr_handle *h)
         k_scale_con_values<<<gridFor(h->L.n_con_nnz, 256, h->smCount * 16), 256, 0, h->stream>>>(A, h->L.n_con_nnz, h->p);
     if (h->useAttT)   // the time-ordered copy takes the same factors
         k_scale_attT<<<gridFor(A.m, 256, h->smCount * 16), 256, 0, h->stream>>>(A, h->p);
+    if (h->useInsT)   // and so does the column-ordered instrument copy
+        k_scale_ins<<<gridFor(A.m * N_INSTR, 256, h->smCount * 16), 256, 0, h->stream>>>(A, h->p);
     CK(cudaGetLastError());
     CK(cudaStreamSynchronize(h->stream));
     h->preconditioned = true;
@@ -984,6 +1103,7 @@ int32_t gsr_path_info(const gsr_handle *h)
     if (h->texV && h->texPack) r |= GSR_PATH_TEX;
     if (h->ic16) r |= GSR_PATH_IC16;
     if (canFuse(h) && h->useUT) r |= GSR_PATH_UT;
+    if (h->useInsT) r |= GSR_PATH_INS_COPY;
     return r;
 }
 
@@ -1002,6 +1122,8 @@ int32_t gsr_bench_set(gsr_handle *h, const char *key, int64_t value)
     if (k == "ins_sm_fused" && value >= 0 && value <= h->nInsSm) h->nInsSmFused = int(value);
     else if (k == "n_rep" && value >= 1 && value <= h->nRepAlloc) h->nRep = int(value);
     else if (k == "att_ctas_per_sm" && value >= 1 && value <= 16) h->gridAtt = gridFor(h->nTiles, 8, h->smCount * int(value));
+    else if (k == "fused_nopriv" && (value == 0 || value == 1)) h->fusedNoPriv = value != 0;
+    else if (k == "a2_ctas_per_sm" && value >= 1 && value <= 2) h->gridA2 = gridFor(h->nTiles, WARPS, h->smCount * int(value));
     else if (k == "use_ut" && (value == 0 || (value == 1 && h->uT))) h->useUT = value != 0;
     else if (k == "ut_ctas_per_sm" && value >= 1 && value <= 16) h->gridUT = gridFor(h->L.n_obs, 256, h->smCount * int(value));
     else return fail(h, GSR_EINVAL, "gsr_bench_set: unknown key or value out of range: %s = %lld", key, (long long)value);
@@ -1016,8 +1138,11 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
 {
     if (!h || !ms_per_launch || reps < 1) return GSR_EINVAL;
     if (which != GSR_TIME_APROD1_GROUP && which != GSR_TIME_APROD2_GROUP && which != GSR_TIME_K_APROD1 &&
-        which != GSR_TIME_K_APROD2_MAIN && which != GSR_TIME_K_APROD2_ATT && which != GSR_TIME_K_FUSED)
+        which != GSR_TIME_K_APROD2_MAIN && which != GSR_TIME_K_APROD2_ATT && which != GSR_TIME_K_FUSED &&
+        which != GSR_TIME_K_INS_SCATTER && which != GSR_TIME_K_U_TO_TIME)
         return fail(h, GSR_EINVAL, "which");
+    if (which == GSR_TIME_K_INS_SCATTER && !h->useInsT) return fail(h, GSR_ESTATE, "no column-ordered instrument copy on this handle");
+    if (which == GSR_TIME_K_U_TO_TIME && !(canFuse(h) && h->useUT)) return fail(h, GSR_ESTATE, "this handle does not keep u in block-time order");
     if (which == GSR_TIME_K_FUSED && !canFuse(h)) return fail(h, GSR_ESTATE, "this handle does not use the fused iteration");
     if (which == GSR_TIME_K_APROD2_ATT && !h->useAttT) return fail(h, GSR_ESTATE, "no time-ordered attitude copy on this handle");
     int rc = readyCheck(h);
@@ -1042,8 +1167,13 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
             MatView Af = A;
             Af.nInsSm = h->nInsSmFused;
             FuseArgs F{h->v, h->u, h->coefTime, h->sqPartialU, h->xPack, h->texV, h->texPack};
-            launchAprod2Main<true>(h, Af, h->u, h->t, h->coefRaw, nullptr, F);
+            if (h->useInsT) launchAprod2NoIns<true>(h, Af, h->u, h->t, h->coefRaw, nullptr, F);
+            else launchAprod2Main<true>(h, Af, h->u, h->t, h->coefRaw, nullptr, F);
         }
+        else if (which == GSR_TIME_K_INS_SCATTER) launchInsScatter(h, A, h->u, h->coefTime, nullptr);
+        else if (which == GSR_TIME_K_U_TO_TIME) k_u_to_time<<<h->gridUT, 256, 0, st>>>(h->u, h->permT, A.m, h->uT, nullptr);
+        else if (h->useInsT)
+            launchAprod2NoIns<false>(h, A, h->u, h->v, h->coefTime, nullptr, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0});
         else if (h->useAttT)
             launchAprod2Main<false>(h, A, h->u, h->v, h->coefTime, nullptr, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0});
         else

@@ -29,6 +29,10 @@ constexpr int TILE = 32;          // rows per warp tile
 constexpr int WARPS = 8;          // warps per CTA of the aprod kernels
 constexpr int THREADS = WARPS * 32;
 constexpr int ATT_BLOCK_BITS = 21;   // rows per block of the time-ordered attitude copy (2^21)
+constexpr int INS_ROW_BITS = 13;     // rows per block of the column-ordered instrument copy (2^13: the block's slice of y is 64 KB of shared memory)
+constexpr int INS_BLOCK = 1 << INS_ROW_BITS;
+constexpr int INS_KEY_COL = INS_ROW_BITS + 3, INS_KEY_BLOCK = INS_KEY_COL + 16;   // sort key of the build: block | column (16 bits) | row in block | slot (3 bits)
+constexpr int INS_BUCKET_MAX = 7680; // instrument columns per bucket: one bucket's accumulators are 60 KB of shared memory
 
 // Device layout of the coefficients ("tile-transposed"): the 32 rows of a warp tile are stored
 // coefficient-major, V[(tile*24 + k)*32 + lane], so that lane <-> row reads each of its 24
@@ -72,6 +76,15 @@ struct MatView {
     double *insRep;
     int nRep;
     int nInsSm;            // instrument columns [0, nInsSm) accumulate in shared memory (k_aprod2<.., PRIV>)
+    // column-ordered copy of the instrumental section (built at upload when memory allows; nullptr otherwise), for
+    // k_ins_scatter: the 6 coefficients of the rows of block b (INS_BLOCK consecutive rows) sorted by column, then row;
+    // insMeta[e] = column << INS_ROW_BITS | row inside the block; columns are cut into insNB buckets of insW (a multiple of
+    // INS_WARPS) and every bucket into INS_WARPS sub-buckets; insPtr[b*insNB*INS_WARPS + j]: first entry of sub-bucket j of
+    // block b
+    double *insVal;
+    const uint32_t *insMeta;
+    const int64_t *insPtr;
+    int insNB, insW;
 };
 
 // Scalars of the LSQR recurrences, resident in device memory.
@@ -132,14 +145,15 @@ __device__ __forceinline__ double block_sum(double v, double *red)
 
 // The 24 coefficients of row (tile, lane): coalesced streaming loads.  ATT: load the attitude
 // coefficients too (k = 5..16).
-template <bool ATT>
+template <bool ATT, bool INS = true>
 __device__ __forceinline__ void load_row(const double *__restrict__ V, int64_t tile, int lane, double (&v)[N_PAR])
 {
     const double *g = V + tile * (N_PAR * TILE) + lane;
 #pragma unroll
     for (int q = 0; q < N_PAR; ++q) {
-        if (ATT || q < N_ASTRO || q >= N_ASTRO + N_ATT) v[q] = __ldcs(g + q * TILE);
-        else v[q] = 0.0;
+        const bool att = q >= N_ASTRO && q < N_ASTRO + N_ATT, ins = q >= N_ASTRO + N_ATT && q < N_PAR - 1;
+        if ((att && !ATT) || (ins && !INS)) v[q] = 0.0;
+        else v[q] = __ldcs(g + q * TILE);
     }
 }
 
@@ -277,7 +291,11 @@ __device__ __forceinline__ double tex_f64(cudaTextureObject_t t, int64_t idx)
 }
 // FUSE_ATT: the attitude terms of A*xin are gathered here too, in star order (whole aprod1 in this pass,
 // y <- cy*y + cx*(A xin)); without it yrw must already hold cy*y + cx*(attitude terms).
-template <bool IC16, bool SQUARE, bool ATT_RED, bool PRIV = false, bool MATCH = false, bool FUSE = false, bool FUSE_ATT = false>
+// INS = false: the instrumental section is scattered by k_ins_scatter on the column-ordered copy instead (no atomics
+// here, no shared-memory table, two CTAs of 256 threads per SM); without FUSE its coefficients and columns are not
+// even loaded.
+template <bool IC16, bool SQUARE, bool ATT_RED, bool PRIV = false, bool MATCH = false, bool FUSE = false, bool FUSE_ATT = false,
+          bool INS = true>
 __global__ void __launch_bounds__(PRIV ? PRIV_THREADS : THREADS, PRIV ? 1 : 2)
 k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
          const double *__restrict__ coef, double *__restrict__ carryFirst,
@@ -310,12 +328,12 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         const bool valid = lane < nrows;
         const int64_t i = r0 + (valid ? lane : nrows - 1);
         double v[N_PAR];
-        load_row<ATT_RED || FUSE_ATT>(A.V, tile, valid ? lane : nrows - 1, v);
+        load_row<ATT_RED || FUSE_ATT, INS || FUSE>(A.V, tile, valid ? lane : nrows - 1, v);
         const unsigned long long tw = __ldg(A.tw + tile);   // one 8-byte word per tile: first star, head mask, cut flags
         const int64_t ia = 5 * star_of(A, tw, i, valid ? lane : nrows - 1);
         // padded storage: the lanes past the last row read column 0 and a zero coefficient
-        int32_t c[N_INSTR];
-        load_ic<IC16>(A, tile, lane, c);
+        int32_t c[N_INSTR] = {0, 0, 0, 0, 0, 0};
+        if (INS || FUSE) load_ic<IC16>(A, tile, lane, c);
         GSR_ASSERT(ia >= 0 && ia + N_ASTRO <= A.offAtt);
 #pragma unroll
         for (int j = 0; j < N_INSTR; ++j) GSR_ASSERT(c[j] >= 0 && c[j] < A.nInstr);
@@ -366,7 +384,7 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
 #pragma unroll
                 for (int j = 0; j < 4; ++j) atomicAdd(xt + a * A.nDof + j, v[5 + 4 * a + j]);
         }
-        {
+        if (INS) {
 #pragma unroll
             for (int j = 0; j < N_INSTR; ++j) {
                 // lanes of the warp that hit the same column (hot columns of a skewed distribution) are summed
@@ -592,6 +610,199 @@ k_aprod2_att(MatView A, const double *__restrict__ y, double *__restrict__ x,
             }
         }
     }
+}
+
+// ---------------------------------------------------------------------------------------
+// aprod2, instrumental section on the column-ordered copy (Alg. 3 instr; the paper uses one atomicAdd
+// per coefficient).  Rows are cut into blocks of INS_BLOCK and the 6 x INS_BLOCK coefficients of a block are sorted by
+// column; the columns are cut into insNB buckets of insW <= INS_BUCKET_MAX.  CTA (g, k) keeps the accumulators of
+// bucket k in shared memory for its whole life and walks the row blocks g, g + nG, ...: it stages the block's slice of
+// y through L1 (32 KB), streams the bucket's entries (12 bytes each, coalesced), multiplies with the gathered y, sums equal columns with a warp segmented scan (they are adjacent) and adds the sum to the
+// accumulator with a plain read-modify-write: a column whose entries lie inside one 32-entry chunk belongs to that
+// chunk alone; only the first and last column of a chunk can continue in a neighbour chunk and take a shared-memory
+// atomic.  (y: see the kernel; a first version staged the slice in shared memory behind two barriers per block and ran
+// at 1.1 TB/s, bound by the latency of those phases.)  No global atomics: every CTA writes its table to its own slice of insRep and k_astro_fixup folds the slices
+// in a fixed order.  The eight CTAs of a group read the same slice of y at about the same time (L2).
+// ---------------------------------------------------------------------------------------
+constexpr int INS_THREADS = 1024;    // k_ins_scatter: 32 warps, one CTA per SM
+constexpr int INS_WARPS = INS_THREADS / 32;   // a bucket is cut into INS_WARPS sub-buckets, one per warp
+constexpr int INS_UNROLL = 8;        // 32-entry chunks of a sub-bucket that a warp holds in registers
+// streaming loads that do not displace anything in L1
+__device__ __forceinline__ uint32_t ld_stream_u32(const uint32_t *p)
+{
+    uint32_t v;
+    asm volatile("ld.global.nc.L1::no_allocate.u32 %0, [%1];" : "=r"(v) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ double ld_stream_f64(const double *p)
+{
+    double v;
+    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
+    return v;
+}
+__global__ void __launch_bounds__(INS_THREADS, 1)
+k_ins_scatter(MatView A, const double *__restrict__ y, const double *__restrict__ coef, const int *done)
+{
+    extern __shared__ double sIns[];   // [insW] accumulators of this CTA's column bucket, then 2 x [INS_BLOCK] slices of y
+    if (done && *done) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int k = blockIdx.x % A.insNB, g = blockIdx.x / A.insNB, nG = gridDim.x / A.insNB;
+    if (g >= nG) return;
+    const int c0 = k * A.insW, w = max(0, min(A.insW, int(A.nInstr) - c0));
+    double *acc = sIns - c0;           // indexed by the column itself
+    double *ybuf = sIns + A.insW;
+    const double cy = coef[1];
+    for (int c = threadIdx.x; c < A.insW; c += INS_THREADS) sIns[c] = 0.0;
+    const int64_t nBlocks = (A.m + INS_BLOCK - 1) >> INS_ROW_BITS;
+    const int nSub = A.insNB * INS_WARPS;
+    const int64_t *ptr = A.insPtr + k * INS_WARPS + warp;   // + b*nSub: this warp's sub-bucket of block b
+
+    // the block's slice of y, copied to shared memory one block ahead (8-byte cp.async: no alignment demands on y)
+    auto stage = [&](int64_t b, int buf) {
+        if (b < nBlocks) {
+            const int64_t r0 = b << INS_ROW_BITS;
+            const int nr = int(min(int64_t(INS_BLOCK), A.m - r0));
+            const unsigned dst = unsigned(__cvta_generic_to_shared(ybuf + buf * INS_BLOCK));
+            for (int r = threadIdx.x; r < nr; r += INS_THREADS)
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst + 8u * r), "l"(y + r0 + r));
+        }
+        asm volatile("cp.async.commit_group;");
+    };
+    // one 32-entry chunk: sums of equal (adjacent) columns, then one plain read-modify-write per column: the columns of a
+    // sub-bucket belong to this warp alone
+    auto chunk = [&](uint32_t meta, double val, bool valid, const double *yb) {
+        const int col = int(meta >> INS_ROW_BITS);
+        GSR_ASSERT(!valid || (col >= c0 && col < c0 + w));
+        double s = valid ? val * (cy * yb[meta & (INS_BLOCK - 1)]) : 0.0;
+        // segmented inclusive scan by column, two fixed steps (runs of up to 4 equal columns); longer runs take more steps
+        // (every lane takes part in every shuffle: no shuffle on the right of a short-circuit operator)
+        const int up1 = __shfl_up_sync(0xffffffffu, col, 1), up2 = __shfl_up_sync(0xffffffffu, col, 2);
+        const int up4 = __shfl_up_sync(0xffffffffu, col, 4), dn1 = __shfl_down_sync(0xffffffffu, col, 1);
+        const bool p1 = lane >= 1 && col == up1;
+        const bool p2 = lane >= 2 && col == up2;
+        const bool tail = valid && (lane == 31 || col != dn1);
+        double t = __shfl_up_sync(0xffffffffu, s, 1);
+        if (p1) s += t;
+        t = __shfl_up_sync(0xffffffffu, s, 2);
+        if (p2) s += t;
+        if (__any_sync(0xffffffffu, lane >= 4 && col == up4)) {
+            for (int d = 4; d < 32; d <<= 1) {
+                const int upd = __shfl_up_sync(0xffffffffu, col, d);
+                t = __shfl_up_sync(0xffffffffu, s, d);
+                if (lane >= d && col == upd) s += t;
+            }
+        }
+        if (tail) acc[col] += s;
+        __syncwarp();   // a column that goes on in the next chunk is read-modify-written again by another lane
+    };
+
+    // The first INS_UNROLL chunks of the sub-bucket live in registers and are loaded one block ahead: chunk q of the next
+    // block is requested as soon as chunk q of this block is done (more than INS_UNROLL chunks is rare; the rest is loaded
+    // when its turn comes).
+    uint32_t meta[INS_UNROLL];
+    double val[INS_UNROLL];
+    int64_t e0 = 0;
+    int cnt = 0;
+    if (g < nBlocks) {
+        e0 = __ldg(ptr + int64_t(g) * nSub);
+        cnt = int(__ldg(ptr + int64_t(g) * nSub + 1) - e0);
+    }
+    {
+        const uint32_t *mp = A.insMeta + e0 + lane;
+        const double *vp = A.insVal + e0 + lane;
+#pragma unroll
+        for (int q = 0; q < INS_UNROLL; ++q) {
+            const bool valid = q * 32 + lane < cnt;
+            meta[q] = valid ? ld_stream_u32(mp + q * 32) : (0xffffffffu - lane);   // past the end: distinct columns
+            val[q] = valid ? ld_stream_f64(vp + q * 32) : 0.0;
+        }
+    }
+    stage(g, 0);
+    int buf = 0;
+    for (int64_t b = g; b < nBlocks; b += nG, buf ^= 1) {
+        int64_t e0n = 0;
+        int cntn = 0;
+        if (b + nG < nBlocks) {
+            e0n = __ldg(ptr + (b + nG) * nSub);
+            cntn = int(__ldg(ptr + (b + nG) * nSub + 1) - e0n);
+        }
+        asm volatile("cp.async.wait_group 0;");
+        __syncthreads();   // this block's slice of y has landed, and every warp is done with the other buffer
+        stage(b + nG, buf ^ 1);
+        const double *yb = ybuf + buf * INS_BLOCK;
+        const uint32_t *mp = A.insMeta + e0n + lane;
+        const double *vp = A.insVal + e0n + lane;
+#pragma unroll
+        for (int q = 0; q < INS_UNROLL; ++q) {
+            if (q * 32 < cnt) chunk(meta[q], val[q], q * 32 + lane < cnt, yb);   // warp-uniform condition
+            const bool valid = q * 32 + lane < cntn;
+            meta[q] = valid ? ld_stream_u32(mp + q * 32) : (0xffffffffu - lane);
+            val[q] = valid ? ld_stream_f64(vp + q * 32) : 0.0;
+        }
+        for (int o = 32 * INS_UNROLL; o < cnt; o += 32) {   // overflow of the register window
+            const bool valid = o + lane < cnt;
+            const uint32_t mt = valid ? ld_stream_u32(A.insMeta + e0 + o + lane) : (0xffffffffu - lane);
+            const double vl = valid ? ld_stream_f64(A.insVal + e0 + o + lane) : 0.0;
+            chunk(mt, vl, valid, yb);
+        }
+        e0 = e0n;
+        cnt = cntn;
+    }
+    asm volatile("cp.async.wait_group 0;");
+    __syncthreads();
+    double *out = A.insRep + int64_t(g) * A.nInstr + c0;
+    for (int c = threadIdx.x; c < w; c += INS_THREADS) out[c] = sIns[c];
+}
+
+// Build of the column-ordered copy (setup).  key = block << INS_KEY_BLOCK | column << INS_KEY_COL | row in block << 3 | slot for the 6
+// coefficients of rows [row0, row0 + cnt); a keys-only radix sort (cub) orders them; k_ins_fill turns the sorted keys
+// into insMeta / insVal; k_ins_ptr finds the first entry of every (block, bucket).
+__global__ void k_ins_keys(MatView A, int64_t row0, int64_t cnt, unsigned long long *__restrict__ key)
+{
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < cnt * N_INSTR; q += int64_t(gridDim.x) * blockDim.x) {
+        const int64_t i = row0 + q / N_INSTR;
+        const int j = int(q % N_INSTR);
+        const unsigned long long col = (unsigned long long)ic_at(A, cpos(i, j));
+        key[q] = ((unsigned long long)(i >> INS_ROW_BITS) << INS_KEY_BLOCK) | (col << INS_KEY_COL) | ((unsigned long long)(i & (INS_BLOCK - 1)) << 3) |
+                 (unsigned long long)j;
+    }
+}
+__global__ void k_ins_fill(MatView A, int64_t e0, int64_t cnt, const unsigned long long *__restrict__ key,
+                           uint32_t *__restrict__ meta)
+{
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < cnt; q += int64_t(gridDim.x) * blockDim.x) {
+        const unsigned long long kk = key[q];
+        const int64_t i = (int64_t(kk >> INS_KEY_BLOCK) << INS_ROW_BITS) | int64_t((kk >> 3) & (INS_BLOCK - 1));
+        meta[e0 + q] = (uint32_t((kk >> INS_KEY_COL) & 0xffffu) << INS_ROW_BITS) | uint32_t((kk >> 3) & (INS_BLOCK - 1));
+        A.insVal[e0 + q] = A.V[vpos(i, N_ASTRO + N_ATT + int(kk & 7))];
+    }
+}
+// insPtr[b*nSub + j] = first entry e of block b with column >= j*(insW/INS_WARPS), nSub = insNB*INS_WARPS sub-buckets
+// (entries of block b start at 6*b*INS_BLOCK)
+__global__ void k_ins_ptr(MatView A, int64_t *__restrict__ ptr)
+{
+    const int64_t nBlocks = (A.m + INS_BLOCK - 1) >> INS_ROW_BITS;
+    const int nSub = A.insNB * INS_WARPS, ws = A.insW / INS_WARPS;
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q <= nBlocks * nSub; q += int64_t(gridDim.x) * blockDim.x) {
+        if (q == nBlocks * nSub) {
+            ptr[q] = A.m * N_INSTR;
+            continue;
+        }
+        const int64_t b = q / nSub;
+        const uint32_t colLo = uint32_t(q % nSub) * uint32_t(ws);
+        int64_t lo = b * (int64_t(INS_BLOCK) * N_INSTR), hi = min(A.m, (b + 1) << INS_ROW_BITS) * N_INSTR;
+        while (lo < hi) {
+            const int64_t mid = (lo + hi) >> 1;
+            if ((A.insMeta[mid] >> INS_ROW_BITS) < colLo) lo = mid + 1; else hi = mid;
+        }
+        ptr[q] = lo;
+    }
+}
+// After the preconditioner: the copy takes the same factors as the row layout (same operands, bit-identical values)
+__global__ void k_scale_ins(MatView A, const double *__restrict__ p)
+{
+    for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < A.m * N_INSTR; e += int64_t(gridDim.x) * blockDim.x)
+        A.insVal[e] = A.insVal[e] * p[A.offInstr + (A.insMeta[e] >> INS_ROW_BITS)];
 }
 
 // ---------------------------------------------------------------------------------------

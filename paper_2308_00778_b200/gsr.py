@@ -20,12 +20,13 @@ LIB_PATH = os.environ.get("GSR_LIBRARY") or os.path.join(_PKG, "libgsr.so")
 GSR_OK, GSR_EINVAL, GSR_EINDEX, GSR_ENOMEM, GSR_ECUDA, GSR_ESTATE = 0, -1, -2, -3, -4, -5
 TRACE_CAP = 4096
 # gsr_layout.flags (include/gsr.h)
-GSR_FLAG_NO_ATT_COPY, GSR_FLAG_NO_FUSE, GSR_FLAG_NO_TEX = 1, 2, 4
+GSR_FLAG_NO_ATT_COPY, GSR_FLAG_NO_FUSE, GSR_FLAG_NO_TEX, GSR_FLAG_INS_COPY = 1, 2, 4, 8
 # gsr_path_info bits
-GSR_PATH_ATT_COPY, GSR_PATH_FUSED, GSR_PATH_INSTR_MATCH, GSR_PATH_TEX, GSR_PATH_IC16, GSR_PATH_UT = 1, 2, 4, 8, 16, 32
+GSR_PATH_ATT_COPY, GSR_PATH_FUSED, GSR_PATH_INSTR_MATCH, GSR_PATH_TEX, GSR_PATH_IC16, GSR_PATH_UT, GSR_PATH_INS_COPY = 1, 2, 4, 8, 16, 32, 64
 # gsr_time_aprod selectors (include/gsr_bench.h)
 GSR_TIME_APROD1_GROUP, GSR_TIME_APROD2_GROUP = 1, 2
 GSR_TIME_K_APROD1, GSR_TIME_K_APROD2_MAIN, GSR_TIME_K_APROD2_ATT, GSR_TIME_K_FUSED = 11, 12, 13, 21
+GSR_TIME_K_INS_SCATTER, GSR_TIME_K_U_TO_TIME = 14, 15
 
 # every symbol include/gsr.h declares (tests check that the library exports each one)
 SYMBOLS = [

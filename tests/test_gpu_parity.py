@@ -156,6 +156,14 @@ def test_astro_and_gamma_are_bit_reproducible():
         for o in outs[1:]:
             assert np.array_equal(o[:na], outs[0][:na])
             assert o[-1] == outs[0][-1]
+    # with the column-ordered instrument copy (opt-in) that section is summed without atomics, in a fixed order too
+    with make_gpu(S, d, b, flags=gsr_mod().GSR_FLAG_INS_COPY) as G:
+        assert G.gsr_path_info() & gsr_mod().GSR_PATH_INS_COPY
+        outs = [G.gsr_aprod2(y, torch.zeros(S.n, dtype=torch.float64, device="cuda")).cpu().numpy() for _ in range(3)]
+        oi = 5 * cfg.n_stars + 3 * cfg.n_dof_att
+        for o in outs[1:]:
+            assert np.array_equal(o[:na], outs[0][:na])
+            assert np.array_equal(o[oi:], outs[0][oi:])
 
 
 @pytest.mark.parametrize("name", ["mini_con", "ragged_tail", "powerlaw"])
@@ -338,14 +346,18 @@ def test_chunked_device_upload_equals_whole_upload():
         check_aprods(S, G)
 
 
-def test_two_attitude_blocks_and_mixed_instrument_table():
-    """2.2 M rows: more than one 2^21-row block of the block-time-ordered attitude copy, and 30,000 instrument
-    columns: more than the per-CTA shared-memory table holds, so both the ATOMS and the RED path run."""
+@pytest.mark.parametrize("ins_copy", [True, False])
+def test_two_attitude_blocks_and_mixed_instrument_table(ins_copy):
+    """2.2 M rows: more than one 2^21-row block of the block-time-ordered attitude copy, 269 row blocks of the
+    column-ordered instrument copy (opt-in, the last one ragged), and 30,000 instrument columns: four column buckets for
+    k_ins_scatter; without that copy more than the per-CTA shared-memory table holds, so both the ATOMS and the RED
+    path run."""
     cfg = synth.SynthConfig("blocks2", 22_000, 4_000, 30_000, obs_per_star=100, seed=11)
     S, d = oracle_system(cfg)
     assert S.m > (1 << 21)
     b = make_b(S, d)
-    with make_gpu(S, d, b) as G:
+    with make_gpu(S, d, b, flags=gsr_mod().GSR_FLAG_INS_COPY if ins_copy else 0) as G:
+        assert bool(G.gsr_path_info() & gsr_mod().GSR_PATH_INS_COPY) == ins_copy
         check_aprods(S, G)
         v, _ = G.gsr_get_values()
         assert np.array_equal(v.cpu().numpy(), d["values"])                     # layout round trip, bit-exact
@@ -583,7 +595,7 @@ def test_reupload_with_constraints_is_clean():
         assert rel(x2, S.lsqr(b, 20, 0.0, 0.0).x) <= X_TOL
 
 
-@pytest.mark.parametrize("flag", ["NO_ATT_COPY", "NO_FUSE", "NO_TEX"])
+@pytest.mark.parametrize("flag", ["NO_ATT_COPY", "NO_FUSE", "NO_TEX", "INS_COPY", "INS_COPY+NO_FUSE"])
 @pytest.mark.parametrize("case", ["mini_con", "zipf_hot", "ragged_tail"])
 def test_fallback_paths(flag, case):
     """gsr_layout.flags, per handle and in-process: the low-memory path (no block-time-ordered attitude copy:
@@ -591,16 +603,19 @@ def test_fallback_paths(flag, case):
     layout, and the fused pass without texture objects (the path systems with n >= 2^27 take) all give the
     oracle's results."""
     gsr = gsr_mod()
-    fl = {"NO_ATT_COPY": gsr.GSR_FLAG_NO_ATT_COPY, "NO_FUSE": gsr.GSR_FLAG_NO_FUSE, "NO_TEX": gsr.GSR_FLAG_NO_TEX}[flag]
+    fl = {"NO_ATT_COPY": gsr.GSR_FLAG_NO_ATT_COPY, "NO_FUSE": gsr.GSR_FLAG_NO_FUSE, "NO_TEX": gsr.GSR_FLAG_NO_TEX,
+          "INS_COPY": gsr.GSR_FLAG_INS_COPY, "INS_COPY+NO_FUSE": gsr.GSR_FLAG_INS_COPY | gsr.GSR_FLAG_NO_FUSE}[flag]
     cfg = CASES[case]["cfg"]
     S, d = oracle_system(cfg)
     b = make_b(S, d)
     with make_gpu(S, d, b, flags=fl) as G:
         info = G.gsr_path_info()
         assert bool(info & gsr.GSR_PATH_ATT_COPY) == (flag != "NO_ATT_COPY")
-        assert bool(info & gsr.GSR_PATH_FUSED) == (flag == "NO_TEX")
+        assert bool(info & gsr.GSR_PATH_FUSED) == (flag in ("NO_TEX", "INS_COPY"))
         assert bool(info & gsr.GSR_PATH_TEX) == (flag != "NO_TEX")
         assert bool(info & gsr.GSR_PATH_INSTR_MATCH) == (case == "zipf_hot")
+        # the column-ordered instrument copy is opt-in and needs unskewed columns
+        assert bool(info & gsr.GSR_PATH_INS_COPY) == (flag.startswith("INS_COPY") and case != "zipf_hot")
         check_aprods(S, G)
         G.gsr_precondition()
         S.precondition()
@@ -613,9 +628,12 @@ def test_fallback_paths(flag, case):
         if flag == "NO_ATT_COPY":
             with pytest.raises(gsr.GsrError):
                 G.gsr_time_aprod(gsr.GSR_TIME_K_APROD2_ATT, 1)
-        if flag != "NO_TEX":
+        if flag not in ("NO_TEX", "INS_COPY"):
             with pytest.raises(gsr.GsrError):
                 G.gsr_time_aprod(gsr.GSR_TIME_K_FUSED, 1)
+        if not (info & gsr.GSR_PATH_INS_COPY):
+            with pytest.raises(gsr.GsrError):
+                G.gsr_time_aprod(gsr.GSR_TIME_K_INS_SCATTER, 1)
 
 
 # ----------------------------------------------------------------------------- model variants
