@@ -21,6 +21,8 @@ typedef enum {
     GSR_TIME_K_APROD2_ATT = 13, /* k_aprod2_att alone (GSR_ESTATE without the attitude copy)            */
     GSR_TIME_K_INS_SCATTER = 14,/* k_ins_scatter alone (GSR_ESTATE without the instrument copy)         */
     GSR_TIME_K_U_TO_TIME = 15,  /* k_u_to_time alone (GSR_ESTATE when u is not kept in block-time order) */
+    GSR_TIME_OVERLAP_PROBE = 31,/* probe: the fused pass on one stream, k_u_to_time + k_aprod2_att on a second one,
+                                   no dependency between them (time per repetition of the three)         */
     GSR_TIME_K_FUSED = 21       /* the fused pass of gsr_lsqr alone: aprod1 + the astro/instr/gamma
                                    scatter of aprod2 on one read of A (GSR_ESTATE if not in use)        */
 } gsr_time_which;

@@ -25,6 +25,8 @@ struct gsr_handle {
     bool prod = true;   // 5/12/6/1: the specialised kernels; any other layout runs k_aprod1_gen / k_aprod2_gen
     cudaStream_t stream = nullptr;
     cudaStream_t userStream = nullptr;
+    cudaStream_t stream2 = nullptr;   // second stream of the overlap probe (gsr_time_aprod)
+    cudaEvent_t evFork = nullptr, evJoin = nullptr;
     int smCount = 148;
     // system
     double *V = nullptr, *b = nullptr, *conVal = nullptr, *p = nullptr;
@@ -473,6 +475,9 @@ int32_t gsr_destroy(gsr_handle *h)
     if (h->ev1) cudaEventDestroy(h->ev1);
     for (auto &e : h->evSlot)
         if (e) cudaEventDestroy(e);
+    if (h->stream2) cudaStreamDestroy(h->stream2);
+    if (h->evFork) cudaEventDestroy(h->evFork);
+    if (h->evJoin) cudaEventDestroy(h->evJoin);
     if (h->stream) cudaStreamDestroy(h->stream);
     cudaGetLastError();
     delete h;
@@ -1139,8 +1144,9 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
     if (!h || !ms_per_launch || reps < 1) return GSR_EINVAL;
     if (which != GSR_TIME_APROD1_GROUP && which != GSR_TIME_APROD2_GROUP && which != GSR_TIME_K_APROD1 &&
         which != GSR_TIME_K_APROD2_MAIN && which != GSR_TIME_K_APROD2_ATT && which != GSR_TIME_K_FUSED &&
-        which != GSR_TIME_K_INS_SCATTER && which != GSR_TIME_K_U_TO_TIME)
+        which != GSR_TIME_K_INS_SCATTER && which != GSR_TIME_K_U_TO_TIME && which != GSR_TIME_OVERLAP_PROBE)
         return fail(h, GSR_EINVAL, "which");
+    if (which == GSR_TIME_OVERLAP_PROBE && !(canFuse(h) && h->useUT)) return fail(h, GSR_ESTATE, "overlap probe needs the fused iteration with u in block-time order");
     if (which == GSR_TIME_K_INS_SCATTER && !h->useInsT) return fail(h, GSR_ESTATE, "no column-ordered instrument copy on this handle");
     if (which == GSR_TIME_K_U_TO_TIME && !(canFuse(h) && h->useUT)) return fail(h, GSR_ESTATE, "this handle does not keep u in block-time order");
     if (which == GSR_TIME_K_FUSED && !canFuse(h)) return fail(h, GSR_ESTATE, "this handle does not use the fused iteration");
@@ -1179,6 +1185,37 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
         else
             launchAprod2Red<false>(h, A, h->u, h->v, h->coefTime, nullptr);
     };
+    if (which == GSR_TIME_OVERLAP_PROBE) {
+        // Probe, not a product path: the fused pass on one stream and k_u_to_time + k_aprod2_att on another, with no
+        // dependency between them (the numbers they produce are not used): how much of the attitude part could hide under
+        // the fused pass if the iteration were cut into row segments?
+        if (!h->stream2) {
+            CK(cudaStreamCreateWithFlags(&h->stream2, cudaStreamNonBlocking));
+            CK(cudaEventCreateWithFlags(&h->evFork, cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&h->evJoin, cudaEventDisableTiming));
+        }
+        MatView Af = A;
+        Af.nInsSm = h->nInsSmFused;
+        FuseArgs F{h->v, h->u, h->coefTime, h->sqPartialU, h->xPack, h->texV, h->texPack};
+        CK(cudaStreamSynchronize(st));
+        CK(cudaEventRecord(h->ev0, st));
+        CK(cudaEventRecord(h->evFork, st));
+        CK(cudaStreamWaitEvent(h->stream2, h->evFork, 0));
+        for (int r = 0; r < reps; ++r) {
+            launchAprod2Main<true>(h, Af, h->u, h->t, h->coefRaw, nullptr, F);
+            k_u_to_time<<<h->gridUT, 256, 0, h->stream2>>>(h->u, h->permT, A.m, h->uT, nullptr);
+            k_aprod2_att<false, true><<<h->gridAtt, 256, 0, h->stream2>>>(A, h->uT, h->v, h->coefTime, nullptr);
+        }
+        CK(cudaEventRecord(h->evJoin, h->stream2));
+        CK(cudaStreamWaitEvent(st, h->evJoin, 0));
+        CK(cudaEventRecord(h->ev1, st));
+        CK(cudaGetLastError());
+        CK(cudaStreamSynchronize(st));
+        float msO = 0.f;
+        CK(cudaEventElapsedTime(&msO, h->ev0, h->ev1));
+        *ms_per_launch = double(msO) / reps;
+        return GSR_OK;
+    }
     once();   // warm-up
     CK(cudaGetLastError());
     CK(cudaEventRecord(h->ev0, st));

@@ -268,7 +268,10 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
 // for the instrument columns [0, nInsSm) in shared memory (ATOMS, no L2 traffic) and only the other
 // columns are added with REDs; the private table is flushed with one RED per touched column at the end.
 // One CTA of PRIV_THREADS per SM (the table takes most of the shared memory).
-constexpr int PRIV_THREADS = 512;
+#ifndef GSR_PRIV_THREADS
+#define GSR_PRIV_THREADS 512
+#endif
+constexpr int PRIV_THREADS = GSR_PRIV_THREADS;
 // MATCH: sum the lanes of a warp that hit the same instrument column before the atomic (one MATCH.ANY per
 // coefficient: costs 3.6 ms at Medium with uniform columns, saves 2.1 of 6.0 ms on the Zipf columns of Skewed;
 // chosen per upload from the column histogram).

@@ -26,7 +26,7 @@ GSR_PATH_ATT_COPY, GSR_PATH_FUSED, GSR_PATH_INSTR_MATCH, GSR_PATH_TEX, GSR_PATH_
 # gsr_time_aprod selectors (include/gsr_bench.h)
 GSR_TIME_APROD1_GROUP, GSR_TIME_APROD2_GROUP = 1, 2
 GSR_TIME_K_APROD1, GSR_TIME_K_APROD2_MAIN, GSR_TIME_K_APROD2_ATT, GSR_TIME_K_FUSED = 11, 12, 13, 21
-GSR_TIME_K_INS_SCATTER, GSR_TIME_K_U_TO_TIME = 14, 15
+GSR_TIME_K_INS_SCATTER, GSR_TIME_K_U_TO_TIME, GSR_TIME_OVERLAP_PROBE = 14, 15, 31
 
 # every symbol include/gsr.h declares (tests check that the library exports each one)
 SYMBOLS = [
