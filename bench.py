@@ -38,6 +38,18 @@ SOLVE_LEN = 20             # iterations per timed solve (see main_ours)
 NOMINAL_HBM_GBS = 8000.0    # north_star's "~8 TB/s", printed beside the measured copy peak
 
 
+def variant_row_bytes(cfg, path_info, gsr):
+    """The same accounting for a layout other than 5/12/6/1 (general kernels; no fusion)."""
+    ic = (2 if path_info & gsr.GSR_PATH_IC16 else 4) * cfg.n_instr_par
+    star = 8 / 32 if cfg.n_astro_par else 0
+    att = 4 if cfg.n_att_par else 0
+    full = 8 * cfg.n_par + ic + att + star
+    return {"k_aprod1": full + 16, "k_aprod2_redatt": full + 8, "k_aprod2": full - 8 * cfg.n_att_par - att + 8,
+            "k_aprod2_att": 96 + 4 + 4 + 8, "method_aprod1": 8 * cfg.n_par + 8 * bool(cfg.n_astro_par) + 8 * bool(cfg.n_att_par)
+            + 4 * cfg.n_instr_par + 16, "method_aprod2": 8 * cfg.n_par + 8 * bool(cfg.n_astro_par) + 8 * bool(cfg.n_att_par)
+            + 4 * cfg.n_instr_par + 8}
+
+
 def kernel_row_bytes(path_info, gsr):
     """Bytes per row each kernel has to stream with the DEVICE layout -- its own algorithmic bytes; a
     kernel is never credited with bytes it does not move.  values 8 B each; instrument columns 2 or 4 B; attitude
@@ -69,13 +81,20 @@ def parse():
     ap.add_argument("--kernel-reps", type=int, default=20)
     ap.add_argument("--skew-alpha", type=float, default=2.0,
                     help="exponent of the skewed workload's obs-count law (2.0: literal, ~53 M rows; 1.47: ~150 M rows, DESIGN.md R18)")
+    ap.add_argument("--layout", default="5,12,6,1",
+                    help="section widths N_Astro,N_Att,N_Instr,N_Glob of the workload (PAPER.md:78; 5,12,6,1 = production; "
+                         "0,12,6,0 and 5,0,0,0 are the section subsets of the paper's 40/300 GB and 100 GB datasets)")
     ap.add_argument("--rerun", type=int, default=0,
                     help="extra solves of the same system after the timed one; reports run-to-run max|dx| (atomics)")
     return ap.parse_args()
 
 
-def workload_cfg(name, skew_alpha=2.0):
+def workload_cfg(name, skew_alpha=2.0, layout="5,12,6,1"):
+    import dataclasses
     from paper_2308_00778_b200 import synth
+    if layout != "5,12,6,1":
+        na, nt, ni, ng = (int(t) for t in layout.split(","))
+        return dataclasses.replace(workload_cfg(name, skew_alpha), n_astro_par=na, n_att_par=nt, n_instr_par=ni, n_glob=ng)
     if name == "skewed":
         return synth.skewed(alpha=skew_alpha)
     return {"tiny": synth.tiny, "small": synth.small, "medium": synth.medium, "skewed": synth.skewed,
@@ -179,7 +198,8 @@ def oracle_sample_run(cfg, steps, warmup, target_rows=3_000_000, omp=True):
     sub = dataclasses.replace(cfg, name=cfg.name + "_sample", n_stars=ns, n_con=0, con_nnz=0)
     d = {k: v.numpy() for k, v in synth.generate(sub).items()}
     S = oracle.OracleSystem(sub.n_stars, sub.n_dof_att, sub.n_instr, d["values"], d["matrixIndexAstro"],
-                            d["matrixIndexAtt"], d["instrCol"])
+                            d["matrixIndexAtt"], d["instrCol"], n_glob=sub.n_glob, n_astro_par=sub.n_astro_par,
+                            n_att_par=sub.n_att_par, n_instr_par=sub.n_instr_par)
     b = S.aprod1(d["x_true"], d["noise"])
     S.precondition()
     out = {"rows_sample": S.m, "rows_full": full_rows, "stars_sample": ns, "steps": steps, "host": host_facts()}
@@ -220,7 +240,7 @@ def main_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    cfg = workload_cfg(args.workload, args.skew_alpha)
+    cfg = workload_cfg(args.workload, args.skew_alpha, args.layout)
     steps = max(1, min(args.steps, 10))
     o = oracle_sample_run(cfg, steps, min(args.warmup, 1))
     blk = cpu_baseline_block(o)
@@ -266,10 +286,12 @@ def main_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    cfg = workload_cfg(args.workload, args.skew_alpha)
+    cfg = workload_cfg(args.workload, args.skew_alpha, args.layout)
     rp = synth.star_rowptr(cfg)
     m = int(rp[-1])
-    G = gsr.Gsr(m, cfg.n_stars, cfg.n_dof_att, cfg.n_instr, cfg.n_con, cfg.n_con * cfg.con_nnz, device=local)
+    prod = (cfg.n_astro_par, cfg.n_att_par, cfg.n_instr_par, cfg.n_glob) == (5, 12, 6, 1)
+    G = gsr.Gsr(m, cfg.n_stars, cfg.n_dof_att, cfg.n_instr, cfg.n_con, cfg.n_con * cfg.con_nnz, device=local,
+                n_glob=cfg.n_glob, n_astro_par=cfg.n_astro_par, n_att_par=cfg.n_att_par, n_instr_par=cfg.n_instr_par)
     t_gen = time.perf_counter()
     build_on_device(cfg, G, dev, torch, synth)
     G.gsr_precondition()
@@ -314,7 +336,7 @@ def main_ours(args):
     info = G.gsr_path_info()
     fused = bool(info & gsr.GSR_PATH_FUSED)
     att_copy = bool(info & gsr.GSR_PATH_ATT_COPY)
-    rb = kernel_row_bytes(info, gsr)
+    rb = kernel_row_bytes(info, gsr) if prod else variant_row_bytes(cfg, info, gsr)
     reps = args.kernel_reps
 
     def timed_kernel(which):
@@ -354,8 +376,8 @@ def main_ours(args):
         if msf is not None else ["k_aprod1", "k_aprod2"] + (["k_aprod2_att"] if ms2a is not None else []) + (["k_ins_scatter"] if ins_copy else [])
     dom = max(in_step, key=lambda n: k[n]["ms"])
     # north-star figures on the METHOD's bytes (two products of 248 + 240 B/row)
-    gb1 = ROW_BYTES_APROD1 * m / 1e9
-    gb2 = (ROW_BYTES_APROD2 * m + 8 * G.n) / 1e9
+    gb1 = (ROW_BYTES_APROD1 if prod else rb["method_aprod1"]) * m / 1e9
+    gb2 = ((ROW_BYTES_APROD2 if prod else rb["method_aprod2"]) * m + 8 * G.n) / 1e9
     ms_step = loop_ms / args.steps
     # bytes the timed step actually has to stream with the device layout
     if msf is not None:
@@ -396,8 +418,8 @@ def main_ours(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": loop_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.workload, "rows": m, "cols": G.n, "nnz_per_row": 24,
-                       "matrix_gb": 232 * m / 1e9, "device_matrix_gb": (rb["k_aprod1"] - 16) * m / 1e9, "path_info": info, "parallelism": "replicas only" if world > 1 else "1 GPU",
+            "config": {"workload": args.workload, "layout": args.layout, "rows": m, "cols": G.n, "nnz_per_row": cfg.n_par,
+                       "matrix_gb": (232 if prod else rb["method_aprod1"] - 16) * m / 1e9, "device_matrix_gb": (rb["k_aprod1"] - 16) * m / 1e9, "path_info": info, "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "inputs larger than L2" if 232 * m > 2.5e8 else "L2-resident (launch-bound config)",
                        "x_rel_err_vs_planted": x_err, "setup_s": t_gen,
                        "timed_as": f"{len(lens)} solve(s) of <= {SOLVE_LEN} iterations; device time of the iteration loops",
@@ -406,10 +428,10 @@ def main_ours(args):
             "clocks": clk.summary(), "gpu_launches": launches, "roofline": roofline}
 
     # ---- end to end through the C ABI with HOST buffers: upload + precondition + K iterations + results
-    if not args.no_e2e and rank == 0:
+    if not args.no_e2e and rank == 0 and prod:
         line["e2e"] = e2e_run(args, cfg, G, dev, torch, synth, gsr)
     if not args.no_cpu_baseline and rank == 0 and world == 1:
-        line["cpu_baseline"] = cpu_baseline_block(oracle_sample_run(cfg, 5, 1))
+        line["cpu_baseline"] = cpu_baseline_block(oracle_sample_run(cfg, 5, 1, omp=prod))
     G.close()
     if rank == 0:
         print(json.dumps(line), flush=True)

@@ -421,7 +421,7 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
         CK(cudaMemGetInfo(&freeB, &totB));
         const size_t need = size_t(m) * (N_ATT * 8 + 4 + 4) + size_t(m) * 12 + (size_t(64) << 20);
         // GSR_FLAG_NO_ATT_COPY forces the low-memory path (attitude REDs in k_aprod2, two-product iteration)
-        if (h->prod && m > 0 && m < (int64_t(1) << 32) && L->n_dof_att < (int64_t(1) << 31) &&
+        if ((h->prod || h->nAtt > 0) && m > 0 && m < (int64_t(1) << 32) && L->n_dof_att < (int64_t(1) << 31) &&
             freeB > need + (size_t(2) << 30) && !(L->flags & GSR_FLAG_NO_ATT_COPY)) {
             bool ok = dalloc(&h->attT, m * N_ATT) == cudaSuccess && dalloc(&h->sT, m) == cudaSuccess &&
                       dalloc(&h->permT, m) == cudaSuccess;
@@ -433,7 +433,7 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
                 h->attT = nullptr; h->sT = nullptr; h->permT = nullptr;
             }
             h->useAttT = ok;
-            if (ok && !(L->flags & GSR_FLAG_NO_FUSE)) {   // u^ in time order for the fused iteration (+8 B/row); optional
+            if (ok && h->prod && !(L->flags & GSR_FLAG_NO_FUSE)) {   // u^ in time order for the fused iteration (+8 B/row); optional
                 bool ok2 = dalloc(&h->uT, m) == cudaSuccess;
                 if (!ok2) {
                     cudaGetLastError();
@@ -799,6 +799,11 @@ int enqueueAprod2(gsr_handle *h, const double *y, double *x, const double *coef,
         launchAprod2NoIns<false>(h, A, y, x, coef, done, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0});
         launchInsScatter(h, A, y, coef, done);
         nk += 2;
+    } else if (!h->prod) {   // other layouts: the attitude kernel does not depend on the other sections' widths
+        launchAtt(h, A, y, x, coef, done);
+        k_aprod2_gen<false, false><<<h->gridA2, THREADS, 0, h->stream>>>(A, y, x, coef, h->carryFirst, h->carryLast,
+                                                                          h->globPartial, done);
+        ++nk;
     } else {
         launchAtt(h, A, y, x, coef, done);
         launchAprod2Main<false>(h, A, y, x, coef, done, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0});
@@ -1180,6 +1185,9 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
         else if (which == GSR_TIME_K_U_TO_TIME) k_u_to_time<<<h->gridUT, 256, 0, st>>>(h->u, h->permT, A.m, h->uT, nullptr);
         else if (h->useInsT)
             launchAprod2NoIns<false>(h, A, h->u, h->v, h->coefTime, nullptr, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0});
+        else if (h->useAttT && !h->prod)
+            k_aprod2_gen<false, false><<<h->gridA2, THREADS, 0, st>>>(A, h->u, h->v, h->coefTime, h->carryFirst, h->carryLast,
+                                                                     h->globPartial, nullptr);
         else if (h->useAttT)
             launchAprod2Main<false>(h, A, h->u, h->v, h->coefTime, nullptr, FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0});
         else

@@ -842,7 +842,7 @@ __global__ void k_gather_att(MatView A)
          t += int64_t(gridDim.x) * blockDim.x) {
         const int64_t i = A.permT[t];
 #pragma unroll
-        for (int k = 0; k < N_ATT; ++k) A.attT[int64_t(k) * A.m + t] = A.V[vpos(i, N_ASTRO + k)];
+        for (int k = 0; k < N_ATT; ++k) A.attT[int64_t(k) * A.m + t] = A.V[vpos(i, A.nA + k, A.nPar)];
     }
 }
 
@@ -951,7 +951,9 @@ k_aprod1_gen(MatView A, const double *__restrict__ x, double *__restrict__ y, co
 
 // x <- cx*x + cy*(A^T y); the attitude / instrumental / global sections of x were multiplied by cx beforehand
 // (k_pre_aprod2).  globPartial[q*gridDim.x + blockIdx.x]: this CTA's share of global column q.
-template <bool SQUARE>
+// ATT = false: the attitude section is left to k_aprod2_att on the block-time-ordered copy (which does not depend on the
+// other sections' widths).
+template <bool SQUARE, bool ATT = true>
 __global__ void __launch_bounds__(THREADS)
 k_aprod2_gen(MatView A, const double *__restrict__ y, double *__restrict__ x, const double *__restrict__ coef,
              double *__restrict__ carryFirst, double *__restrict__ carryLast, double *__restrict__ globPartial,
@@ -998,7 +1000,7 @@ k_aprod2_gen(MatView A, const double *__restrict__ y, double *__restrict__ x, co
                 }
             }
         }
-        if (A.nAtt > 0 && valid) {   // ---- attitude
+        if (ATT && A.nAtt > 0 && valid) {   // ---- attitude
             const int64_t s = __ldcs(A.iatt + i);
             GSR_ASSERT(s >= 0 && s + 4 <= A.nDof);
             double *xt = x + A.offAtt + s;

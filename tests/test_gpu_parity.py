@@ -666,7 +666,9 @@ def test_model_variants_aprod_and_precondition(widths, shape):
     b = make_b(S, d)
     with make_gpu(S, d, b) as G:
         assert G.n == S.n == cfg.n and G.m_tot == S.m_tot
-        assert not (G.gsr_path_info() & (gsr_mod().GSR_PATH_FUSED | gsr_mod().GSR_PATH_ATT_COPY))
+        info = G.gsr_path_info()
+        assert not (info & gsr_mod().GSR_PATH_FUSED)
+        assert bool(info & gsr_mod().GSR_PATH_ATT_COPY) == (widths[1] == 12)   # the attitude kernel serves every layout
         if widths[0]:
             rp = G.gsr_get_star_rowptr().cpu().numpy()
             assert np.array_equal(rp, d["rowptr"])
@@ -698,6 +700,27 @@ def test_model_variants_lsqr(widths):
     with G:
         assert r.istop == ro.istop and abs(r.itn - ro.itn) <= 2, (r.istop, r.itn, ro.istop, ro.itn)
         assert rel(r.x.cpu().numpy(), ro.x) <= 1e-8
+
+
+@pytest.mark.parametrize("widths", [(0, 12, 6, 0), (3, 12, 4, 2)])
+def test_model_variants_without_attitude_copy(widths):
+    """GSR_FLAG_NO_ATT_COPY on a non-production layout: the attitude section goes through the REDs of k_aprod2_gen."""
+    gsr = gsr_mod()
+    Sp, dp = oracle_system(variant_cfg(widths, "powerlaw"))      # stars cut by tile edges, bursts: products only (the
+    with make_gpu(Sp, dp, make_b(Sp, dp), flags=gsr.GSR_FLAG_NO_ATT_COPY) as G:   # Zipf / burst system is too ill-posed
+        check_aprods(Sp, G, seed=5)                              # for the 1e-9 bound on x, DESIGN.md 2)
+    cfg = variant_cfg(widths, "ragged")
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    with make_gpu(S, d, b, flags=gsr.GSR_FLAG_NO_ATT_COPY) as G:
+        assert not (G.gsr_path_info() & gsr.GSR_PATH_ATT_COPY)
+        check_aprods(S, G, seed=4)
+        G.gsr_precondition()
+        S.precondition()
+        r = G.gsr_lsqr(25, 0.0, 0.0)
+        ro = S.lsqr(b, 25, 0.0, 0.0)
+        assert (r.istop, r.itn) == (ro.istop, ro.itn) == (7, 25)
+        assert rel(r.x.cpu().numpy(), ro.x) <= X_TOL
 
 
 def test_model_variants_global_columns_bit_reproducible():
