@@ -38,34 +38,27 @@ SOLVE_LEN = 20             # iterations per timed solve (see main_ours)
 NOMINAL_HBM_GBS = 8000.0    # north_star's "~8 TB/s", printed beside the measured copy peak
 
 
-def variant_row_bytes(cfg, path_info, gsr):
-    """The same accounting for a layout other than 5/12/6/1 (general kernels; no fusion)."""
+def kernel_row_bytes(cfg, path_info, gsr):
+    """Bytes per row each kernel has to stream with the DEVICE layout (DESIGN.md 5) -- its own algorithmic bytes; a
+    kernel is never credited with bytes it does not move.  values 8 B each; instrument columns 2 or 4 B; attitude
+    start 4 B; star: 8 B per 32-row tile; u 8 B read (+ 8 B written).  For any section widths (cfg); `method_*` are the
+    METHOD's bytes with the upload-format index widths (8 B per M_i entry, 4 B per instrument column)."""
     ic = (2 if path_info & gsr.GSR_PATH_IC16 else 4) * cfg.n_instr_par
     star = 8 / 32 if cfg.n_astro_par else 0
     att = 4 if cfg.n_att_par else 0
     full = 8 * cfg.n_par + ic + att + star
-    return {"k_aprod1": full + 16, "k_aprod2_redatt": full + 8, "k_aprod2": full - 8 * cfg.n_att_par - att + 8,
-            "k_aprod2_att": 96 + 4 + 4 + 8, "method_aprod1": 8 * cfg.n_par + 8 * bool(cfg.n_astro_par) + 8 * bool(cfg.n_att_par)
-            + 4 * cfg.n_instr_par + 16, "method_aprod2": 8 * cfg.n_par + 8 * bool(cfg.n_astro_par) + 8 * bool(cfg.n_att_par)
-            + 4 * cfg.n_instr_par + 8}
-
-
-def kernel_row_bytes(path_info, gsr):
-    """Bytes per row each kernel has to stream with the DEVICE layout (DESIGN.md 5) -- its own algorithmic bytes; a
-    kernel is never credited with bytes it does not move.  values 8 B each; instrument columns 2 or 4 B; attitude
-    start 4 B; star: 8 B per 32-row tile; u 8 B read (+ 8 B written)."""
-    ic = 2 * 6 if path_info & gsr.GSR_PATH_IC16 else 4 * 6
-    star = 8 / 32
+    idx = 8 * bool(cfg.n_astro_par) + 8 * bool(cfg.n_att_par) + 4 * cfg.n_instr_par
     return {
-        "k_aprod1": 192 + ic + 4 + star + 8 + 8,                 # whole row, y read + written
-        "k_aprod2_redatt": 192 + ic + 4 + star + 8,              # all four sections in one kernel (no attitude copy)
-        "k_aprod2": 96 + ic + star + 8,                          # astro / instr / gamma sections only
+        "k_aprod1": full + 8 + 8,                                # whole row, y read + written
+        "k_aprod2_redatt": full + 8,                             # all sections in one kernel (no attitude copy)
+        "k_aprod2": full - 8 * cfg.n_att_par - att + 8,          # astro / instr / global sections only
         "k_aprod2_att": 96 + 4 + 4 + 8,                          # attT + start + permutation + gathered y
         "k_aprod2_att_linear": 96 + 4 + 8,                       # attT + start + uT
         "k_u_to_time": 4 + 8 + 8,                                # permutation + gathered u + uT written
-        "k_aprod2_fused": 192 + ic + 4 + star + 8 + 8,           # whole row ONCE, u read + written
-        "k_aprod2_noins": 40 + 8 + star + 8,                     # astro + gamma coefficients only (instr by k_ins_scatter)
+        "k_aprod2_fused": full + 8 + 8,                          # whole row ONCE, u read + written
+        "k_aprod2_noins": 8 * (cfg.n_astro_par + cfg.n_glob) + star + 8,   # astro + global coefficients only (instr by k_ins_scatter)
         "k_ins_scatter": 6 * (8 + 4) + 8,                        # column-ordered copy: value + (column, row) word; u staged once
+        "method_aprod1": 8 * cfg.n_par + idx + 16, "method_aprod2": 8 * cfg.n_par + idx + 8,
     }
 
 
@@ -336,7 +329,7 @@ def main_ours(args):
     info = G.gsr_path_info()
     fused = bool(info & gsr.GSR_PATH_FUSED)
     att_copy = bool(info & gsr.GSR_PATH_ATT_COPY)
-    rb = kernel_row_bytes(info, gsr) if prod else variant_row_bytes(cfg, info, gsr)
+    rb = kernel_row_bytes(cfg, info, gsr)
     reps = args.kernel_reps
 
     def timed_kernel(which):
@@ -376,8 +369,8 @@ def main_ours(args):
         if msf is not None else ["k_aprod1", "k_aprod2"] + (["k_aprod2_att"] if ms2a is not None else []) + (["k_ins_scatter"] if ins_copy else [])
     dom = max(in_step, key=lambda n: k[n]["ms"])
     # north-star figures on the METHOD's bytes (two products of 248 + 240 B/row)
-    gb1 = (ROW_BYTES_APROD1 if prod else rb["method_aprod1"]) * m / 1e9
-    gb2 = ((ROW_BYTES_APROD2 if prod else rb["method_aprod2"]) * m + 8 * G.n) / 1e9
+    gb1 = rb["method_aprod1"] * m / 1e9      # 248 B/row in the production layout (ROW_BYTES_APROD1)
+    gb2 = (rb["method_aprod2"] * m + 8 * G.n) / 1e9      # 240 B/row
     ms_step = loop_ms / args.steps
     # bytes the timed step actually has to stream with the device layout
     if msf is not None:
@@ -419,7 +412,7 @@ def main_ours(args):
             "warmup": max(args.warmup, 3), "ms_per_step": loop_ms / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.workload, "layout": args.layout, "rows": m, "cols": G.n, "nnz_per_row": cfg.n_par,
-                       "matrix_gb": (232 if prod else rb["method_aprod1"] - 16) * m / 1e9, "device_matrix_gb": (rb["k_aprod1"] - 16) * m / 1e9, "path_info": info, "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "matrix_gb": (rb["method_aprod1"] - 16) * m / 1e9, "device_matrix_gb": (rb["k_aprod1"] - 16) * m / 1e9, "path_info": info, "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "inputs larger than L2" if 232 * m > 2.5e8 else "L2-resident (launch-bound config)",
                        "x_rel_err_vs_planted": x_err, "setup_s": t_gen,
                        "timed_as": f"{len(lens)} solve(s) of <= {SOLVE_LEN} iterations; device time of the iteration loops",

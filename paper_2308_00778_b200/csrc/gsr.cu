@@ -18,11 +18,22 @@
 
 using namespace gsr;
 
+// Runs CALL with NA_ / NG_ bound to the section widths of the handle's layout (the three layouts that share the
+// specialised kernels, see gsr_handle::lay).
+#define GSR_LAY(h, CALL)                              \
+    switch ((h)->lay) {                               \
+    case 0: { constexpr int NA_ = 5, NG_ = 1; CALL; } break; \
+    case 1: { constexpr int NA_ = 5, NG_ = 0; CALL; } break; \
+    default: { constexpr int NA_ = 0, NG_ = 0; CALL; } break; \
+    }
+
 struct gsr_handle {
     gsr_layout L{};
     int64_t n = 0, mTot = 0, nTiles = 0;
     int nA = N_ASTRO, nAtt = N_ATT, nI = N_INSTR, nG = 1, nPar = N_PAR;   // section widths
-    bool prod = true;   // 5/12/6/1: the specialised kernels; any other layout runs k_aprod1_gen / k_aprod2_gen
+    bool prod = true;   // 5/12/6/1, 5/12/6/0 or 0/12/6/0: the specialised kernels (fused iteration); any other layout runs
+                        // k_aprod1_gen / k_aprod2_gen
+    int lay = 0;        // which of the three: 0 = 5/12/6/1 (production), 1 = 5/12/6/0, 2 = 0/12/6/0
     cudaStream_t stream = nullptr;
     cudaStream_t userStream = nullptr;
     cudaStream_t stream2 = nullptr;   // second stream of the overlap probe (gsr_time_aprod)
@@ -212,7 +223,7 @@ int buildInsT(gsr_handle *h)
         if (q) cudaFree(q);
     h->insVal = nullptr; h->insMeta = nullptr; h->insPtr = nullptr;
     h->useInsT = false;
-    if (!h->prod || !h->useAttT || !h->ic16 || h->instrSkewed || !(h->L.flags & GSR_FLAG_INS_COPY) || m <= 0)
+    if (!h->prod || h->lay != 0 || !h->useAttT || !h->ic16 || h->instrSkewed || !(h->L.flags & GSR_FLAG_INS_COPY) || m <= 0)
         return GSR_OK;
     const int64_t slabRows = int64_t(1) << 22, nBlocks = (m + INS_BLOCK - 1) >> INS_ROW_BITS;
     const int64_t slabE = std::min(m, slabRows) * N_INSTR;
@@ -286,7 +297,9 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
                     "(got %d/%d/%d/%d)", GSR_MAX_GLOB, L->n_astro_par, L->n_att_par, L->n_instr_par, L->n_glob_par);
     h->nA = L->n_astro_par; h->nAtt = L->n_att_par; h->nI = L->n_instr_par; h->nG = L->n_glob_par;
     h->nPar = h->nA + h->nAtt + h->nI + h->nG;
-    h->prod = h->nA == GSR_N_ASTRO && h->nAtt == GSR_N_ATT && h->nI == GSR_N_INSTR && h->nG == GSR_N_GLOB;
+    h->lay = h->nA == GSR_N_ASTRO ? (h->nG == 1 ? 0 : 1) : 2;
+    h->prod = h->nAtt == GSR_N_ATT && h->nI == GSR_N_INSTR &&
+              ((h->nA == GSR_N_ASTRO && h->nG <= 1) || (h->nA == 0 && h->nG == 0));
     if (L->n_obs < 0 || L->n_stars < 0 || (h->nA > 0 && L->n_stars < 1) || (h->nAtt > 0 && L->n_dof_att < 4) ||
         L->n_dof_att < 0 || L->n_instr < h->nI || L->n_con < 0 || L->n_con_nnz < 0 || (L->n_con == 0 && L->n_con_nnz != 0))
         return fail(h, GSR_EINVAL, "bad sizes");
@@ -324,14 +337,15 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
         const int64_t fit = (int64_t(maxSm) - 1024) / int64_t(sizeof(double));
         h->nInsSm = int(std::max<int64_t>(0, std::min<int64_t>(L->n_instr, fit)));
         const int smB = int(h->nInsSm * sizeof(double));
-        CK(cudaFuncSetAttribute(k_aprod2<false, false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
-        CK(cudaFuncSetAttribute(k_aprod2<false, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
-        CK(cudaFuncSetAttribute(k_aprod2<false, false, false, true, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
-        CK(cudaFuncSetAttribute(k_aprod2<false, false, false, true, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
-        CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
-        CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
-        CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, false, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
-        CK(cudaFuncSetAttribute(k_aprod2<true, false, false, true, true, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smB));
+        cudaError_t ea = cudaSuccess;
+        auto setSm = [&](const void *f) {
+            if (ea == cudaSuccess) ea = cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, smB);
+        };
+#define GSR_SETSM(IC, MA, FU) GSR_LAY(h, (setSm((const void *)k_aprod2<IC, false, false, true, MA, FU, FU, true, NA_, NG_>)))
+        GSR_SETSM(false, false, false); GSR_SETSM(false, true, false); GSR_SETSM(false, false, true); GSR_SETSM(false, true, true);
+        GSR_SETSM(true, false, false); GSR_SETSM(true, true, false); GSR_SETSM(true, false, true); GSR_SETSM(true, true, true);
+#undef GSR_SETSM
+        CK(ea);
         // the fused kernel also gathers x, which needs L1: the table takes 128 KB of the SM's 228 KB (measured at Medium,
         // fused pass alone: 0 / 4 k / 8 k / 12 k / 16 k / 20 k columns -> 16.7 / 16.5 / 15.8 / 15.5 / 15.3 / 15.7 ms)
         h->nInsSmFused = std::min(h->nInsSm, 16384);
@@ -340,7 +354,7 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     h->gridVec = gridFor(std::max(h->n, h->mTot), 256 * 4, h->smCount * 8);
     h->gridCon = gridFor(L->n_con, 8, h->smCount * 8);
     // fix-up grid: one thread per star, then one per instrument column (replica fold), then gamma
-    h->gridFix = int((L->n_stars + 255) / 256) + int((L->n_instr + 255) / 256) + 1;
+    h->gridFix = (h->nA > 0 ? int((L->n_stars + 255) / 256) : 0) + int((L->n_instr + 255) / 256) + 1;
     if (!h->prod) h->gridFix = (h->nA > 0 ? int((L->n_stars + 255) / 256) : 0) + 1;   // k_fixup_gen: stars, then the global columns
     h->gridAtt = gridFor(h->nTiles, 8, h->smCount * 4);
     h->gridUT = gridFor(L->n_obs, 256, h->smCount * 4);
@@ -699,8 +713,8 @@ void launchAprod1(gsr_handle *h, const MatView &A, const double *x, double *y, c
                   const int *done)
 {
     if (!h->prod) k_aprod1_gen<<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done);
-    else if (h->ic16) k_aprod1<true><<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done, h->xPack);
-    else k_aprod1<false><<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done, h->xPack);
+    else if (h->ic16) GSR_LAY(h, (k_aprod1<true, NA_, NG_><<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done, h->xPack)))
+    else GSR_LAY(h, (k_aprod1<false, NA_, NG_><<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done, h->xPack)))
 }
 
 // all sections in one kernel, attitude by REDs (preconditioner pass; low-memory path)
@@ -711,11 +725,11 @@ void launchAprod2Red(gsr_handle *h, const MatView &A, const double *y, double *x
         k_aprod2_gen<SQUARE><<<h->gridA2, THREADS, 0, h->stream>>>(A, y, x, coef, h->carryFirst, h->carryLast,
                                                                   h->globPartial, done);
     else if (h->ic16)
-        k_aprod2<true, SQUARE, true><<<h->gridA2, THREADS, 0, h->stream>>>(A, y, x, coef, h->carryFirst, h->carryLast,
-                                                                          h->globPartial, done);
+        GSR_LAY(h, (k_aprod2<true, SQUARE, true, false, false, false, false, true, NA_, NG_><<<h->gridA2, THREADS, 0, h->stream>>>(
+                       A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done)))
     else
-        k_aprod2<false, SQUARE, true><<<h->gridA2, THREADS, 0, h->stream>>>(A, y, x, coef, h->carryFirst, h->carryLast,
-                                                                           h->globPartial, done);
+        GSR_LAY(h, (k_aprod2<false, SQUARE, true, false, false, false, false, true, NA_, NG_><<<h->gridA2, THREADS, 0, h->stream>>>(
+                       A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done)))
 }
 
 // astro / instr / gamma with the shared-memory instrument table; FUSE: the fused pass of gsr_lsqr
@@ -727,17 +741,17 @@ void launchAprod2Main(gsr_handle *h, const MatView &A, const double *y, double *
     const int g = h->gridA2m;
     cudaStream_t st = h->stream;
     if (FUSE && h->fusedNoPriv && h->ic16 && !h->instrSkewed) {
-        k_aprod2<true, false, false, false, false, FUSE, FUSE, true><<<h->gridA2, THREADS, 0, st>>>(
-            A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done, F);
+        GSR_LAY(h, (k_aprod2<true, false, false, false, false, FUSE, FUSE, true, NA_, NG_><<<h->gridA2, THREADS, 0, st>>>(
+                       A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done, F)))
         return;
     }
 #define GSR_A2M(IC, MA)                                                                                          \
-    k_aprod2<IC, false, false, true, MA, FUSE, FUSE><<<g, PRIV_THREADS, sm, st>>>(A, y, x, coef, h->carryFirst,    \
-                                                                                 h->carryLast, h->globPartial, done, F)
+    GSR_LAY(h, (k_aprod2<IC, false, false, true, MA, FUSE, FUSE, true, NA_, NG_><<<g, PRIV_THREADS, sm, st>>>(       \
+                   A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done, F)))
     if (h->ic16) {
-        if (h->instrSkewed) GSR_A2M(true, true); else GSR_A2M(true, false);
+        if (h->instrSkewed) { GSR_A2M(true, true) } else { GSR_A2M(true, false) }
     } else {
-        if (h->instrSkewed) GSR_A2M(false, true); else GSR_A2M(false, false);
+        if (h->instrSkewed) { GSR_A2M(false, true) } else { GSR_A2M(false, false) }
     }
 #undef GSR_A2M
 }

@@ -145,13 +145,16 @@ __device__ __forceinline__ double block_sum(double v, double *red)
 
 // The 24 coefficients of row (tile, lane): coalesced streaming loads.  ATT: load the attitude
 // coefficients too (k = 5..16).
-template <bool ATT, bool INS = true>
-__device__ __forceinline__ void load_row(const double *__restrict__ V, int64_t tile, int lane, double (&v)[N_PAR])
+// NA (5 or 0 astrometric coefficients) and NG (1 or 0 global ones) select the layouts that share the specialised kernels:
+// 5/12/6/1 (production), 5/12/6/0 and 0/12/6/0 (the section subsets the paper's datasets solve).
+template <bool ATT, bool INS = true, int NA = N_ASTRO, int NG = 1>
+__device__ __forceinline__ void load_row(const double *__restrict__ V, int64_t tile, int lane, double (&v)[NA + N_ATT + N_INSTR + NG])
 {
-    const double *g = V + tile * (N_PAR * TILE) + lane;
+    constexpr int NP = NA + N_ATT + N_INSTR + NG;
+    const double *g = V + tile * (NP * TILE) + lane;
 #pragma unroll
-    for (int q = 0; q < N_PAR; ++q) {
-        const bool att = q >= N_ASTRO && q < N_ASTRO + N_ATT, ins = q >= N_ASTRO + N_ATT && q < N_PAR - 1;
+    for (int q = 0; q < NP; ++q) {
+        const bool att = q >= NA && q < NA + N_ATT, ins = q >= NA + N_ATT && q < NA + N_ATT + N_INSTR;
         if ((att && !ATT) || (ins && !INS)) v[q] = 0.0;
         else v[q] = __ldcs(g + q * TILE);
     }
@@ -196,7 +199,7 @@ __global__ void k_pack_att(MatView A, const double *__restrict__ x, double *__re
     }
 }
 
-template <bool IC16>
+template <bool IC16, int NA = N_ASTRO, int NG = 1>
 __global__ void __launch_bounds__(THREADS, 2)
 k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
          const double *__restrict__ coef, double *__restrict__ sqPartial, const int *done,
@@ -208,7 +211,8 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
     const double cx = coef[0], cy = coef[1];
     const int64_t nTiles = (A.m + TILE - 1) / TILE;
     const double *xIns = x + A.offInstr;
-    const double xg = __ldg(x + A.offGlob);
+    const double xg = NG ? __ldg(x + A.offGlob) : 0.0;
+    constexpr int KT = NA, KI = NA + N_ATT, KG = NA + N_ATT + N_INSTR;
     double sq = 0.0;
     for (int64_t tile = int64_t(blockIdx.x) * WARPS + warp; tile < nTiles;
          tile += int64_t(gridDim.x) * WARPS) {
@@ -216,28 +220,31 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
         const int nrows = int(min(int64_t(TILE), A.m - r0));
         if (lane < nrows) {
             const int64_t i = r0 + lane;
-            double v[N_PAR];
-            load_row<true>(A.V, tile, lane, v);
-            const double *xa = x + 5 * star_of(A, __ldg(A.tw + tile), i, lane);
+            double v[KG + NG];
+            load_row<true, true, NA, NG>(A.V, tile, lane, v);
             const int64_t iatt = __ldcs(A.iatt + i);
             int32_t c[N_INSTR];
             load_ic<IC16>(A, tile, lane, c);
-            GSR_ASSERT(xa >= x && xa + N_ASTRO <= x + A.offAtt && iatt >= 0 && iatt + 4 <= A.nDof);
+            GSR_ASSERT(iatt >= 0 && iatt + 4 <= A.nDof);
 #pragma unroll
             for (int j = 0; j < N_INSTR; ++j) GSR_ASSERT(c[j] >= 0 && c[j] < A.nInstr);
             double sum = 0.0;
+            if (NA > 0) {
+                const double *xa = x + NA * star_of(A, __ldg(A.tw + tile), i, lane);
+                GSR_ASSERT(xa >= x && xa + NA <= x + A.offAtt);
 #pragma unroll
-            for (int k = 0; k < N_ASTRO; ++k) sum = fma(v[k], __ldg(xa + k), sum);
+                for (int k = 0; k < NA; ++k) sum = fma(v[k], __ldg(xa + k), sum);
+            }
             {
                 const double *xp = xPack + 3 * iatt;
 #pragma unroll
                 for (int j = 0; j < 4; ++j)
 #pragma unroll
-                    for (int a = 0; a < 3; ++a) sum = fma(v[5 + 4 * a + j], __ldg(xp + 3 * j + a), sum);
+                    for (int a = 0; a < 3; ++a) sum = fma(v[KT + 4 * a + j], __ldg(xp + 3 * j + a), sum);
             }
 #pragma unroll
-            for (int j = 0; j < N_INSTR; ++j) sum = fma(v[17 + j], __ldg(xIns + c[j]), sum);
-            sum = fma(v[23], xg, sum);
+            for (int j = 0; j < N_INSTR; ++j) sum = fma(v[KI + j], __ldg(xIns + c[j]), sum);
+            if (NG) sum = fma(v[NG ? KG : 0], xg, sum);
             const double yi = fma(cy, y[i], cx * sum);
             y[i] = yi;
             sq = fma(yi, yi, sq);
@@ -298,7 +305,7 @@ __device__ __forceinline__ double tex_f64(cudaTextureObject_t t, int64_t idx)
 // here, no shared-memory table, two CTAs of 256 threads per SM); without FUSE its coefficients and columns are not
 // even loaded.
 template <bool IC16, bool SQUARE, bool ATT_RED, bool PRIV = false, bool MATCH = false, bool FUSE = false, bool FUSE_ATT = false,
-          bool INS = true>
+          bool INS = true, int NA = N_ASTRO, int NG = 1>
 __global__ void __launch_bounds__(PRIV ? PRIV_THREADS : THREADS, PRIV ? 1 : 2)
 k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
          const double *__restrict__ coef, double *__restrict__ carryFirst,
@@ -323,21 +330,22 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
     }
     double gsum = 0.0, sq = 0.0;
     const double cx1 = FUSE ? F.coef1[0] : 0.0;
-    const double xg1 = FUSE ? __ldg(F.xin + A.offGlob) : 0.0;
+    const double xg1 = FUSE && NG ? __ldg(F.xin + A.offGlob) : 0.0;
+    constexpr int KT = NA, KI = NA + N_ATT, KG = NA + N_ATT + N_INSTR, NP = KG + NG;
     for (int64_t tile = int64_t(blockIdx.x) * nWarpsCta + warp; tile < nTiles;
          tile += int64_t(gridDim.x) * nWarpsCta) {
         const int64_t r0 = tile * TILE;
         const int nrows = int(min(int64_t(TILE), A.m - r0));
         const bool valid = lane < nrows;
         const int64_t i = r0 + (valid ? lane : nrows - 1);
-        double v[N_PAR];
-        load_row<ATT_RED || FUSE_ATT, INS || FUSE>(A.V, tile, valid ? lane : nrows - 1, v);
-        const unsigned long long tw = __ldg(A.tw + tile);   // one 8-byte word per tile: first star, head mask, cut flags
-        const int64_t ia = 5 * star_of(A, tw, i, valid ? lane : nrows - 1);
+        double v[NP];
+        load_row<ATT_RED || FUSE_ATT, INS || FUSE, NA, NG>(A.V, tile, valid ? lane : nrows - 1, v);
+        const unsigned long long tw = NA ? __ldg(A.tw + tile) : 0ull;   // one 8-byte word per tile: first star, head mask, cut flags
+        const int64_t ia = NA ? NA * star_of(A, tw, i, valid ? lane : nrows - 1) : 0;
         // padded storage: the lanes past the last row read column 0 and a zero coefficient
         int32_t c[N_INSTR] = {0, 0, 0, 0, 0, 0};
         if (INS || FUSE) load_ic<IC16>(A, tile, lane, c);
-        GSR_ASSERT(ia >= 0 && ia + N_ASTRO <= A.offAtt);
+        GSR_ASSERT(ia >= 0 && ia + NA <= A.offAtt);
 #pragma unroll
         for (int j = 0; j < N_INSTR; ++j) GSR_ASSERT(c[j] >= 0 && c[j] < A.nInstr);
         double yv = 0.0;
@@ -346,13 +354,13 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
                 const double *xa = F.xin + ia, *xIn = F.xin + A.offInstr;
                 double sum = 0.0;
 #pragma unroll
-                for (int k = 0; k < N_ASTRO; ++k) sum = fma(v[k], __ldg(xa + k), sum);
+                for (int k = 0; k < NA; ++k) sum = fma(v[k], __ldg(xa + k), sum);
 #pragma unroll
                 for (int j = 0; j < N_INSTR; ++j) {
                     const double xj = F.texX ? tex_f64(F.texX, A.offInstr + c[j]) : __ldg(xIn + c[j]);
-                    sum = fma(v[17 + j], xj, sum);
+                    sum = fma(v[KI + j], xj, sum);
                 }
-                sum = fma(v[23], xg1, sum);
+                if (NG) sum = fma(v[NG ? KG : 0], xg1, sum);
                 double yOld = F.yrw[i];
                 if (FUSE_ATT) {
                     const int64_t iattRow = __ldcs(A.iatt + i);
@@ -363,7 +371,7 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
 #pragma unroll
                         for (int a = 0; a < 3; ++a) {
                             const double xa3 = F.texPack ? tex_f64(F.texPack, 3 * iattRow + 3 * j + a) : __ldg(xp + 3 * j + a);
-                            sum = fma(v[5 + 4 * a + j], xa3, sum);
+                            sum = fma(v[KT + 4 * a + j], xa3, sum);
                         }
                     yOld *= F.coef1[1];
                 }
@@ -376,7 +384,7 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
             yv = SQUARE ? 1.0 : cy * y[i];
         }
 #pragma unroll
-        for (int k = 0; k < N_PAR; ++k) v[k] = SQUARE ? v[k] * v[k] * yv : v[k] * yv;
+        for (int k = 0; k < NP; ++k) v[k] = SQUARE ? v[k] * v[k] * yv : v[k] * yv;
 
         // ---- attitude + instrumental scatter (invalid lanes hold zeros and add nothing)
         if (ATT_RED && valid) {
@@ -385,14 +393,14 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
 #pragma unroll
             for (int a = 0; a < 3; ++a)
 #pragma unroll
-                for (int j = 0; j < 4; ++j) atomicAdd(xt + a * A.nDof + j, v[5 + 4 * a + j]);
+                for (int j = 0; j < 4; ++j) atomicAdd(xt + a * A.nDof + j, v[KT + 4 * a + j]);
         }
         if (INS) {
 #pragma unroll
             for (int j = 0; j < N_INSTR; ++j) {
                 // lanes of the warp that hit the same column (hot columns of a skewed distribution) are summed
                 // in lane order first and the lowest lane adds once: no same-address atomics inside a warp
-                double val = v[17 + j];
+                double val = v[KI + j];
                 bool add = valid;
                 const unsigned peers = MATCH ? __match_any_sync(0xffffffffu, valid ? c[j] : -1 - lane) : 0u;
                 if (MATCH && __any_sync(0xffffffffu, (peers & (peers - 1)) != 0)) {
@@ -415,20 +423,21 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
             }
         }
         // ---- gamma: fixed-order warp sum, accumulated per warp over its tiles
-        gsum += warp_sum(v[23]);
+        if (NG) gsum += warp_sum(v[NG ? KG : 0]);
 
         // ---- astro: segmented scan by star over the tile's rows
+        if (NA == 0) continue;
         const unsigned heads = uint32_t(tw) | 1u;          // segment starts inside the tile (lane 0 always opens one)
         const bool tail = valid && ((lane == nrows - 1) || ((heads >> 1) >> lane) & 1u);
         const int segStart = 31 - __clz(heads & (0xffffffffu >> (31 - lane)));
         const int dist = lane - segStart;
-        double s[N_ASTRO];
+        double s[NA > 0 ? NA : 1];
 #pragma unroll
-        for (int k = 0; k < N_ASTRO; ++k) s[k] = v[k];
+        for (int k = 0; k < NA; ++k) s[k] = v[k];
 #pragma unroll
         for (int d = 1; d < 32; d <<= 1) {
 #pragma unroll
-            for (int k = 0; k < N_ASTRO; ++k) {
+            for (int k = 0; k < NA; ++k) {
                 const double t = __shfl_up_sync(0xffffffffu, s[k], d);
                 if (dist >= d) s[k] += t;
             }
@@ -440,12 +449,12 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
             if (!cut) {
                 double *xa = x + ia;
 #pragma unroll
-                for (int k = 0; k < N_ASTRO; ++k) xa[k] = fma(cx, xa[k], s[k]);
+                for (int k = 0; k < NA; ++k) xa[k] = fma(cx, xa[k], s[k]);
             } else {
                 GSR_ASSERT(tile >= 0 && tile < nTiles);
                 double *c = (segStart == 0 ? carryFirst : carryLast) + tile * N_ASTRO;
 #pragma unroll
-                for (int k = 0; k < N_ASTRO; ++k) c[k] = s[k];
+                for (int k = 0; k < NA; ++k) c[k] = s[k];
             }
         }
     }
@@ -453,7 +462,7 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
     __syncthreads();
     if (lane == 0) red[warp] = gsum;
     __syncthreads();
-    if (threadIdx.x == 0) {
+    if (NG && threadIdx.x == 0) {
         double g = 0.0;
         for (int w = 0; w < nWarpsCta; ++w) g += red[w];
         globPartial[blockIdx.x] = g;
@@ -480,8 +489,9 @@ k_astro_fixup(MatView A, double *__restrict__ x, const double *__restrict__ coef
     __shared__ double red[32];
     if (done && *done) return;
     const double cx = coef[0];
-    const int starBlocks = int((A.nStars + blockDim.x - 1) / blockDim.x);
+    const int starBlocks = A.nA > 0 ? int((A.nStars + blockDim.x - 1) / blockDim.x) : 0;
     if (blockIdx.x == gridDim.x - 1) {
+        if (A.nG == 0) return;
         double g = 0.0;
         for (int p = threadIdx.x; p < nGlobPartial; p += blockDim.x) g += globPartial[p];
         g = block_sum(g, red);
@@ -502,10 +512,9 @@ k_astro_fixup(MatView A, double *__restrict__ x, const double *__restrict__ coef
     if (s >= A.nStars) return;
     const int64_t r0 = A.rp[s], r1 = A.rp[s + 1];
     GSR_ASSERT(r0 >= 0 && r0 <= r1 && r1 <= A.m);
-    double *xa = x + s * N_ASTRO;
+    double *xa = x + s * A.nA;
     if (r0 == r1) {
-#pragma unroll
-        for (int k = 0; k < N_ASTRO; ++k) xa[k] *= cx;
+        for (int k = 0; k < A.nA; ++k) xa[k] *= cx;
         return;
     }
     const int64_t t0 = r0 / TILE, t1 = (r1 - 1) / TILE;
@@ -514,10 +523,11 @@ k_astro_fixup(MatView A, double *__restrict__ x, const double *__restrict__ coef
     for (int64_t t = t0; t <= t1; ++t) {
         const double *c = ((t == t0 && r0 != t * TILE) ? carryLast : carryFirst) + t * N_ASTRO;
 #pragma unroll
-        for (int k = 0; k < N_ASTRO; ++k) acc[k] += c[k];
+        for (int k = 0; k < N_ASTRO; ++k) acc[k] += k < A.nA ? c[k] : 0.0;
     }
 #pragma unroll
-    for (int k = 0; k < N_ASTRO; ++k) xa[k] = fma(cx, xa[k], acc[k]);
+    for (int k = 0; k < N_ASTRO; ++k)
+        if (k < A.nA) xa[k] = fma(cx, xa[k], acc[k]);
 }
 
 // Before the scatter of aprod2: x[lo..hi) *= coef[0] (att + instr + gamma sections, only when

@@ -667,7 +667,9 @@ def test_model_variants_aprod_and_precondition(widths, shape):
     with make_gpu(S, d, b) as G:
         assert G.n == S.n == cfg.n and G.m_tot == S.m_tot
         info = G.gsr_path_info()
-        assert not (info & gsr_mod().GSR_PATH_FUSED)
+        # 5/12/6/0 and 0/12/6/0 (the section subsets of the paper's datasets) share the specialised kernels and the fused
+        # iteration with the production layout; the other layouts run the general kernels
+        assert bool(info & gsr_mod().GSR_PATH_FUSED) == (widths in ((5, 12, 6, 0), (0, 12, 6, 0)))
         assert bool(info & gsr_mod().GSR_PATH_ATT_COPY) == (widths[1] == 12)   # the attitude kernel serves every layout
         if widths[0]:
             rp = G.gsr_get_star_rowptr().cpu().numpy()
@@ -700,6 +702,26 @@ def test_model_variants_lsqr(widths):
     with G:
         assert r.istop == ro.istop and abs(r.itn - ro.itn) <= 2, (r.istop, r.itn, ro.istop, ro.itn)
         assert rel(r.x.cpu().numpy(), ro.x) <= 1e-8
+
+
+@pytest.mark.parametrize("flag", ["NO_FUSE", "NO_TEX"])
+@pytest.mark.parametrize("widths", [(5, 12, 6, 0), (0, 12, 6, 0)])
+def test_fast_variant_layouts_fallback_paths(widths, flag):
+    """The two non-production layouts that run the specialised kernels, in the two-product form and without textures."""
+    gsr = gsr_mod()
+    cfg = variant_cfg(widths, "multi_cta")
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    with make_gpu(S, d, b, flags={"NO_FUSE": gsr.GSR_FLAG_NO_FUSE, "NO_TEX": gsr.GSR_FLAG_NO_TEX}[flag]) as G:
+        assert bool(G.gsr_path_info() & gsr.GSR_PATH_FUSED) == (flag == "NO_TEX")
+        check_aprods(S, G, seed=6)
+        G.gsr_precondition()
+        S.precondition()
+        r = G.gsr_lsqr(15, 0.0, 0.0)
+        ro = S.lsqr(b, 15, 0.0, 0.0)
+        assert (r.istop, r.itn) == (ro.istop, ro.itn) == (7, 15)
+        assert rel(r.x.cpu().numpy(), ro.x) <= X_TOL
+        assert rel(r.se.cpu().numpy(), ro.se) <= 1e-8
 
 
 @pytest.mark.parametrize("widths", [(0, 12, 6, 0), (3, 12, 4, 2)])
