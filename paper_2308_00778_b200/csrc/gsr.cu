@@ -746,7 +746,7 @@ void launchAprod2Main(gsr_handle *h, const MatView &A, const double *y, double *
         return;
     }
 #define GSR_A2M(IC, MA)                                                                                          \
-    GSR_LAY(h, (k_aprod2<IC, false, false, true, MA, FUSE, FUSE, true, NA_, NG_><<<g, PRIV_THREADS, sm, st>>>(       \
+    GSR_LAY(h, (k_aprod2<IC, false, false, true, MA, FUSE, FUSE, true, NA_, NG_><<<g, priv_threads(FUSE), sm, st>>>(       \
                    A, y, x, coef, h->carryFirst, h->carryLast, h->globPartial, done, F)))
     if (h->ic16) {
         if (h->instrSkewed) { GSR_A2M(true, true) } else { GSR_A2M(true, false) }

@@ -274,11 +274,15 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
 // PRIV ("shared-memory histogram plus global atomics", north_star): the CTA keeps private accumulators
 // for the instrument columns [0, nInsSm) in shared memory (ATOMS, no L2 traffic) and only the other
 // columns are added with REDs; the private table is flushed with one RED per touched column at the end.
-// One CTA of PRIV_THREADS per SM (the table takes most of the shared memory).
+// One CTA per SM (the table takes most of the shared memory).
 #ifndef GSR_PRIV_THREADS
 #define GSR_PRIV_THREADS 512
 #endif
-constexpr int PRIV_THREADS = GSR_PRIV_THREADS;
+constexpr int PRIV_THREADS = GSR_PRIV_THREADS;   // fused pass (117 registers per thread)
+// The standalone main kernel needs 64 registers: 32 warps per SM instead of 16 hide twice the load latency
+// (Medium: 7.93 -> 6.86 ms)
+constexpr int PRIV_THREADS_MAIN = 1024;
+__host__ __device__ constexpr int priv_threads(bool fuse) { return fuse ? PRIV_THREADS : PRIV_THREADS_MAIN; }
 // MATCH: sum the lanes of a warp that hit the same instrument column before the atomic (one MATCH.ANY per
 // coefficient: costs 3.6 ms at Medium with uniform columns, saves 2.1 of 6.0 ms on the Zipf columns of Skewed;
 // chosen per upload from the column histogram).
@@ -306,7 +310,7 @@ __device__ __forceinline__ double tex_f64(cudaTextureObject_t t, int64_t idx)
 // even loaded.
 template <bool IC16, bool SQUARE, bool ATT_RED, bool PRIV = false, bool MATCH = false, bool FUSE = false, bool FUSE_ATT = false,
           bool INS = true, int NA = N_ASTRO, int NG = 1>
-__global__ void __launch_bounds__(PRIV ? PRIV_THREADS : THREADS, PRIV ? 1 : 2)
+__global__ void __launch_bounds__(PRIV ? priv_threads(FUSE) : THREADS, PRIV ? 1 : 2)
 k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
          const double *__restrict__ coef, double *__restrict__ carryFirst,
          double *__restrict__ carryLast, double *__restrict__ globPartial, const int *done,
@@ -316,7 +320,8 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
     extern __shared__ double sIns[];   // PRIV: nInsSm private instrument accumulators
     if (done && *done) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int nWarpsCta = PRIV ? PRIV_THREADS / 32 : WARPS;
+    constexpr int PT = PRIV ? priv_threads(FUSE) : THREADS;
+    const int nWarpsCta = PT / 32;
     const double cx = coef[0], cy = coef[1];
     const int64_t nTiles = (A.m + TILE - 1) / TILE;
     double *xAtt = x + A.offAtt;
@@ -325,7 +330,7 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
     double *xIns = A.insRep + int64_t((blockIdx.x * nWarpsCta + warp) % A.nRep) * A.nInstr;
     const int32_t nSm = PRIV ? A.nInsSm : 0;
     if (PRIV) {
-        for (int c = threadIdx.x; c < nSm; c += PRIV_THREADS) sIns[c] = 0.0;
+        for (int c = threadIdx.x; c < nSm; c += PT) sIns[c] = 0.0;
         __syncthreads();
     }
     double gsum = 0.0, sq = 0.0;
@@ -472,7 +477,7 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         if (threadIdx.x == 0) F.sqPartial[blockIdx.x] = b;
     }
     if (PRIV) {   // flush the private table (the barrier above ordered the ATOMS before these reads)
-        for (int c = threadIdx.x; c < nSm; c += PRIV_THREADS) {
+        for (int c = threadIdx.x; c < nSm; c += PT) {
             const double t = sIns[c];
             if (t != 0.0) atomicAdd(xIns + c, t);
         }
