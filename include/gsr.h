@@ -28,8 +28,8 @@
  *     k < kT : offAtt + a*n_dof_att + matrixIndexAtt[i] + j,  a=(k-kA)/4, j=(k-kA)%4
  *     k < kI : offInstr + instrCol[n_instr_par*i + (k-kT)]
  *     else   : offGlob + (k-kI)                 (Alg. 2 "glob")
- * The production layout 5/12/6/1 and the section subsets 5/12/6/0 and 0/12/6/0 run the specialised
- * kernels (fused iteration, attitude copy); every other layout runs one general pair of aprod kernels
+ * The production layout 5/12/6/1, 5/12/6/N_Glob for any other N_Glob, and the section subset
+ * 0/12/6/0 run the specialised kernels (fused iteration, attitude copy); every other layout runs one general pair of aprod kernels
  * and the two-product iteration (its attitude section still on the attitude copy).
  *
  * Conventions

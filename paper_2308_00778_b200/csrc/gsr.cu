@@ -24,16 +24,18 @@ using namespace gsr;
     switch ((h)->lay) {                               \
     case 0: { constexpr int NA_ = 5, NG_ = 1; CALL; } break; \
     case 1: { constexpr int NA_ = 5, NG_ = 0; CALL; } break; \
-    default: { constexpr int NA_ = 0, NG_ = 0; CALL; } break; \
+    case 2: { constexpr int NA_ = 0, NG_ = 0; CALL; } break; \
+    default: { constexpr int NA_ = 5, NG_ = -1; CALL; } break; \
     }
 
 struct gsr_handle {
     gsr_layout L{};
     int64_t n = 0, mTot = 0, nTiles = 0;
     int nA = N_ASTRO, nAtt = N_ATT, nI = N_INSTR, nG = 1, nPar = N_PAR;   // section widths
-    bool prod = true;   // 5/12/6/1, 5/12/6/0 or 0/12/6/0: the specialised kernels (fused iteration); any other layout runs
+    bool prod = true;   // 5/12/6/N_Glob or 0/12/6/0: the specialised kernels (fused iteration); any other layout runs
                         // k_aprod1_gen / k_aprod2_gen
-    int lay = 0;        // which of the three: 0 = 5/12/6/1 (production), 1 = 5/12/6/0, 2 = 0/12/6/0
+    int lay = 0;        // which: 0 = 5/12/6/1 (production), 1 = 5/12/6/0, 2 = 0/12/6/0, 3 = 5/12/6/N_Glob > 1
+                        //
     cudaStream_t stream = nullptr;
     cudaStream_t userStream = nullptr;
     cudaStream_t stream2 = nullptr;   // second stream of the overlap probe (gsr_time_aprod)
@@ -297,9 +299,8 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
                     "(got %d/%d/%d/%d)", GSR_MAX_GLOB, L->n_astro_par, L->n_att_par, L->n_instr_par, L->n_glob_par);
     h->nA = L->n_astro_par; h->nAtt = L->n_att_par; h->nI = L->n_instr_par; h->nG = L->n_glob_par;
     h->nPar = h->nA + h->nAtt + h->nI + h->nG;
-    h->lay = h->nA == GSR_N_ASTRO ? (h->nG == 1 ? 0 : 1) : 2;
-    h->prod = h->nAtt == GSR_N_ATT && h->nI == GSR_N_INSTR &&
-              ((h->nA == GSR_N_ASTRO && h->nG <= 1) || (h->nA == 0 && h->nG == 0));
+    h->lay = h->nA == GSR_N_ASTRO ? (h->nG == 1 ? 0 : h->nG == 0 ? 1 : 3) : 2;
+    h->prod = h->nAtt == GSR_N_ATT && h->nI == GSR_N_INSTR && (h->nA == GSR_N_ASTRO || (h->nA == 0 && h->nG == 0));
     if (L->n_obs < 0 || L->n_stars < 0 || (h->nA > 0 && L->n_stars < 1) || (h->nAtt > 0 && L->n_dof_att < 4) ||
         L->n_dof_att < 0 || L->n_instr < h->nI || L->n_con < 0 || L->n_con_nnz < 0 || (L->n_con == 0 && L->n_con_nnz != 0))
         return fail(h, GSR_EINVAL, "bad sizes");
@@ -334,7 +335,8 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
         // nInsSm instrument columns (as many as fit beside the static shared memory)
         int maxSm = 0;
         CK(cudaDeviceGetAttribute(&maxSm, cudaDevAttrMaxSharedMemoryPerBlockOptin, L->device));
-        const int64_t fit = (int64_t(maxSm) - 1024) / int64_t(sizeof(double));
+        // beside the static shared memory (lay 3: 4 KB of per-warp sums of the global columns)
+        const int64_t fit = (int64_t(maxSm) - 1024 - (h->lay == 3 ? 4096 : 0)) / int64_t(sizeof(double));
         h->nInsSm = int(std::max<int64_t>(0, std::min<int64_t>(L->n_instr, fit)));
         const int smB = int(h->nInsSm * sizeof(double));
         cudaError_t ea = cudaSuccess;

@@ -147,11 +147,13 @@ __device__ __forceinline__ double block_sum(double v, double *red)
 // coefficients too (k = 5..16).
 // NA (5 or 0 astrometric coefficients) and NG (1 or 0 global ones) select the layouts that share the specialised kernels:
 // 5/12/6/1 (production), 5/12/6/0 and 0/12/6/0 (the section subsets the paper's datasets solve).
+// NG = -1: any number of global columns (A.nG, up to MAX_GLOB; "future astrometric models will have more global
+// parameters"): their coefficients are not held in v but loaded where they are used, and the row width is
+// A.nPar.
 template <bool ATT, bool INS = true, int NA = N_ASTRO, int NG = 1>
-__device__ __forceinline__ void load_row(const double *__restrict__ V, int64_t tile, int lane, double (&v)[NA + N_ATT + N_INSTR + NG])
+__device__ __forceinline__ void load_row(const double *__restrict__ g, double (&v)[NA + N_ATT + N_INSTR + (NG > 0 ? NG : 0)])
 {
-    constexpr int NP = NA + N_ATT + N_INSTR + NG;
-    const double *g = V + tile * (NP * TILE) + lane;
+    constexpr int NP = NA + N_ATT + N_INSTR + (NG > 0 ? NG : 0);
 #pragma unroll
     for (int q = 0; q < NP; ++q) {
         const bool att = q >= NA && q < NA + N_ATT, ins = q >= NA + N_ATT && q < NA + N_ATT + N_INSTR;
@@ -211,8 +213,9 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
     const double cx = coef[0], cy = coef[1];
     const int64_t nTiles = (A.m + TILE - 1) / TILE;
     const double *xIns = x + A.offInstr;
-    const double xg = NG ? __ldg(x + A.offGlob) : 0.0;
-    constexpr int KT = NA, KI = NA + N_ATT, KG = NA + N_ATT + N_INSTR;
+    const double xg = NG > 0 ? __ldg(x + A.offGlob) : 0.0;
+    constexpr int KT = NA, KI = NA + N_ATT, KG = NA + N_ATT + N_INSTR, NGR = NG > 0 ? NG : 0;
+    const int np = NG < 0 ? A.nPar : KG + NG;   // stored coefficients per row
     double sq = 0.0;
     for (int64_t tile = int64_t(blockIdx.x) * WARPS + warp; tile < nTiles;
          tile += int64_t(gridDim.x) * WARPS) {
@@ -220,8 +223,9 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
         const int nrows = int(min(int64_t(TILE), A.m - r0));
         if (lane < nrows) {
             const int64_t i = r0 + lane;
-            double v[KG + NG];
-            load_row<true, true, NA, NG>(A.V, tile, lane, v);
+            double v[KG + NGR];
+            const double *g = A.V + tile * (int64_t(np) * TILE) + lane;
+            load_row<true, true, NA, NG>(g, v);
             const int64_t iatt = __ldcs(A.iatt + i);
             int32_t c[N_INSTR];
             load_ic<IC16>(A, tile, lane, c);
@@ -244,7 +248,9 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
             }
 #pragma unroll
             for (int j = 0; j < N_INSTR; ++j) sum = fma(v[KI + j], __ldg(xIns + c[j]), sum);
-            if (NG) sum = fma(v[NG ? KG : 0], xg, sum);
+            if (NG > 0) sum = fma(v[NG > 0 ? KG : 0], xg, sum);
+            if (NG < 0)
+                for (int q = 0; q < A.nG; ++q) sum = fma(__ldcs(g + (KG + q) * TILE), __ldg(x + A.offGlob + q), sum);
             const double yi = fma(cy, y[i], cx * sum);
             y[i] = yi;
             sq = fma(yi, yi, sq);
@@ -317,6 +323,7 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
          FuseArgs F = FuseArgs{nullptr, nullptr, nullptr, nullptr, nullptr, 0, 0})
 {
     __shared__ double red[32];
+    __shared__ double gAcc[NG < 0 ? 32 : 1][NG < 0 ? MAX_GLOB : 1];   // NG = -1: per-warp sums of the global columns
     extern __shared__ double sIns[];   // PRIV: nInsSm private instrument accumulators
     if (done && *done) return;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -335,8 +342,13 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
     }
     double gsum = 0.0, sq = 0.0;
     const double cx1 = FUSE ? F.coef1[0] : 0.0;
-    const double xg1 = FUSE && NG ? __ldg(F.xin + A.offGlob) : 0.0;
-    constexpr int KT = NA, KI = NA + N_ATT, KG = NA + N_ATT + N_INSTR, NP = KG + NG;
+    const double xg1 = FUSE && NG > 0 ? __ldg(F.xin + A.offGlob) : 0.0;
+    constexpr int KT = NA, KI = NA + N_ATT, KG = NA + N_ATT + N_INSTR, NP = KG + (NG > 0 ? NG : 0);
+    const int np = NG < 0 ? A.nPar : NP;   // stored coefficients per row
+    if (NG < 0) {
+        if (lane < MAX_GLOB) gAcc[warp][lane] = 0.0;
+        __syncwarp();
+    }
     for (int64_t tile = int64_t(blockIdx.x) * nWarpsCta + warp; tile < nTiles;
          tile += int64_t(gridDim.x) * nWarpsCta) {
         const int64_t r0 = tile * TILE;
@@ -344,7 +356,8 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         const bool valid = lane < nrows;
         const int64_t i = r0 + (valid ? lane : nrows - 1);
         double v[NP];
-        load_row<ATT_RED || FUSE_ATT, INS || FUSE, NA, NG>(A.V, tile, valid ? lane : nrows - 1, v);
+        const double *g = A.V + tile * (int64_t(np) * TILE) + (valid ? lane : nrows - 1);
+        load_row<ATT_RED || FUSE_ATT, INS || FUSE, NA, NG>(g, v);
         const unsigned long long tw = NA ? __ldg(A.tw + tile) : 0ull;   // one 8-byte word per tile: first star, head mask, cut flags
         const int64_t ia = NA ? NA * star_of(A, tw, i, valid ? lane : nrows - 1) : 0;
         // padded storage: the lanes past the last row read column 0 and a zero coefficient
@@ -365,7 +378,9 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
                     const double xj = F.texX ? tex_f64(F.texX, A.offInstr + c[j]) : __ldg(xIn + c[j]);
                     sum = fma(v[KI + j], xj, sum);
                 }
-                if (NG) sum = fma(v[NG ? KG : 0], xg1, sum);
+                if (NG > 0) sum = fma(v[NG > 0 ? KG : 0], xg1, sum);
+                if (NG < 0)
+                    for (int q = 0; q < A.nG; ++q) sum = fma(__ldg(g + (KG + q) * TILE), __ldg(F.xin + A.offGlob + q), sum);
                 double yOld = F.yrw[i];
                 if (FUSE_ATT) {
                     const int64_t iattRow = __ldcs(A.iatt + i);
@@ -428,7 +443,14 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
             }
         }
         // ---- gamma: fixed-order warp sum, accumulated per warp over its tiles
-        if (NG) gsum += warp_sum(v[NG ? KG : 0]);
+        if (NG > 0) gsum += warp_sum(v[NG > 0 ? KG : 0]);
+        if (NG < 0) {   // every global column: fixed-order warp sum into this warp's accumulator (lanes past the last row: yv = 0)
+            for (int q = 0; q < A.nG; ++q) {
+                const double a = __ldg(g + (KG + q) * TILE);
+                const double t = warp_sum(SQUARE ? a * a * yv : a * yv);
+                if (lane == 0) gAcc[warp][q] += t;
+            }
+        }
 
         // ---- astro: segmented scan by star over the tile's rows
         if (NA == 0) continue;
@@ -467,10 +489,15 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
     __syncthreads();
     if (lane == 0) red[warp] = gsum;
     __syncthreads();
-    if (NG && threadIdx.x == 0) {
+    if (NG > 0 && threadIdx.x == 0) {
         double g = 0.0;
         for (int w = 0; w < nWarpsCta; ++w) g += red[w];
         globPartial[blockIdx.x] = g;
+    }
+    if (NG < 0 && threadIdx.x < A.nG) {   // globPartial[q*gridDim.x + blockIdx.x]: this CTA's share of global column q
+        double g = 0.0;
+        for (int w = 0; w < nWarpsCta; ++w) g += gAcc[w][threadIdx.x];
+        globPartial[int64_t(threadIdx.x) * gridDim.x + blockIdx.x] = g;
     }
     if (FUSE) {
         const double b = block_sum(sq, red);
@@ -496,11 +523,12 @@ k_astro_fixup(MatView A, double *__restrict__ x, const double *__restrict__ coef
     const double cx = coef[0];
     const int starBlocks = A.nA > 0 ? int((A.nStars + blockDim.x - 1) / blockDim.x) : 0;
     if (blockIdx.x == gridDim.x - 1) {
-        if (A.nG == 0) return;
-        double g = 0.0;
-        for (int p = threadIdx.x; p < nGlobPartial; p += blockDim.x) g += globPartial[p];
-        g = block_sum(g, red);
-        if (threadIdx.x == 0) x[A.offGlob] += g;   // section already scaled by cx
+        for (int q = 0; q < A.nG; ++q) {
+            double g = 0.0;
+            for (int p = threadIdx.x; p < nGlobPartial; p += blockDim.x) g += globPartial[int64_t(q) * nGlobPartial + p];
+            g = block_sum(g, red);
+            if (threadIdx.x == 0) x[A.offGlob + q] += g;   // section already scaled by cx
+        }
         return;
     }
     if (blockIdx.x >= starBlocks) {

@@ -667,9 +667,9 @@ def test_model_variants_aprod_and_precondition(widths, shape):
     with make_gpu(S, d, b) as G:
         assert G.n == S.n == cfg.n and G.m_tot == S.m_tot
         info = G.gsr_path_info()
-        # 5/12/6/0 and 0/12/6/0 (the section subsets of the paper's datasets) share the specialised kernels and the fused
-        # iteration with the production layout; the other layouts run the general kernels
-        assert bool(info & gsr_mod().GSR_PATH_FUSED) == (widths in ((5, 12, 6, 0), (0, 12, 6, 0)))
+        # 5/12/6/N_Glob and 0/12/6/0 (the section subsets of the paper's datasets, any number of global columns) share the
+        # specialised kernels and the fused iteration with the production layout; the other layouts run the general kernels
+        assert bool(info & gsr_mod().GSR_PATH_FUSED) == (widths[:3] == (5, 12, 6) or widths == (0, 12, 6, 0))
         assert bool(info & gsr_mod().GSR_PATH_ATT_COPY) == (widths[1] == 12)   # the attitude kernel serves every layout
         if widths[0]:
             rp = G.gsr_get_star_rowptr().cpu().numpy()
@@ -705,7 +705,7 @@ def test_model_variants_lsqr(widths):
 
 
 @pytest.mark.parametrize("flag", ["NO_FUSE", "NO_TEX"])
-@pytest.mark.parametrize("widths", [(5, 12, 6, 0), (0, 12, 6, 0)])
+@pytest.mark.parametrize("widths", [(5, 12, 6, 0), (0, 12, 6, 0), (5, 12, 6, 5), (5, 12, 6, 16)])
 def test_fast_variant_layouts_fallback_paths(widths, flag):
     """The two non-production layouts that run the specialised kernels, in the two-product form and without textures."""
     gsr = gsr_mod()
@@ -746,17 +746,19 @@ def test_model_variants_without_attitude_copy(widths):
 
 
 def test_model_variants_global_columns_bit_reproducible():
-    """Every global column is reduced in a fixed order (warp -> CTA -> one block), as gamma is in production."""
-    cfg = variant_cfg((3, 12, 4, 5), "multi_cta")
-    S, d = oracle_system(cfg)
-    b = make_b(S, d)
-    with make_gpu(S, d, b) as G:
-        y = torch.from_numpy(np.random.default_rng(0).standard_normal(S.m_tot)).cuda()
-        outs = [G.gsr_aprod2(y, torch.zeros(S.n, dtype=torch.float64, device="cuda")).cpu().numpy() for _ in range(3)]
-        na = 3 * cfg.n_stars
-        for o in outs[1:]:
-            assert np.array_equal(o[:na], outs[0][:na])
-            assert np.array_equal(o[-5:], outs[0][-5:])
+    """Every global column is reduced in a fixed order (warp -> CTA -> one block), as gamma is in production: in the
+    general kernels (3/12/4/5) and in the specialised ones (5/12/6/5)."""
+    for widths in ((3, 12, 4, 5), (5, 12, 6, 5)):
+        cfg = variant_cfg(widths, "multi_cta")
+        S, d = oracle_system(cfg)
+        b = make_b(S, d)
+        with make_gpu(S, d, b) as G:
+            y = torch.from_numpy(np.random.default_rng(0).standard_normal(S.m_tot)).cuda()
+            outs = [G.gsr_aprod2(y, torch.zeros(S.n, dtype=torch.float64, device="cuda")).cpu().numpy() for _ in range(3)]
+            na = widths[0] * cfg.n_stars
+            for o in outs[1:]:
+                assert np.array_equal(o[:na], outs[0][:na])
+                assert np.array_equal(o[-5:], outs[0][-5:])
 
 
 def test_layout_width_validation():
