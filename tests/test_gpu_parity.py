@@ -371,7 +371,7 @@ def test_two_attitude_blocks_and_mixed_instrument_table(ins_copy):
         assert np.linalg.norm(xg - ro.x) <= X_TOL * np.linalg.norm(ro.x)
 
 
-def stream_oracle_aprods(cfg, G, x, y, y1, x2, chunk_stars, threads=8):
+def stream_oracle_aprods(cfg, G, x, y, y1, x2, chunk_stars, threads=8, x_extra=None, ab_extra=None):
     """Chunk-streamed oracle over a system that exists only on the device: the rows of `chunk_stars`
     stars at a time are regenerated on the device (same seeded generator, same bytes as the upload), copied to the
     host and handed to oracle/gsr_oracle.c.  aprod1 is row-local: every row of y1 = A x is compared; aprod2
@@ -418,6 +418,9 @@ def stream_oracle_aprods(cfg, G, x, y, y1, x2, chunk_stars, threads=8):
             drain(threads)
         drain(0)
     assert rows_checked == y1.shape[0]
+    if x_extra is not None:     # contribution of rows the caller ran through the oracle itself (constraint rows)
+        x_ref += x_extra
+        ab_ref += ab_extra
     xg = x2.cpu().numpy()
     err2 = np.abs(xg - x_ref) / (ab_ref + 1e-300)
     return worst1, err2
@@ -454,6 +457,42 @@ def test_medium_full_size_every_element():
         worst = {k: float(v.max()) for k, v in sect.items()}
         assert all(w <= APROD_TOL for w in worst.values()), worst
         print(f"medium every element: aprod1 worst {worst1:.2e}, aprod2 worst by section {worst} (x 1e-12 bound)")
+
+
+def test_large_full_size_every_element():
+    """BASELINE configs[4] at full size (500 M rows + 10,000 constraint rows x 1,000 non-zeros, ~170 GB resident) in the
+    launch configuration bench.py times: every output of aprod1 (observation and constraint rows) and every output of
+    aprod2 against the chunk-streamed oracle ("oracle parity on aprod only, chunk-streamed")."""
+    import bench
+    gsr = gsr_mod()
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    if free < 183e9:
+        pytest.skip("needs a whole 180 GB B200")
+    cfg = synth.large()
+    dv = torch.device("cuda", 0)
+    m = int(synth.star_rowptr(cfg)[-1])
+    with gsr.Gsr(m, cfg.n_stars, cfg.n_dof_att, cfg.n_instr, cfg.n_con, cfg.n_con * cfg.con_nnz) as G:
+        bench.build_on_device(cfg, G, dv, torch, synth)
+        assert G.gsr_path_info() & gsr.GSR_PATH_IC16
+        g = torch.Generator(device="cuda").manual_seed(6)
+        x = torch.randn(G.n, dtype=torch.float64, device=dv, generator=g)
+        y = torch.randn(G.m_tot, dtype=torch.float64, device=dv, generator=g)
+        y1 = G.gsr_aprod1(x, torch.zeros(G.m_tot, dtype=torch.float64, device=dv))
+        x2 = G.gsr_aprod2(y, torch.zeros(G.n, dtype=torch.float64, device=dv))
+        # constraint rows alone through the oracle (an oracle system without observation rows)
+        rp, cc, cv = (t.cpu().numpy() for t in synth.constraints(cfg, dv))
+        e = np.zeros((0, 24))
+        Sc = oracle.OracleSystem(cfg.n_stars, cfg.n_dof_att, cfg.n_instr, e, np.zeros(0, np.int64), np.zeros(0, np.int64),
+                                 np.zeros((0, 6), np.int32), rp, cc, cv)
+        xc = x.cpu().numpy()
+        yc, abc = Sc.aprod1(xc, np.zeros(cfg.n_con), want_abs=True)
+        assert np.all(np.abs(y1[m:].cpu().numpy() - yc) <= APROD_TOL * abc)
+        x2c, ab2c = Sc.aprod2(y[m:].cpu().numpy(), np.zeros(G.n), want_abs=True)
+        # observation rows, chunk by chunk; the constraint rows' share of A^T y and of its bound is added to the reference
+        worst1, err2 = stream_oracle_aprods(cfg, G, x, y[:m], y1[:m], x2, chunk_stars=10_000, x_extra=x2c, ab_extra=ab2c)
+        assert float(err2.max()) <= APROD_TOL, float(err2.max())
+        print(f"large every element: aprod1 worst {worst1:.2e}, aprod2 worst {float(err2.max()):.2e} (x 1e-12 bound)")
 
 
 def test_small_config_lsqr():
