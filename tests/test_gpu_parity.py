@@ -495,6 +495,28 @@ def test_large_full_size_every_element():
         print(f"large every element: aprod1 worst {worst1:.2e}, aprod2 worst {float(err2.max()):.2e} (x 1e-12 bound)")
 
 
+def test_skewed_full_size_every_element():
+    """BASELINE configs[3] at full size (literal alpha = 2: 53 M rows, power-law rows per star, bursty attitude starts, 60,000
+    Zipf columns: the MATCH variant, global REDs and the shared-memory table together): every output of both products
+    against the chunk-streamed oracle."""
+    import bench
+    gsr = gsr_mod()
+    cfg = synth.skewed()
+    dv = torch.device("cuda", 0)
+    m = int(synth.star_rowptr(cfg)[-1])
+    with gsr.Gsr(m, cfg.n_stars, cfg.n_dof_att, cfg.n_instr) as G:
+        bench.build_on_device(cfg, G, dv, torch, synth)
+        assert G.gsr_path_info() & gsr.GSR_PATH_INSTR_MATCH
+        g = torch.Generator(device="cuda").manual_seed(7)
+        x = torch.randn(G.n, dtype=torch.float64, device=dv, generator=g)
+        y = torch.randn(m, dtype=torch.float64, device=dv, generator=g)
+        y1 = G.gsr_aprod1(x, torch.zeros(m, dtype=torch.float64, device=dv))
+        x2 = G.gsr_aprod2(y, torch.zeros(G.n, dtype=torch.float64, device=dv))
+        worst1, err2 = stream_oracle_aprods(cfg, G, x, y, y1, x2, chunk_stars=20_000)
+        assert float(err2.max()) <= APROD_TOL, float(err2.max())
+        print(f"skewed every element: aprod1 worst {worst1:.2e}, aprod2 worst {float(err2.max()):.2e} (x 1e-12 bound)")
+
+
 def test_small_config_lsqr():
     """BASELINE configs[1] (20 M rows; SURVEY 8(d) asks for full parity on Small): gsr_lsqr against the oracle's LSQR on
     the same bytes.  The preconditioned system reaches the rounding floor near iteration 40 (1 + test2 <= 1, istop 5),
