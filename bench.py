@@ -7,8 +7,12 @@ configs[2] "medium" (1M stars x 200 obs = 200M rows, 46.4 GB), the config the me
 target is quoted on.  Inputs are seeded and synthetic (paper_2308_00778_b200.synth); the paper's
 Gaia datasets are proprietary.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload medium|small|tiny|skewed]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload medium|small|tiny|skewed|large]
+                  [--skew-alpha 1.47] [--rerun 2] [--layout NA,NT,NI,NG]
   python bench.py --impl reference ...     # the CPU oracle, as it stands, on a bounded sample
+
+K iterations are timed as solves of at most 20 iterations of the same system (the synthetic systems reach the rounding
+floor, istop 5, after ~31 iterations at Medium); the timed quantity is the device time of the iteration loops.
 
 N > 1: the path does not shard in this build (north_star: one GPU, no collectives), so N ranks run
 N independent replicas ("replicas only") and `value` is their aggregate.
