@@ -517,6 +517,32 @@ def test_skewed_full_size_every_element():
         print(f"skewed every element: aprod1 worst {worst1:.2e}, aprod2 worst {float(err2.max()):.2e} (x 1e-12 bound)")
 
 
+@pytest.mark.parametrize("n_instr", [65_536, 65_537])
+def test_instrument_column_width_boundary(n_instr):
+    """65,536 columns still fit 2 bytes (the last column is 65,535), 65,537 do not: 4-byte columns, and the opt-in
+    column-ordered copy is silently not built.  Both with and without GSR_FLAG_INS_COPY."""
+    gsr = gsr_mod()
+    cfg = synth.SynthConfig("edge", 600, 500, n_instr, obs_per_star=30, seed=41)
+    S, d = oracle_system(cfg)
+    for i in (5, 777, 17_999):                   # make sure the last column is in use (the rows keep 6 distinct columns)
+        assert n_instr - 1 not in d["instrCol"][i]
+        d["instrCol"][i, 3] = n_instr - 1
+    S, _ = oracle_system(cfg, d)
+    b = make_b(S, d)
+    for flags in (0, gsr.GSR_FLAG_INS_COPY):
+        with make_gpu(S, d, b, flags=flags) as G:
+            info = G.gsr_path_info()
+            assert bool(info & gsr.GSR_PATH_IC16) == (n_instr <= 65_536)
+            assert bool(info & gsr.GSR_PATH_INS_COPY) == (flags != 0 and n_instr <= 65_536)
+            check_aprods(S, G, seed=8)
+            G.gsr_precondition()
+    S.precondition()
+    with make_gpu(S, {**d, "values": S.V}, b, flags=gsr.GSR_FLAG_INS_COPY) as G:   # the preconditioned matrix through LSQR
+        r = G.gsr_lsqr(15, 0.0, 0.0)
+        ro = S.lsqr(b, 15, 0.0, 0.0)
+        assert rel(r.x.cpu().numpy() * S.p, ro.x) <= X_TOL
+
+
 def test_small_config_lsqr():
     """BASELINE configs[1] (20 M rows; SURVEY 8(d) asks for full parity on Small): gsr_lsqr against the oracle's LSQR on
     the same bytes.  The preconditioned system reaches the rounding floor near iteration 40 (1 + test2 <= 1, istop 5),
