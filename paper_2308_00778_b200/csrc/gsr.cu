@@ -67,7 +67,7 @@ struct gsr_handle {
     double *attT = nullptr, *insRep = nullptr;
     int32_t *sT = nullptr;
     uint32_t *permT = nullptr;
-    int nRep = 1, gridAtt = 1, perIter = 0, nInsSm = 0;
+    int nRep = 1, gridAtt = 1, gridAttLin = 1, perIter = 0, nInsSm = 0;
     bool useAttT = false;
     bool instrSkewed = false;   // some instrument column holds > 64x the mean number of coefficients
     // column-ordered copy of the instrumental section (k_ins_scatter): +72 B/row; built by gsr_upload_finish when it fits
@@ -358,8 +358,11 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     // fix-up grid: one thread per star, then one per instrument column (replica fold), then gamma
     h->gridFix = (h->nA > 0 ? int((L->n_stars + 255) / 256) : 0) + int((L->n_instr + 255) / 256) + 1;
     if (!h->prod) h->gridFix = (h->nA > 0 ? int((L->n_stars + 255) / 256) : 0) + 1;   // k_fixup_gen: stars, then the global columns
+    // CTAs per SM from A/B runs of the whole iteration at Medium: the attitude kernel that gathers y needs 58
+    // registers (4 CTAs of 256 threads fit), the one that streams uT 46 (5 fit: one full wave; 6 would start a second)
     h->gridAtt = gridFor(h->nTiles, 8, h->smCount * 4);
-    h->gridUT = gridFor(L->n_obs, 256, h->smCount * 4);
+    h->gridAttLin = gridFor(h->nTiles, 8, h->smCount * 5);
+    h->gridUT = gridFor(L->n_obs, 256, h->smCount * 6);
     // instrument replicas: spread the REDs of aprod2 over >= ~512k distinct addresses
     h->nRep = int(std::max<int64_t>(1, std::min<int64_t>(128, (524288 + L->n_instr - 1) / std::max<int64_t>(L->n_instr, 1))));
 
@@ -706,7 +709,7 @@ int readyCheck(gsr_handle *h)
 void launchAtt(gsr_handle *h, const MatView &A, const double *y, double *x, const double *coef, const int *done,
                bool linear = false)
 {
-    if (linear) k_aprod2_att<false, true><<<h->gridAtt, 256, 0, h->stream>>>(A, y, x, coef, done);
+    if (linear) k_aprod2_att<false, true><<<h->gridAttLin, 256, 0, h->stream>>>(A, y, x, coef, done);
     else k_aprod2_att<false, false><<<h->gridAtt, 256, 0, h->stream>>>(A, y, x, coef, done);
 }
 
@@ -1147,7 +1150,7 @@ int32_t gsr_bench_set(gsr_handle *h, const char *key, int64_t value)
     const std::string k(key);
     if (k == "ins_sm_fused" && value >= 0 && value <= h->nInsSm) h->nInsSmFused = int(value);
     else if (k == "n_rep" && value >= 1 && value <= h->nRepAlloc) h->nRep = int(value);
-    else if (k == "att_ctas_per_sm" && value >= 1 && value <= 16) h->gridAtt = gridFor(h->nTiles, 8, h->smCount * int(value));
+    else if (k == "att_ctas_per_sm" && value >= 1 && value <= 16) h->gridAtt = h->gridAttLin = gridFor(h->nTiles, 8, h->smCount * int(value));
     else if (k == "fused_nopriv" && (value == 0 || value == 1)) h->fusedNoPriv = value != 0;
     else if (k == "a2_ctas_per_sm" && value >= 1 && value <= 2) h->gridA2 = gridFor(h->nTiles, WARPS, h->smCount * int(value));
     else if (k == "use_ut" && (value == 0 || (value == 1 && h->uT))) h->useUT = value != 0;
@@ -1228,7 +1231,7 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
         for (int r = 0; r < reps; ++r) {
             launchAprod2Main<true>(h, Af, h->u, h->t, h->coefRaw, nullptr, F);
             k_u_to_time<<<h->gridUT, 256, 0, h->stream2>>>(h->u, h->permT, A.m, h->uT, nullptr);
-            k_aprod2_att<false, true><<<h->gridAtt, 256, 0, h->stream2>>>(A, h->uT, h->v, h->coefTime, nullptr);
+            k_aprod2_att<false, true><<<h->gridAttLin, 256, 0, h->stream2>>>(A, h->uT, h->v, h->coefTime, nullptr);
         }
         CK(cudaEventRecord(h->evJoin, h->stream2));
         CK(cudaStreamWaitEvent(st, h->evJoin, 0));
