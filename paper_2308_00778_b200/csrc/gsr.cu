@@ -401,7 +401,7 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(dalloc(&h->trace, 5 * GSR_TRACE_CAP));
     CK(dalloc(&h->S, 1));
     CK(dalloc(&h->badDev, 1));
-    h->nRepAlloc = h->nRep;
+    h->nRepAlloc = std::max(h->nRep, 64);   // room for the replica sweep of gsr_bench_set
     // k_ins_scatter: buckets of <= INS_BUCKET_MAX columns, two CTAs per SM shared out over the buckets; every CTA owns a
     // slice of insRep
     h->insNB = int(std::max<int64_t>(1, (L->n_instr + INS_BUCKET_MAX - 1) / INS_BUCKET_MAX));
@@ -409,7 +409,7 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     h->insNG = std::max(1, h->smCount / h->insNB);
     CK(cudaFuncSetAttribute(k_ins_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize,
                             int((h->insW + 2 * INS_BLOCK) * sizeof(double))));
-    CK(dalloc(&h->insRep, int64_t(std::max(h->nRep, h->insNG)) * L->n_instr));
+    CK(dalloc(&h->insRep, int64_t(std::max(h->nRepAlloc, h->insNG)) * L->n_instr));
     CK(dalloc(&h->u, h->mTot));
     CK(dalloc(&h->v, h->n));
     CK(dalloc(&h->w, h->n));
