@@ -726,7 +726,9 @@ void launchAprod1(gsr_handle *h, const MatView &A, const double *x, double *y, c
 template <bool SQUARE>
 void launchAprod2Red(gsr_handle *h, const MatView &A, const double *y, double *x, const double *coef, const int *done)
 {
-    if (!h->prod)
+    if (!h->prod && h->nA > 0 && h->nAtt == 0 && h->nI == 0 && h->nG == 0)   // astrometric-only layout
+        k_aprod2_astro<SQUARE><<<h->gridA2, THREADS, 0, h->stream>>>(A, y, x, coef, h->carryFirst, h->carryLast, done);
+    else if (!h->prod)
         k_aprod2_gen<SQUARE><<<h->gridA2, THREADS, 0, h->stream>>>(A, y, x, coef, h->carryFirst, h->carryLast,
                                                                   h->globPartial, done);
     else if (h->ic16)

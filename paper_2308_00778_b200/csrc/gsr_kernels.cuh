@@ -126,6 +126,31 @@ __device__ __forceinline__ double warp_sum(double v)
     return v;
 }
 
+// Totals of up to 5 per-lane values over the 32 lanes of a warp with 9 shuffles instead of 5 x 5 (the values are
+// handed round while they are summed: 4 + 2 + 1 exchanges, then two plain butterfly steps).  Afterwards lane 4k holds
+// the total of value k; the tree is fixed, so the result is reproducible.
+__device__ __forceinline__ double warp_sum5(const double (&s)[5], int lane)
+{
+    const bool h16 = lane & 16, h8 = lane & 8, h4 = lane & 4;
+    double a[4], b[2];
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const double lo = s[j], hi = j == 0 ? s[4] : 0.0;   // values 5..7 do not exist
+        const double recv = __shfl_xor_sync(0xffffffffu, h16 ? lo : hi, 16);
+        a[j] = (h16 ? hi : lo) + recv;
+    }
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+        const double recv = __shfl_xor_sync(0xffffffffu, h8 ? a[j] : a[2 + j], 8);
+        b[j] = (h8 ? a[2 + j] : a[j]) + recv;
+    }
+    const double recv = __shfl_xor_sync(0xffffffffu, h4 ? b[0] : b[1], 4);
+    double c = (h4 ? b[1] : b[0]) + recv;
+    c += __shfl_xor_sync(0xffffffffu, c, 2);
+    c += __shfl_xor_sync(0xffffffffu, c, 1);
+    return c;
+}
+
 // Deterministic block sum (fixed tree); result valid in thread 0.  red: >= 32 doubles of smem.
 __device__ __forceinline__ double block_sum(double v, double *red)
 {
@@ -455,6 +480,19 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
         // ---- astro: segmented scan by star over the tile's rows
         if (NA == 0) continue;
         const unsigned heads = uint32_t(tw) | 1u;          // segment starts inside the tile (lane 0 always opens one)
+        if (heads == 1u) {   // the whole tile belongs to one star (the common case): totals instead of a scan
+            double s5[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+            for (int k = 0; k < NA; ++k) s5[k] = v[k];
+            const double tot = warp_sum5(s5, lane);
+            const int k = (lane >> 2) & 7;   // lane 4k holds value k
+            if ((lane & 3) == 0 && k < NA) {
+                // the star began in an earlier tile and / or goes on in the next one: the fix-up adds the pieces
+                if (!(uint32_t(tw) & 1u) || ((tw >> 61) & 1ull)) carryFirst[tile * N_ASTRO + k] = tot;
+                else x[ia + k] = fma(cx, x[ia + k], tot);
+            }
+            continue;
+        }
         const bool tail = valid && ((lane == nrows - 1) || ((heads >> 1) >> lane) & 1u);
         const int segStart = 31 - __clz(heads & (0xffffffffu >> (31 - lane)));
         const int dist = lane - segStart;
@@ -1073,6 +1111,75 @@ k_aprod2_gen(MatView A, const double *__restrict__ y, double *__restrict__ x, co
         double t = 0.0;
         for (int w = 0; w < WARPS; ++w) t += gAcc[w][threadIdx.x];
         globPartial[int64_t(threadIdx.x) * gridDim.x + blockIdx.x] = t;
+    }
+}
+
+// Astrometric-only layouts (N_Att = N_Instr = N_Glob = 0: the paper's 100 GB dataset "solves the astrometric part",
+// PAPER.md:263): the N_Astro <= 5 coefficients of a row are loaded together (predicated on the width, which is uniform over
+// the grid) and scanned side by side, instead of one after the other as in k_aprod2_gen (Medium-sized system: 4.1 -> see
+// DESIGN.md 5).  Same carries, same fix-up (k_fixup_gen).
+template <bool SQUARE>
+__global__ void __launch_bounds__(THREADS)
+k_aprod2_astro(MatView A, const double *__restrict__ y, double *__restrict__ x, const double *__restrict__ coef,
+               double *__restrict__ carryFirst, double *__restrict__ carryLast, const int *done)
+{
+    if (done && *done) return;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const double cx = coef[0], cy = coef[1];
+    const int64_t nTiles = (A.m + TILE - 1) / TILE;
+    const int nA = A.nA;
+    for (int64_t tile = int64_t(blockIdx.x) * WARPS + warp; tile < nTiles; tile += int64_t(gridDim.x) * WARPS) {
+        const int64_t r0 = tile * TILE;
+        const int nrows = int(min(int64_t(TILE), A.m - r0));
+        const bool valid = lane < nrows;
+        const int ln = valid ? lane : nrows - 1;
+        const int64_t i = r0 + ln;
+        const double *g = A.V + tile * (int64_t(A.nPar) * TILE) + ln;
+        const double yv = valid ? (SQUARE ? 1.0 : cy * y[i]) : 0.0;     // lanes past the last row add zeros
+        double s[N_ASTRO];
+#pragma unroll
+        for (int k = 0; k < N_ASTRO; ++k) {
+            const double a = k < nA ? __ldcs(g + k * TILE) : 0.0;
+            s[k] = SQUARE ? a * a * yv : a * yv;
+        }
+        const unsigned long long tw = __ldg(A.tw + tile);
+        const int64_t ia = nA * star_of(A, tw, i, ln);
+        GSR_ASSERT(ia >= 0 && ia + nA <= A.offAtt);
+        const unsigned heads = uint32_t(tw) | 1u;
+        if (heads == 1u) {   // one star in the whole tile: totals instead of a scan (see k_aprod2)
+            const double tot = warp_sum5(s, lane);
+            const int k = (lane >> 2) & 7;
+            if ((lane & 3) == 0 && k < nA) {
+                if (!(uint32_t(tw) & 1u) || ((tw >> 61) & 1ull)) carryFirst[tile * N_ASTRO + k] = tot;
+                else x[ia + k] = fma(cx, x[ia + k], tot);
+            }
+            continue;
+        }
+        const bool tail = valid && ((lane == nrows - 1) || ((heads >> 1) >> lane) & 1u);
+        const int segStart = 31 - __clz(heads & (0xffffffffu >> (31 - lane)));
+        const int dist = lane - segStart;
+        bool cut = false;
+        if (segStart == 0) cut = !(uint32_t(tw) & 1u);
+        if (lane == nrows - 1) cut = cut || ((tw >> 61) & 1ull);
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+#pragma unroll
+            for (int k = 0; k < N_ASTRO; ++k) {
+                if (k < nA) {   // uniform over the grid
+                    const double t = __shfl_up_sync(0xffffffffu, s[k], d);
+                    if (dist >= d) s[k] += t;
+                }
+            }
+        }
+        if (tail) {
+#pragma unroll
+            for (int k = 0; k < N_ASTRO; ++k) {
+                if (k < nA) {
+                    if (!cut) x[ia + k] = fma(cx, x[ia + k], s[k]);
+                    else (segStart == 0 ? carryFirst : carryLast)[tile * N_ASTRO + k] = s[k];
+                }
+            }
+        }
     }
 }
 
