@@ -468,7 +468,7 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
             }
         }
         // ---- gamma: fixed-order warp sum, accumulated per warp over its tiles
-        if (NG > 0) gsum += warp_sum(v[NG > 0 ? KG : 0]);
+        if (NG > 0) gsum += v[NG > 0 ? KG : 0];   // per lane over its tiles; the lanes are summed once, after the loop
         if (NG < 0) {   // every global column: fixed-order warp sum into this warp's accumulator (lanes past the last row: yv = 0)
             for (int q = 0; q < A.nG; ++q) {
                 const double a = __ldg(g + (KG + q) * TILE);
@@ -523,7 +523,9 @@ k_aprod2(MatView A, const double *__restrict__ y, double *__restrict__ x,
             }
         }
     }
-    // CTA partial of gamma in fixed order (lane 0 of each warp holds its running sum)
+    // CTA partial of gamma in fixed order: every lane summed its own rows in tile order, then a fixed tree over the lanes and
+    // the warps in order
+    if (NG > 0) gsum = warp_sum(gsum);
     __syncthreads();
     if (lane == 0) red[warp] = gsum;
     __syncthreads();
