@@ -54,7 +54,8 @@ struct gsr_handle {
     double *carryFirst = nullptr, *carryLast = nullptr, *globPartial = nullptr;
     double *sqPartialU = nullptr, *sqPartialV = nullptr, *ddPartial = nullptr;
     double *coefOne = nullptr, *coefTime = nullptr, *trace = nullptr;
-    double *xPack = nullptr;   // attitude unknowns of the current aprod1 operand, [s][axis]
+    double *xPack = nullptr;   // attitude unknowns of the operand of the fused pass, [s][axis]
+    double *xPack4 = nullptr;  // the same four wide (one 32-byte sector per start) for the standalone k_aprod1
     double *t = nullptr;       // fused iteration: unscaled A^T u' (n doubles)
     double *coefRaw = nullptr; // {0, 1}: "x <- 0*x + 1*(A^T y)"
     int nInsSmFused = 0;       // columns of the shared-memory table in the fused main kernel
@@ -396,6 +397,7 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(dalloc(&h->sqPartialV, h->gridVec));
     CK(dalloc(&h->ddPartial, h->gridVec));
     CK(dalloc(&h->xPack, 3 * L->n_dof_att));
+    CK(dalloc(&h->xPack4, 4 * L->n_dof_att));
     CK(dalloc(&h->coefOne, 2));
     CK(dalloc(&h->coefTime, 2));
     CK(dalloc(&h->trace, 5 * GSR_TRACE_CAP));
@@ -486,7 +488,7 @@ int32_t gsr_destroy(gsr_handle *h)
     void *ptrs[] = {h->V, h->b, h->conVal, h->p, h->star, h->iatt, h->stageI, h->rp, h->conRp, h->conCol, h->ic, h->ic16, h->tw,
                     h->u, h->v, h->w, h->z, h->var, h->carryFirst, h->carryLast, h->globPartial,
                     h->sqPartialU, h->sqPartialV, h->ddPartial, h->coefOne, h->coefTime, h->trace,
-                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC, h->xPack, h->t, h->coefRaw, h->uT, h->insVal, h->insMeta, h->insPtr};
+                    h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC, h->xPack, h->xPack4, h->t, h->coefRaw, h->uT, h->insVal, h->insMeta, h->insPtr};
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (h->hostS) cudaFreeHost(h->hostS);
@@ -718,8 +720,8 @@ void launchAprod1(gsr_handle *h, const MatView &A, const double *x, double *y, c
                   const int *done)
 {
     if (!h->prod) k_aprod1_gen<<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done);
-    else if (h->ic16) GSR_LAY(h, (k_aprod1<true, NA_, NG_><<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done, h->xPack)))
-    else GSR_LAY(h, (k_aprod1<false, NA_, NG_><<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done, h->xPack)))
+    else if (h->ic16) GSR_LAY(h, (k_aprod1<true, NA_, NG_><<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done, h->xPack4)))
+    else GSR_LAY(h, (k_aprod1<false, NA_, NG_><<<h->gridA1, THREADS, 0, h->stream>>>(A, x, y, coef, sq, done, h->xPack4)))
 }
 
 // all sections in one kernel, attitude by REDs (preconditioner pass; low-memory path)
@@ -786,7 +788,7 @@ int enqueueAprod1(gsr_handle *h, const double *x, double *y, const double *coef,
     MatView A = view(h);
     int nk = 1, np = h->gridA1;
     if (h->prod) {   // the specialised kernel gathers the attitude unknowns from their axis-interleaved copy
-        k_pack_att<<<h->gridVec, 256, 0, h->stream>>>(A, x, h->xPack, done);
+        k_pack_att4<<<h->gridVec, 256, 0, h->stream>>>(A, x, h->xPack4, done);
         ++nk;
     }
     launchAprod1(h, A, x, y, coef, sqPartial, done);
@@ -1186,7 +1188,10 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
     // bounded operands: u = b, v = 1e-3; coefficients 0.5 keep repeated products finite
     CK(cudaMemcpyAsync(h->u, h->b, size_t(h->mTot) * sizeof(double), cudaMemcpyDeviceToDevice, st));
     k_fill<<<h->gridVec, 256, 0, st>>>(h->v, h->n, 1e-3);
-    if (h->prod) k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, nullptr);   // operand of k_aprod1 / the fused pass timed alone
+    if (h->prod) {   // operands of k_aprod1 / the fused pass timed alone
+        k_pack_att<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack, nullptr);
+        k_pack_att4<<<h->gridVec, 256, 0, st>>>(A, h->v, h->xPack4, nullptr);
+    }
     k_pre_aprod2<<<h->gridVec, 256, 0, st>>>(h->t, 0, A.n, h->coefRaw, h->insRep, int64_t(h->nRep) * A.nInstr, 2, nullptr);
     auto once = [&]() {
         if (which == GSR_TIME_APROD1_GROUP) enqueueAprod1(h, h->v, h->u, h->coefTime, h->sqPartialU, nullptr, nullptr);

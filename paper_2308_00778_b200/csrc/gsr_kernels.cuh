@@ -210,7 +210,7 @@ __device__ __forceinline__ int32_t ic_at(const MatView &A, int64_t pos) { return
 // SURVEY a3).  coef = {cx, cy} in device memory.  Row i <-> one lane; a warp owns 32
 // consecutive rows, a CTA 256.
 // ---------------------------------------------------------------------------------------
-// xPack[3*s + a] = x[offAtt + a*nDof + s]: the attitude unknowns of the operand of aprod1 interleaved by
+// xPack[3*s + a] = x[offAtt + a*nDof + s]: the attitude unknowns of the operand of the fused pass interleaved by
 // axis, so that the 12 unknowns of a row (3 axes x 4 consecutive starts; the paper keeps the axes N_DFA
 // apart) are one contiguous 96-byte run: 3-4 L2 sectors per row instead of 5-6, and the
 // 12 gathers of a lane fall into one or two L1 lines.  24 MB copied per product (~15 us).
@@ -223,6 +223,22 @@ __global__ void k_pack_att(MatView A, const double *__restrict__ x, double *__re
         const int64_t s = e / 3;
         const int a = int(e - s * 3);
         xPack[e] = x[A.offAtt + a * A.nDof + s];
+    }
+}
+// The standalone k_aprod1 is held by the LSU data pipe (86 % of its wavefronts, 12 of them per row for the attitude
+// unknowns alone): there the unknowns are packed four wide, xPack4[4*s + a] (a = 3: unused), so that every start is one
+// aligned 32-byte sector and a row takes 4 loads of 32 bytes instead of 12 of 8 (Medium: 10.2 -> 9.5 ms).  The fused pass
+// keeps the three-wide layout and the texture path: it is held by requests, not by LSU wavefronts, and ran 0.45 ms
+// slower with these loads.
+__global__ void k_pack_att4(MatView A, const double *__restrict__ x, double *__restrict__ xPack4, const int *done)
+{
+    if (done && *done) return;
+    const int64_t total = A.nDof * 4;
+    for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < total;
+         e += int64_t(gridDim.x) * blockDim.x) {
+        const int64_t s = e >> 2;
+        const int a = int(e & 3);
+        xPack4[e] = a < 3 ? x[A.offAtt + a * A.nDof + s] : 0.0;
     }
 }
 
@@ -265,11 +281,16 @@ k_aprod1(MatView A, const double *__restrict__ x, double *__restrict__ y,
                 for (int k = 0; k < NA; ++k) sum = fma(v[k], __ldg(xa + k), sum);
             }
             {
-                const double *xp = xPack + 3 * iatt;
+                const double *xp = xPack + 4 * iatt;   // xPack4 (k_pack_att4)
 #pragma unroll
-                for (int j = 0; j < 4; ++j)
+                for (int j = 0; j < 4; ++j) {
+                    double q[4];
+                    asm volatile("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];"
+                                 : "=d"(q[0]), "=d"(q[1]), "=d"(q[2]), "=d"(q[3])
+                                 : "l"(xp + 4 * j));
 #pragma unroll
-                    for (int a = 0; a < 3; ++a) sum = fma(v[KT + 4 * a + j], __ldg(xp + 3 * j + a), sum);
+                    for (int a = 0; a < 3; ++a) sum = fma(v[KT + 4 * a + j], q[a], sum);
+                }
             }
 #pragma unroll
             for (int j = 0; j < N_INSTR; ++j) sum = fma(v[KI + j], __ldg(xIns + c[j]), sum);
