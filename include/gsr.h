@@ -29,8 +29,9 @@
  *     k < kI : offInstr + instrCol[n_instr_par*i + (k-kT)]
  *     else   : offGlob + (k-kI)                 (Alg. 2 "glob")
  * The production layout 5/12/6/1, 5/12/6/N_Glob for any other N_Glob, and the section subset
- * 0/12/6/0 run the specialised kernels (fused iteration, attitude copy); every other layout runs one general pair of aprod kernels
- * and the two-product iteration (its attitude section still on the attitude copy).
+ * 0/12/6/0 run the specialised kernels (fused iteration, attitude copy); every other layout
+ * runs one general pair of aprod kernels and the two-product iteration (its attitude section
+ * still on the attitude copy; astrometric-only layouts have an aprod2 kernel of their own).
  *
  * Conventions
  *  - every call returns a gsr_status (0 = OK, negative = error); nothing throws;
