@@ -185,10 +185,13 @@ def test_lsqr_planted_noiseless():
     assert np.linalg.norm(r.x - d["x_true"]) <= 1e-10 * np.linalg.norm(d["x_true"])
 
 
-@pytest.mark.parametrize("tol,conlim,itnlim", [(1e-14, 0.0, 5000), (1e-8, 1e8, 5000), (0.0, 0.0, 25)])
+@pytest.mark.parametrize("tol,conlim,itnlim", [(1e-14, 0.0, 5000), (1e-8, 1e8, 5000), (0.0, 0.0, 25),
+                                               (0.0, 0.0, 5000)])
 def test_lsqr_matches_scipy(tol, conlim, itnlim):
     """scipy.sparse.linalg.lsqr is an independent implementation of the same published
-    algorithm with the same istop codes."""
+    algorithm with the same istop codes.  The four cases end with istop 2, 2, 7 and 5: with
+    atol = btol = 0 and no iteration limit in reach only the rounding-floor tests are left, and
+    1 + test2 <= 1 (istop 5) fires first -- the one branch no constructed case reaches."""
     cfg = synth.mini(seed=4, n_stars=30, obs=14, n_dof_att=16, n_instr=12, n_con=3, con_nnz=6)
     S, d = oracle_system(cfg)
     b = make_b(S, d)
@@ -198,6 +201,7 @@ def test_lsqr_matches_scipy(tol, conlim, itnlim):
     z, istop, itn, r1norm, _, anorm, acond, arnorm, xnorm, var = spla.lsqr(
         A, b, atol=tol, btol=tol, conlim=conlim, iter_lim=itnlim, calc_var=True)
     assert r.istop == istop
+    assert r.istop == {(1e-14, 5000): 2, (1e-8, 5000): 2, (0.0, 25): 7, (0.0, 5000): 5}[(tol, itnlim)]
     assert abs(r.itn - itn) <= 1
     if r.itn == itn:
         assert np.linalg.norm(r.x - S.p * z) <= 1e-12 * np.linalg.norm(z)
@@ -206,7 +210,8 @@ def test_lsqr_matches_scipy(tol, conlim, itnlim):
         # alpha_k, beta_k of late iterations (after the Krylov space is numerically exhausted)
         # amplify rounding differences between two implementations, and anorm / acond sum
         # them: bit-level agreement only away from the rounding floor (R19).
-        loose = 1e-9 if itnlim == 25 else 1e-5
+        # The istop-5 case runs ~50 iterations beyond the floor: there the two agree to percent level only.
+        loose = 1e-9 if itnlim == 25 else (1e-5 if tol > 0.0 else 2e-2)
         for mine, theirs in ((r.anorm, anorm), (r.acond, acond)):
             assert mine == pytest.approx(theirs, rel=loose)
         assert r.arnorm == pytest.approx(arnorm, rel=1e-6, abs=1e-12 * anorm * r1norm)
