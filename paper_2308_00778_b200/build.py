@@ -10,9 +10,9 @@ import subprocess
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
 _ROOT = os.path.dirname(_PKG)
-SRC = [os.path.join(_PKG, "csrc", "gsr.cu")]
+SRC = [os.path.join(_PKG, "csrc", "gsr.cu"), os.path.join(_PKG, "csrc", "gsr_noalloc.cu")]
 DEPS = SRC + [os.path.join(_PKG, "csrc", "gsr_kernels.cuh"), os.path.join(_ROOT, "include", "gsr.h"),
-              os.path.join(_ROOT, "include", "gsr_bench.h")]
+              os.path.join(_ROOT, "include", "gsr_bench.h"), os.path.join(_ROOT, "include", "gsr_noalloc.h")]
 LIB = os.path.join(_PKG, "libgsr.so")
 LIB_CHECK = os.path.join(_PKG, "libgsr_check.so")     # -DGSR_BOUNDS_CHECK: every gather / scatter index asserted
 

@@ -37,6 +37,10 @@ SYMBOLS = [
 ]
 # the measurement hook of include/gsr_bench.h
 BENCH_SYMBOLS = ["gsr_bench_set", "gsr_time_aprod"]
+# the allocation-free entry point of include/gsr_noalloc.h
+NOALLOC_SYMBOLS = ["gsr_norm2_noalloc"]
+NOALLOC_CHUNK, NOALLOC_MAX_PARTIALS = 65536, 16384
+NOALLOC_MAX_N = NOALLOC_CHUNK * NOALLOC_MAX_PARTIALS
 
 
 class GsrError(RuntimeError):
@@ -96,6 +100,7 @@ def load_library():
         "gsr_last_timing": (I32, [P, C.POINTER(D), C.POINTER(I64)]),
         "gsr_time_aprod": (I32, [P, I32, I32, C.POINTER(D)]),
         "gsr_bench_set": (I32, [P, C.c_char_p, I64]),
+        "gsr_norm2_noalloc": (I32, [P, I64, P, I32, P, C.c_char_p, I64]),
     }
     for name, (res, args) in sig.items():
         f = getattr(lib, name)
@@ -278,3 +283,27 @@ class Gsr:
         ms = C.c_double()
         self._ck(self.lib.gsr_time_aprod(self._h, which, reps, C.byref(ms)))
         return ms.value
+
+
+def gsr_norm2_noalloc(a, out, n=None, stream=None):
+    """out[0] = |a[:n]|_2 through gsr_norm2_noalloc (include/gsr_noalloc.h), the entry point for callers that
+    cannot allocate device memory: no handle, and the library itself allocates nothing -- its scratch is a fixed
+    array inside libgsr.so.  Both tensors are the CALLER's: `a` a float64 CUDA tensor, `out` a float64 CUDA
+    tensor of one element on the same GPU (this binding does not create it, so that the call stays free of
+    allocations end to end).  n defaults to a.numel(); the library rejects n > NOALLOC_MAX_N with GSR_EINVAL.
+    Calls share the built-in scratch: never run two of them at the same time on one GPU."""
+    lib = load_library()
+    if not (isinstance(out, torch.Tensor) and out.is_cuda and out.numel() >= 1):
+        raise TypeError("out: CUDA tensor with one element required")
+    n = a.numel() if n is None else int(n)
+    pa = _dev(a, torch.float64, "a") if a is not None else None
+    if a is not None and (a.device != out.device or n > a.numel()):
+        raise ValueError("a and out must be on the same GPU and n <= a.numel()")
+    device = out.device.index if out.device.index is not None else torch.cuda.current_device()
+    if stream is None:
+        stream = torch.cuda.current_stream(device).cuda_stream
+    err = C.create_string_buffer(512)
+    rc = lib.gsr_norm2_noalloc(pa, n, _dev(out, torch.float64, "out"), device, stream or None, err, len(err))
+    if rc != GSR_OK:
+        raise GsrError(rc, err.value.decode())
+    return out
