@@ -142,7 +142,8 @@ int64_t gsr_ncols(const gsr_handle *h);
 int64_t gsr_nrows(const gsr_handle *h);
 
 /* Copies the system to the device (A_d, M_i, I_c; Alg. 1 l.6-12).
- *   values           f64 [n_obs*N_par] row-major, section order as above (N_par = 24)
+ *   values           f64 [n_obs*N_par] row-major, section order as above (N_par = the layout's
+ *                    section widths summed; 24 in production)
  *   matrixIndexAstro i64 [n_obs]   = n_astro_par*star(i), non-decreasing (5*star(i) in production)
  *   matrixIndexAtt   i64 [n_obs]   = s_i in [0, n_dof_att-4] (axis-0 relative)
  *   instrCol         i32 [n_obs*n_instr_par] in [0, n_instr)
@@ -162,7 +163,12 @@ int32_t gsr_upload(gsr_handle *h, const double *values, const int64_t *matrixInd
  * may be NULL when n_con == 0) holds the known terms of the constraint rows.
  * A new upload always starts from scratch: every row must come again before the next
  * gsr_upload_finish (the 4-byte star indices of the rows are upload scratch that the
- * finish step turns into the star row pointer and frees). */
+ * finish step turns into the star row pointer and frees).  The ranges may come in any
+ * order and may overlap (the last copy of a row counts); gsr_upload_finish returns
+ * GSR_ESTATE, naming the first missing row, when some row has not been sent since the last
+ * successful finish, and the handle stays unusable until the upload is completed.  After a
+ * finish that failed with GSR_EINDEX the rows sent so far are kept: re-sending the offending
+ * rows and calling gsr_upload_finish again is enough. */
 int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double *values,
                         const int64_t *matrixIndexAstro, const int64_t *matrixIndexAtt,
                         const int32_t *instrCol, const double *b);

@@ -15,6 +15,8 @@
 #include <cstring>
 #include <new>
 #include <string>
+#include <utility>
+#include <vector>
 
 using namespace gsr;
 
@@ -47,7 +49,7 @@ struct gsr_handle {
     int32_t *ic = nullptr, *star = nullptr, *iatt = nullptr;   // 4-byte row indices
     uint16_t *ic16 = nullptr;                                  // instrument columns in 2 bytes when n_instr <= 65536 (ic stays null)
     unsigned long long *tw = nullptr;                          // per-tile star word (MatView::tw); star[] is upload scratch
-    int64_t badIngest = -1;                                    // first row whose instrument column did not fit 2 bytes
+    std::vector<std::pair<int64_t, int64_t>> rowsIn;           // disjoint sorted row ranges received since star[] was allocated
     int64_t *stageI = nullptr;                                 // upload staging of the two i64 index arrays
     // work
     double *u = nullptr, *v = nullptr, *w = nullptr, *z = nullptr, *var = nullptr;
@@ -403,15 +405,19 @@ int32_t gsr_create(const gsr_layout *L, gsr_handle **out)
     CK(dalloc(&h->trace, 5 * GSR_TRACE_CAP));
     CK(dalloc(&h->S, 1));
     CK(dalloc(&h->badDev, 1));
-    h->nRepAlloc = std::max(h->nRep, 64);   // room for the replica sweep of gsr_bench_set
+    // replicas of the instrument accumulators: what the product path uses (the replica sweep of gsr_bench_set grows the
+    // buffer when it asks for more); the opt-in instrument copy needs one slice per CTA of a bucket instead
+    const bool insCopy = (L->flags & GSR_FLAG_INS_COPY) != 0;
     // k_ins_scatter: buckets of <= INS_BUCKET_MAX columns, two CTAs per SM shared out over the buckets; every CTA owns a
     // slice of insRep
     h->insNB = int(std::max<int64_t>(1, (L->n_instr + INS_BUCKET_MAX - 1) / INS_BUCKET_MAX));
     h->insW = int(std::max<int64_t>(1, (L->n_instr + int64_t(h->insNB) * INS_WARPS - 1) / (int64_t(h->insNB) * INS_WARPS))) * INS_WARPS;
     h->insNG = std::max(1, h->smCount / h->insNB);
-    CK(cudaFuncSetAttribute(k_ins_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                            int((h->insW + 2 * INS_BLOCK) * sizeof(double))));
-    CK(dalloc(&h->insRep, int64_t(std::max(h->nRepAlloc, h->insNG)) * L->n_instr));
+    if (insCopy)
+        CK(cudaFuncSetAttribute(k_ins_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                int((h->insW + 2 * INS_BLOCK) * sizeof(double))));
+    h->nRepAlloc = std::max(h->nRep, insCopy ? h->insNG : 1);
+    CK(dalloc(&h->insRep, int64_t(h->nRepAlloc) * L->n_instr));
     CK(dalloc(&h->u, h->mTot));
     CK(dalloc(&h->v, h->n));
     CK(dalloc(&h->w, h->n));
@@ -525,8 +531,13 @@ int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double
     h->uploaded = false;
     h->preconditioned = false;
     h->conUploaded = false;   // gsr_precondition scaled conVal in place: the constraint rows must come again
-    if (!h->star) CK(dalloc(&h->star, h->L.n_obs));
+    if (!h->star) {   // a new upload: every row has to come (again) before gsr_upload_finish
+        CK(dalloc(&h->star, h->L.n_obs));
+        h->rowsIn.clear();
+    }
     const size_t r = size_t(nrows);
+    // without an astrometric section nothing else writes star[]: it only carries the bad-row marks of k_ingest_rows
+    if (!ia && nrows > 0) CK(cudaMemsetAsync(h->star + row0, 0, r * sizeof(int32_t), h->stream));
     CK(cudaMemcpyAsync(h->b + row0, b, r * sizeof(double), cudaMemcpyDefault, h->stream));
     {   // the two i64 index arrays -> 4-byte star / attitude start (device sources in place, host sources staged)
         const bool devI = nrows > 0 && (!ia || isDevicePtr(ia)) && (!iatt || isDevicePtr(iatt));
@@ -548,8 +559,6 @@ int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double
     // values and instrCol: row-major in the caller's memory -> tile-transposed on the device.
     // Device sources are read in place; host sources go through a bounded staging buffer.
     MatView A = view(h);
-    const unsigned long long noneI = ~0ull;
-    CK(cudaMemcpyAsync(h->badDev, &noneI, sizeof(noneI), cudaMemcpyHostToDevice, h->stream));
     const bool devV = nrows > 0 && isDevicePtr(values), devC = nrows > 0 && (!ic || isDevicePtr(ic));
     if (nrows > 0 && (!devV || !devC) && !h->stageV) {
         CK(dalloc(&h->stageV, STAGE_ROWS * h->nPar));
@@ -568,13 +577,21 @@ int32_t gsr_upload_rows(gsr_handle *h, int64_t row0, int64_t nrows, const double
             srcC = h->stageC;
         }
         k_ingest_rows<<<gridFor(cnt * (h->nPar + h->nI), 256 * 4, h->smCount * 16), 256, 0, h->stream>>>(
-            A, h->ic, h->ic16, row0 + q0, cnt, srcV, srcC, h->badDev);
+            A, h->ic, h->ic16, row0 + q0, cnt, srcV, srcC, h->star);
         CK(cudaGetLastError());
     }
-    unsigned long long badI = noneI;
-    CK(cudaMemcpyAsync(&badI, h->badDev, sizeof(badI), cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
-    if (badI != noneI && (h->badIngest < 0 || int64_t(badI) < h->badIngest)) h->badIngest = int64_t(badI);
+    if (nrows > 0) {   // rowsIn <- rowsIn U [row0, row0 + nrows), kept sorted and merged
+        int64_t lo = row0, hi = row0 + nrows;
+        std::vector<std::pair<int64_t, int64_t>> merged;
+        for (const auto &iv : h->rowsIn) {
+            if (iv.second < lo || iv.first > hi) merged.push_back(iv);
+            else { lo = std::min(lo, iv.first); hi = std::max(hi, iv.second); }
+        }
+        merged.emplace_back(lo, hi);
+        std::sort(merged.begin(), merged.end());
+        h->rowsIn.swap(merged);
+    }
     return GSR_OK;
 }
 
@@ -583,6 +600,12 @@ int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail)
     if (!h) return GSR_EINVAL;
     if (h->L.n_con > 0 && !b_tail) return fail(h, GSR_EINVAL, "b_tail is NULL but n_con > 0");
     if (!h->star) return fail(h, GSR_ESTATE, "no rows uploaded since the last gsr_upload_finish");
+    if (h->L.n_obs > 0 && !(h->rowsIn.size() == 1 && h->rowsIn[0].first == 0 && h->rowsIn[0].second == h->L.n_obs)) {
+        // star[] (and with it the row pointer) is only defined for rows that came since the last finish
+        const int64_t gap = h->rowsIn.empty() || h->rowsIn[0].first > 0 ? 0 : h->rowsIn[0].second;
+        return fail(h, GSR_ESTATE, "incomplete upload: observation row %lld has not been sent since the last "
+                    "gsr_upload_finish (every row must come again)", (long long)gap);
+    }
     int rc = enter(h);
     if (rc) return rc;
     if (h->L.n_con > 0)
@@ -596,8 +619,6 @@ int32_t gsr_upload_finish(gsr_handle *h, const double *b_tail)
     unsigned long long bad = none;
     CK(cudaMemcpyAsync(&bad, h->badDev, sizeof(bad), cudaMemcpyDeviceToHost, h->stream));
     CK(cudaStreamSynchronize(h->stream));
-    if (h->badIngest >= 0 && (bad == none || h->badIngest < int64_t(bad))) bad = (unsigned long long)h->badIngest;
-    h->badIngest = -1;
     if (bad != none) {
         h->badRow = int64_t(bad);
         return fail(h, GSR_EINDEX, "index contract violated at observation row %lld", (long long)bad);
@@ -1153,10 +1174,21 @@ int32_t gsr_bench_set(gsr_handle *h, const char *key, int64_t value)
     if (!h || !key) return GSR_EINVAL;
     const std::string k(key);
     if (k == "ins_sm_fused" && value >= 0 && value <= h->nInsSm) h->nInsSmFused = int(value);
-    else if (k == "n_rep" && value >= 1 && value <= h->nRepAlloc) h->nRep = int(value);
+    else if (k == "n_rep" && value >= 1 && value <= 128) {
+        if (value > h->nRepAlloc) {   // the sweep asks for more replicas than the product path allocated: grow the buffer
+            int rc = enter(h);        // (k_pre_aprod2 zeroes the replicas in use at the start of every product)
+            if (rc) return rc;
+            CK(cudaStreamSynchronize(h->stream));
+            double *grown = nullptr;
+            CK(dalloc(&grown, value * h->L.n_instr));
+            cudaFree(h->insRep);
+            h->insRep = grown;
+            h->nRepAlloc = int(value);
+        }
+        h->nRep = int(value);
+    }
     else if (k == "att_ctas_per_sm" && value >= 1 && value <= 16) h->gridAtt = h->gridAttLin = gridFor(h->nTiles, 8, h->smCount * int(value));
     else if (k == "fused_nopriv" && (value == 0 || value == 1)) h->fusedNoPriv = value != 0;
-    else if (k == "a2_ctas_per_sm" && value >= 1 && value <= 2) h->gridA2 = gridFor(h->nTiles, WARPS, h->smCount * int(value));
     else if (k == "use_ut" && (value == 0 || (value == 1 && h->uT))) h->useUT = value != 0;
     else if (k == "ut_ctas_per_sm" && value >= 1 && value <= 16) h->gridUT = gridFor(h->L.n_obs, 256, h->smCount * int(value));
     else return fail(h, GSR_EINVAL, "gsr_bench_set: unknown key or value out of range: %s = %lld", key, (long long)value);

@@ -1479,8 +1479,9 @@ __global__ void k_validate(MatView A, unsigned long long *badRow)
     for (int64_t i = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; i < A.m;
          i += int64_t(gridDim.x) * blockDim.x) {
         // k_ingest_index stored -1 for a matrixIndexAstro that is not 5*star with star in [0, nStars) and for a
-        // matrixIndexAtt outside [0, nDof-4]
-        bool bad = (A.nA > 0 && A.star[i] < 0) || (A.nAtt > 0 && A.iatt[i] < 0);
+        // matrixIndexAtt outside [0, nDof-4]; k_ingest_rows stored -1 in star[] for a row with a column that does not
+        // fit 2 bytes (star[] is the per-row mark of the upload for every layout: zeros when there is no astro section)
+        bool bad = A.star[i] < 0 || (A.nAtt > 0 && A.iatt[i] < 0);
         if (A.nA > 0 && i > 0) bad = bad || A.star[i - 1] > A.star[i];
         for (int j = 0; j < A.nI; ++j) {
             const int32_t c = ic_at(A, cpos(i, j, A.nI));
@@ -1607,11 +1608,12 @@ __global__ void k_scale_con_values(MatView A, int64_t nnz, const double *__restr
 // Upload (Alg. 1 l.6-12): rows [row0, row0+cnt) arrive row-major (A_d, I_c as the paper
 // stores them) and are written tile-transposed.  One thread per stored element; the
 // reads are coalesced, the writes hit 32 lines per warp but only once per upload.
-// A column outside [0, 65536) cannot be stored in 2 bytes: it is written as column 0 and the row is reported through
-// badRow (k_validate would not see it any more).
+// A column outside [0, nInstr) cannot be stored in 2 bytes: it is written as column 0 and the row is marked bad in the
+// upload scratch (rowMark[i] = -1, the value k_ingest_index gives a broken star index), where k_validate finds it.  The mark
+// lives with the row: sending the row again rewrites it, so an abandoned upload leaves nothing behind.
 __global__ void k_ingest_rows(MatView A, int32_t *__restrict__ icDev, uint16_t *__restrict__ ic16Dev, int64_t row0, int64_t cnt,
                               const double *__restrict__ values, const int32_t *__restrict__ ic,
-                              unsigned long long *badRow)
+                              int32_t *rowMark)
 {
     const int64_t nV = cnt * A.nPar, nC = cnt * A.nI;
     for (int64_t e = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; e < nV + nC;
@@ -1625,7 +1627,7 @@ __global__ void k_ingest_rows(MatView A, int32_t *__restrict__ icDev, uint16_t *
             if (ic16Dev) {
                 const bool ok = c >= 0 && c < A.nInstr;
                 ic16Dev[cpos(row0 + r, int(f - r * A.nI), A.nI)] = ok ? uint16_t(c) : uint16_t(0);
-                if (!ok) atomicMin(badRow, (unsigned long long)(row0 + r));
+                if (!ok) rowMark[row0 + r] = -1;
             } else {
                 icDev[cpos(row0 + r, int(f - r * A.nI), A.nI)] = c;
             }

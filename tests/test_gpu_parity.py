@@ -346,6 +346,57 @@ def test_chunked_device_upload_equals_whole_upload():
         check_aprods(S, G)
 
 
+def test_upload_state_partial_reupload_and_abandoned_upload():
+    """gsr_upload_finish needs every row since the last finish (the per-row star scratch is rebuilt per upload): a
+    partial re-upload is GSR_ESTATE, not a row pointer derived from stale memory.  And a chunk with a column that does
+    not fit 2 bytes, sent in an upload that is then abandoned, leaves nothing behind once its rows come again."""
+    cfg = CASES["ragged_tail"]["cfg"]
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    gsr = gsr_mod()
+    half = S.m // 2
+
+    def send(G, r0, r1, instr=None):
+        G.gsr_upload_rows(r0, r1 - r0, d["values"][r0:r1], d["matrixIndexAstro"][r0:r1], d["matrixIndexAtt"][r0:r1],
+                          np.ascontiguousarray((d["instrCol"] if instr is None else instr)[r0:r1]), b[r0:r1])
+
+    with gsr.Gsr(S.m, S.n_stars, S.n_dof_att, S.n_instr) as G:
+        with pytest.raises(gsr.GsrError) as e:               # nothing sent at all
+            G.gsr_upload_finish()
+        assert e.value.code == gsr.GSR_ESTATE
+        send(G, 0, S.m)
+        G.gsr_upload_finish()
+        check_aprods(S, G)
+        send(G, 0, half)                                     # partial re-upload
+        with pytest.raises(gsr.GsrError) as e:
+            G.gsr_upload_finish()
+        assert e.value.code == gsr.GSR_ESTATE and str(half) in str(e.value)
+        with pytest.raises(gsr.GsrError) as e:               # and the handle is not usable in between
+            G.gsr_aprod1(dev(np.zeros(S.n)), dev(np.zeros(S.m)))
+        assert e.value.code == gsr.GSR_ESTATE
+        send(G, half, S.m)                                   # the rest, out of order with an overlap
+        send(G, half - 7, half + 9)
+        G.gsr_upload_finish()
+        check_aprods(S, G, seed=3)
+        # abandoned upload with a bad 2-byte column, then a clean one in another chunking
+        bad = np.array(d["instrCol"], copy=True)
+        bad[40, 1] = 65536 + 2
+        send(G, 0, 100, instr=bad)
+        send(G, 0, 60)
+        send(G, 60, S.m)
+        G.gsr_upload_finish()
+        check_aprods(S, G, seed=4)
+        # the same bad chunk, not replaced: reported with its row
+        send(G, 100, S.m)
+        send(G, 0, 100, instr=bad)
+        with pytest.raises(gsr.GsrError) as e:
+            G.gsr_upload_finish()
+        assert e.value.code == gsr.GSR_EINDEX and G.gsr_bad_row() == 40
+        send(G, 30, 50)                                      # after a failed finish the other rows are still there
+        G.gsr_upload_finish()
+        check_aprods(S, G, seed=5)
+
+
 @pytest.mark.parametrize("ins_copy", [True, False])
 def test_two_attitude_blocks_and_mixed_instrument_table(ins_copy):
     """2.2 M rows: more than one 2^21-row block of the block-time-ordered attitude copy, 269 row blocks of the
@@ -457,6 +508,107 @@ def test_medium_full_size_every_element():
         worst = {k: float(v.max()) for k, v in sect.items()}
         assert all(w <= APROD_TOL for w in worst.values()), worst
         print(f"medium every element: aprod1 worst {worst1:.2e}, aprod2 worst by section {worst} (x 1e-12 bound)")
+
+
+def test_medium_lsqr_fused_path_vs_oracle():
+    """BASELINE configs[2] at full size through gsr_lsqr on the path bench.py times (fused single pass, texture gathers,
+    u kept in block-time order, 2-byte instrument columns; coefficient offsets beyond 2^32, 96 attitude blocks, most
+    instrument adds outside the shared-memory table) and through the two-product form, against the oracle's LSQR on the
+    same bytes: 3 iterations (a few LSQR iterations at Medium when the host has the RAM; the one-thread
+    oracle needs ~45 s per iteration), Alg. 1 l.13-27.  b = A x_true + noise is formed by the oracle."""
+    import psutil
+    gsr = gsr_mod()
+    torch.cuda.empty_cache()
+    free, _ = torch.cuda.mem_get_info()
+    if free < 90e9 or psutil.virtual_memory().available < 120e9:
+        pytest.skip("needs ~80 GB of free HBM and ~100 GB of host RAM")
+    cfg = synth.medium()
+    dv = torch.device("cuda", 0)
+    rp = synth.star_rowptr(cfg, dv)
+    m = int(rp[-1])
+    V = np.empty((m, 24))
+    ia, iatt = np.empty(m, dtype=np.int64), np.empty(m, dtype=np.int64)
+    ic = np.empty((m, 6), dtype=np.int32)
+    noise = np.empty(m)
+    for s0 in range(0, cfg.n_stars, 20_000):      # generated on the device (same seeded generator as the bench), kept on the host
+        part = synth.generate_rows(cfg, s0, min(s0 + 20_000, cfg.n_stars), dv, rp)
+        r0, nr = part["row0"], part["values"].shape[0]
+        V[r0:r0 + nr] = part["values"].cpu().numpy()
+        ia[r0:r0 + nr] = part["matrixIndexAstro"].cpu().numpy()
+        iatt[r0:r0 + nr] = part["matrixIndexAtt"].cpu().numpy()
+        ic[r0:r0 + nr] = part["instrCol"].cpu().numpy()
+        noise[r0:r0 + nr] = part["noise"].cpu().numpy()
+        del part
+    torch.cuda.empty_cache()
+    S = oracle.OracleSystem(cfg.n_stars, cfg.n_dof_att, cfg.n_instr, V, ia, iatt, ic)
+    del V, ia, iatt, ic
+    b = S.aprod1(synth.x_true(cfg, dv).cpu().numpy(), noise)
+    got = {}
+    for flags in (0, gsr.GSR_FLAG_NO_FUSE):
+        with gsr.Gsr(m, cfg.n_stars, cfg.n_dof_att, cfg.n_instr, flags=flags) as G:
+            G.gsr_upload(S.V, S.ia, S.iatt, S.ic, b)          # the unscaled bytes: S.precondition() comes later
+            info = G.gsr_path_info()
+            want = gsr.GSR_PATH_ATT_COPY | gsr.GSR_PATH_IC16 | (0 if flags else gsr.GSR_PATH_FUSED | gsr.GSR_PATH_TEX | gsr.GSR_PATH_UT)
+            assert info & want == want and bool(info & gsr.GSR_PATH_FUSED) == (flags == 0), info
+            G.gsr_precondition()
+            p = G.gsr_get_colscale().cpu().numpy()
+            r = G.gsr_lsqr(3, 0.0, 0.0)
+            got[flags] = (p, r, r.x.cpu().numpy(), r.se.cpu().numpy(), G.gsr_get_trace())
+        torch.cuda.empty_cache()
+    S.precondition()
+    ro = S.lsqr(b, 3, 0.0, 0.0, 0.0, True)
+    assert (ro.istop, ro.itn) == (7, 3)
+    for flags, (p, r, x, se, tr) in got.items():
+        np.testing.assert_allclose(p, S.p, rtol=P_TOL, atol=0)
+        assert (r.istop, r.itn) == (7, 3), flags
+        assert rel(x, ro.x) <= X_TOL, (flags, rel(x, ro.x))
+        assert rel(se, ro.se) <= 1e-8, (flags, rel(se, ro.se))
+        for c in (0, 2, 4):                                  # rnorm, anorm, xnorm per iteration
+            np.testing.assert_allclose(tr[:, c], ro.trace[:, c], rtol=1e-9)
+        print(f"medium lsqr flags={flags}: x rel {rel(x, ro.x):.2e}, se rel {rel(se, ro.se):.2e}")
+
+
+def test_rows_unsorted_in_time_and_repeated_instrument_columns():
+    """Inputs the header allows and the generator never makes (the instrument columns of a row follow no
+    particular scheme; nothing orders a star's rows in time): the rows of every star shuffled, and 5 % of the rows with
+    the same instrument column twice (same-lane repeated atomics, equal keys in the column-ordered copy, MATCH peers
+    inside one lane).  Every path: default, two-product, attitude atomics, instrument copy, and a Zipf case (MATCH)."""
+    gsr = gsr_mod()
+
+    def scramble(cfg, d):
+        rng = np.random.default_rng(77)
+        rp = synth.star_rowptr(cfg).numpy()
+        perm = np.concatenate([rp[s] + rng.permutation(rp[s + 1] - rp[s]) for s in range(cfg.n_stars)])
+        out = dict(d)
+        for k in ("values", "matrixIndexAstro", "matrixIndexAtt", "instrCol", "noise"):
+            out[k] = np.ascontiguousarray(d[k][perm])
+        assert np.array_equal(out["matrixIndexAstro"], d["matrixIndexAstro"])       # still sorted by star
+        assert (np.diff(out["matrixIndexAtt"]) < 0).mean() > 0.3                      # no longer by time
+        rows = rng.choice(len(perm), len(perm) // 20, replace=False)
+        out["instrCol"][rows, 4] = out["instrCol"][rows, 1]
+        return out
+
+    plain = synth.SynthConfig("shuf", 3_000, 4_000, 300, obs_per_star=90, seed=51)
+    zipf = synth.SynthConfig("shuf_zipf", 6_000, 3_000, 60_000, obs_powerlaw=(2.0, 10, 2000), att_bursts=(200, 2e-3, 0.7),
+                             instr_zipf=1.1, seed=52)      # the shape of test_skewed_shape_match_red_and_table
+    for cfg, flag_list in ((plain, (0, gsr.GSR_FLAG_NO_FUSE, gsr.GSR_FLAG_NO_ATT_COPY, gsr.GSR_FLAG_INS_COPY)),
+                           (zipf, (0, gsr.GSR_FLAG_NO_FUSE))):
+        d = scramble(cfg, np_inputs(cfg))
+        S, _ = oracle_system(cfg, d)
+        b = make_b(S, d)
+        for flags in flag_list:
+            with make_gpu(S, d, b, flags=flags) as G:
+                info = G.gsr_path_info()
+                assert bool(info & gsr.GSR_PATH_INSTR_MATCH) == (cfg is zipf)
+                assert bool(info & gsr.GSR_PATH_INS_COPY) == (flags == gsr.GSR_FLAG_INS_COPY)
+                check_aprods(S, G, seed=flags)
+        S.precondition()
+        ro = S.lsqr(b, 25, 0.0, 0.0)
+        for flags in flag_list:
+            with make_gpu(S, {**d, "values": S.V}, b, flags=flags) as G:      # the preconditioned matrix
+                r = G.gsr_lsqr(25, 0.0, 0.0)
+                assert (r.istop, r.itn) == (ro.istop, ro.itn) == (7, 25)
+                assert rel(r.x.cpu().numpy() * S.p, ro.x) <= X_TOL, (cfg.name, flags)
 
 
 def test_large_full_size_every_element():
