@@ -40,7 +40,9 @@ int32_t gsr_time_aprod(gsr_handle *h, int32_t which, int32_t reps, double *ms_pe
  * "att_ctas_per_sm" (grid of k_aprod2_att, 1..16), "ut_ctas_per_sm" (grid of k_u_to_time, 1..16), "use_ut" (0: the fused
  * iteration gathers u through permT instead of keeping the block-time-ordered copy; 1: back, only if the handle has it),
  * "fused_nopriv" (1: fused pass without the shared-memory instrument table, REDs only; a rejected variant kept for the
- * record in DESIGN.md 5).  "n_rep" takes 1..128 and grows the replica buffer (cudaMalloc) when the value exceeds what
+ * record in DESIGN.md 5), "l2_persist" (experiment: 1 = persisting L2 access-policy window over the packed attitude
+ * unknowns the fused pass gathers, 2 = over the instrument replicas its atomics hit, 0 = off and persisting lines reset).
+ * "n_rep" takes 1..128 and grows the replica buffer (cudaMalloc) when the value exceeds what
  * gsr_create allocated for the product path.  GSR_EINVAL for an unknown key or a value out of range.  The captured
  * iteration is rebuilt by the next gsr_lsqr. */
 int32_t gsr_bench_set(gsr_handle *h, const char *key, int64_t value);

@@ -79,6 +79,7 @@ struct gsr_handle {
     int64_t *insPtr = nullptr;
     int insNB = 1, insW = 1, insNG = 1;   // column buckets, columns per bucket, CTAs per bucket
     bool useInsT = false;
+    int l2Persist = 0;          // bench knob: 1 = persisting L2 window over xPack (attitude unknowns of the fused pass), 2 = over insRep
     bool fusedNoPriv = false;   // bench knob: fused pass without the shared-memory instrument table (REDs only), 256 threads x 2 CTAs per SM
     Scalars *S = nullptr;
     Scalars *hostS = nullptr;           // pinned, 2 slots
@@ -1078,6 +1079,25 @@ int32_t gsr_lsqr(gsr_handle *h, int64_t itnlim, double atol, double btol, double
         h->perIter = enqueueIteration(h);
         cudaError_t ec = cudaStreamEndCapture(st, &g);
         if (ec != cudaSuccess) return fail(h, GSR_ECUDA, "graph capture: %s", cudaGetErrorString(ec));
+        if (h->l2Persist) {   // bench knob: the stream's access-policy window on every kernel node of the iteration
+            cudaStreamAttrValue sv;
+            size_t nn = 0;
+            ec = cudaStreamGetAttribute(st, cudaStreamAttributeAccessPolicyWindow, &sv);
+            if (ec == cudaSuccess) ec = cudaGraphGetNodes(g, nullptr, &nn);
+            std::vector<cudaGraphNode_t> nodes(nn);
+            if (ec == cudaSuccess && nn) ec = cudaGraphGetNodes(g, nodes.data(), &nn);
+            for (size_t q = 0; ec == cudaSuccess && q < nn; ++q) {
+                cudaGraphNodeType ty;
+                ec = cudaGraphNodeGetType(nodes[q], &ty);
+                if (ec == cudaSuccess && ty == cudaGraphNodeTypeKernel) {
+                    cudaKernelNodeAttrValue kv;
+                    memset(&kv, 0, sizeof(kv));
+                    kv.accessPolicyWindow = sv.accessPolicyWindow;
+                    ec = cudaGraphKernelNodeSetAttribute(nodes[q], cudaKernelNodeAttributeAccessPolicyWindow, &kv);
+                }
+            }
+            if (ec != cudaSuccess) { cudaGraphDestroy(g); return fail(h, GSR_ECUDA, "graph access policy: %s", cudaGetErrorString(ec)); }
+        }
         ec = cudaGraphInstantiate(&h->iterGraph, g, 0);
         cudaGraphDestroy(g);
         if (ec != cudaSuccess) return fail(h, GSR_ECUDA, "graph instantiate: %s", cudaGetErrorString(ec));
@@ -1189,6 +1209,34 @@ int32_t gsr_bench_set(gsr_handle *h, const char *key, int64_t value)
     }
     else if (k == "att_ctas_per_sm" && value >= 1 && value <= 16) h->gridAtt = h->gridAttLin = gridFor(h->nTiles, 8, h->smCount * int(value));
     else if (k == "fused_nopriv" && (value == 0 || value == 1)) h->fusedNoPriv = value != 0;
+    else if (k == "l2_persist" && value >= 0 && value <= 2) {
+        // experiment (VERDICT r2 next 3 ii): keep the gather / atomic targets of the fused pass in L2 against the 45 GB
+        // __ldcs stream of A.  One window per stream: 1 = xPack (3 N_DFA doubles), 2 = the instrument replicas
+        int rc = enter(h);
+        if (rc) return rc;
+        CK(cudaStreamSynchronize(h->stream));
+        cudaStreamAttrValue av;
+        memset(&av, 0, sizeof(av));
+        if (value > 0) {
+            int maxPersist = 0, maxWin = 0;
+            CK(cudaDeviceGetAttribute(&maxPersist, cudaDevAttrMaxPersistingL2CacheSize, h->L.device));
+            CK(cudaDeviceGetAttribute(&maxWin, cudaDevAttrMaxAccessPolicyWindowSize, h->L.device));
+            void *base = value == 1 ? static_cast<void *>(h->xPack) : static_cast<void *>(h->insRep);
+            size_t bytes = value == 1 ? size_t(3) * h->L.n_dof_att * sizeof(double)
+                                      : size_t(h->nRep) * h->L.n_instr * sizeof(double);
+            bytes = std::min(bytes, size_t(maxWin));
+            CK(cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, std::min(size_t(maxPersist), bytes)));
+            av.accessPolicyWindow.base_ptr = base;
+            av.accessPolicyWindow.num_bytes = bytes;
+            av.accessPolicyWindow.hitRatio = bytes <= size_t(maxPersist) ? 1.0f : float(double(maxPersist) / double(bytes));
+            av.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+            av.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+        } else {
+            CK(cudaCtxResetPersistingL2Cache());
+        }
+        CK(cudaStreamSetAttribute(h->stream, cudaStreamAttributeAccessPolicyWindow, &av));
+        h->l2Persist = int(value);
+    }
     else if (k == "use_ut" && (value == 0 || (value == 1 && h->uT))) h->useUT = value != 0;
     else if (k == "ut_ctas_per_sm" && value >= 1 && value <= 16) h->gridUT = gridFor(h->L.n_obs, 256, h->smCount * int(value));
     else return fail(h, GSR_EINVAL, "gsr_bench_set: unknown key or value out of range: %s = %lld", key, (long long)value);
