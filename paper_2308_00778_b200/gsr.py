@@ -181,9 +181,10 @@ class Gsr:
             raise GsrError(rc, self.lib.gsr_last_error(self._h).decode())
 
     def close(self):
-        if getattr(self, "_h", None):
-            self.lib.gsr_destroy(self._h)
-            self._h = C.c_void_p()
+        h = getattr(self, "_h", None)
+        if h:
+            self._h = None          # (no module globals here: close also runs from __del__ at interpreter exit)
+            self.lib.gsr_destroy(h)
 
     __del__ = close
 

@@ -748,6 +748,18 @@ def test_small_config_lsqr():
         np.testing.assert_allclose(tr[:, 4], ro.trace[:, 4], rtol=1e-9)      # xnorm
         assert rc.istop == roc.istop and rc.istop != 7, (rc.istop, roc.istop)
         assert abs(rc.itn - roc.itn) <= 2, (rc.itn, roc.itn)
+        # The paper's own form of validation (section 6): mean +- std of the differences of the solution and of its
+        # standard errors per section between two codes (Table 1), and the ratio
+        # q = |dx| / sqrt(se_1^2 + se_2^2) < 1 for every unknown (Eq. 5) -- here CUDA path vs oracle.
+        xg, sg = rc.x.cpu().numpy(), rc.se.cpu().numpy()
+        na, nd = 5 * cfg.n_stars, 3 * cfg.n_dof_att
+        for name, sl in (("astro", slice(0, na)), ("att", slice(na, na + nd)), ("instr", slice(na + nd, S.n - 1)),
+                         ("glob", slice(S.n - 1, S.n))):
+            dx, ds = xg[sl] - roc.x[sl], sg[sl] - roc.se[sl]
+            q = np.abs(dx) / np.sqrt(sg[sl] ** 2 + roc.se[sl] ** 2)
+            print(f"paper-style check, {name}: dx {dx.mean():.2e} +- {dx.std():.2e}, dse {ds.mean():.2e} +- {ds.std():.2e}, "
+                  f"max q {q.max():.2e}")
+            assert q.max() < 1.0, name
         assert rel(rc.x.cpu().numpy(), roc.x) <= X_TOL_CONVERGED
         assert rel(rc.x.cpu().numpy(), d["x_true"]) <= 1e-3
 
