@@ -108,6 +108,9 @@ def _load():
         lib.gsr_oracle_lsqr.restype = C.c_int
         lib.gsr_oracle_lsqr.argtypes = [P, P, C.c_int64, C.c_double, C.c_double, C.c_double,
                                         P, P, P, P, P]
+        lib.gsr_oracle_lsqr_cov.restype = C.c_int
+        lib.gsr_oracle_lsqr_cov.argtypes = [P, P, C.c_int64, C.c_double, C.c_double, C.c_double,
+                                            P, P, P, P, P, C.c_int64, P, P, P]
         _lib = lib
     return _lib
 
@@ -128,6 +131,7 @@ class LsqrResult:
     arnorm: float
     xnorm: float
     trace: np.ndarray | None = None  # [itn, 5]: rnorm, arnorm, anorm, acond, xnorm
+    cov: np.ndarray | None = None    # covariances of the couples passed to lsqr(pairs=...)
 
 
 class OracleSystem:
@@ -205,21 +209,33 @@ class OracleSystem:
         self.lib.gsr_oracle_precondition(self._sp, _ptr(self.p))
         return self.p
 
-    def lsqr(self, b, itnlim, atol, btol, conlim=0.0, want_trace=False) -> LsqrResult:
-        """LSQR on the system as stored; if preconditioned, returns x = p*z, se = p*se_z."""
+    def lsqr(self, b, itnlim, atol, btol, conlim=0.0, want_trace=False, pairs=None) -> LsqrResult:
+        """LSQR on the system as stored; if preconditioned, returns x = p*z, se = p*se_z.
+        pairs = (i[], j[]): also the covariances of those couples of unknowns (gsr_oracle_lsqr_cov)."""
         b = np.ascontiguousarray(b, dtype=np.float64)
         assert b.shape == (self.m_tot,)
         x = np.zeros(self.n)
         se = np.zeros(self.n)
         res = _Res()
         trace = np.zeros((max(int(itnlim), 1), 5)) if want_trace else None
-        rc = self.lib.gsr_oracle_lsqr(self._sp, _ptr(b), int(itnlim), float(atol), float(btol),
-                                      float(conlim), _ptr(self.p), _ptr(x), _ptr(se),
-                                      C.addressof(res), _ptr(trace))
+        cov = None
+        if pairs is None:
+            rc = self.lib.gsr_oracle_lsqr(self._sp, _ptr(b), int(itnlim), float(atol), float(btol),
+                                          float(conlim), _ptr(self.p), _ptr(x), _ptr(se),
+                                          C.addressof(res), _ptr(trace))
+        else:
+            pi = np.ascontiguousarray(pairs[0], dtype=np.int64)
+            pj = np.ascontiguousarray(pairs[1], dtype=np.int64)
+            assert pi.shape == pj.shape and pi.ndim == 1
+            assert pi.size == 0 or (min(pi.min(), pj.min()) >= 0 and max(pi.max(), pj.max()) < self.n)
+            cov = np.zeros(pi.shape[0])
+            rc = self.lib.gsr_oracle_lsqr_cov(self._sp, _ptr(b), int(itnlim), float(atol), float(btol),
+                                              float(conlim), _ptr(self.p), _ptr(x), _ptr(se),
+                                              C.addressof(res), _ptr(trace), pi.shape[0], _ptr(pi), _ptr(pj), _ptr(cov))
         if rc != 0:
             raise MemoryError("oracle lsqr allocation failed")
         return LsqrResult(x, se, int(res.istop), int(res.itn), res.anorm, res.acond, res.rnorm,
-                          res.arnorm, res.xnorm, None if trace is None else trace[: res.itn])
+                          res.arnorm, res.xnorm, None if trace is None else trace[: res.itn], cov)
 
 
 class OmpRunner:

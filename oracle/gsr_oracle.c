@@ -24,6 +24,8 @@
  *   x_k, se (standard errors)   : closed form V_k (B_k^T B_k)^-1 V_k^T from a dense,
  *                                 re-orthogonalised Golub-Kahan bidiagonalisation
  *                                 (k <= 20), upper bound diag((A'^T A')^-1), scipy var
+ *   cov (covariances of couples): off-diagonal entries of the same closed form (k <= 20), scaled by the
+ *                                 true residual; cov(i,i) = se_i^2; symmetry in (i, j); |cov_ij| <= se_i se_j
  *
  * Matrix definition (PAPER.md:78-80 and the index expressions
  * of Algorithm 2).  Row i of A holds
@@ -230,9 +232,41 @@ typedef struct {
  * x / se instead of z / se_z.  trace, if not NULL, receives 5 doubles per
  * iteration: rnorm, arnorm, anorm, acond, xnorm.
  */
+static int lsqr_body(const gsr_oracle_system *S, const double *b, int64_t itnlim, double atol,
+                     double btol, double conlim, const double *p, double *x, double *se,
+                     gsr_oracle_result *R, double *trace, int64_t npairs, const int64_t *pi,
+                     const int64_t *pj, double *cov);
+
 int gsr_oracle_lsqr(const gsr_oracle_system *S, const double *b, int64_t itnlim, double atol,
                     double btol, double conlim, const double *p, double *x, double *se,
                     gsr_oracle_result *R, double *trace)
+{
+    return lsqr_body(S, b, itnlim, atol, btol, conlim, p, x, se, R, trace, 0, NULL, NULL, NULL);
+}
+
+/*
+ * The same solve, with the covariances between chosen couples of unknowns ("the errors
+ * (variances) on the unknowns and the covariances between the different couples of unknowns are
+ * calculated"; Alg. 1 l.26-27).  The paper names neither the couples nor a formula
+ * (reading R26): the couples (pi[q], pj[q]), q < npairs, are the caller's, and the estimate is
+ * the one LSQR's variances are the diagonal of -- Paige & Saunders' sum_k d_k d_k^T with d_k = w_k/rho_k,
+ * which tends to (A'^T A')^-1 -- scaled like the standard errors: with s = rnorm/sqrt(m - n) (s = rnorm
+ * when m <= n),
+ *     cov[q] = p_i p_j s^2 sum_k d_k[i] d_k[j],     i = pi[q], j = pj[q],
+ * so that cov(i, i) = se_i^2.  Everything else is gsr_oracle_lsqr, step for step.
+ */
+int gsr_oracle_lsqr_cov(const gsr_oracle_system *S, const double *b, int64_t itnlim, double atol,
+                        double btol, double conlim, const double *p, double *x, double *se,
+                        gsr_oracle_result *R, double *trace, int64_t npairs, const int64_t *pi,
+                        const int64_t *pj, double *cov)
+{
+    return lsqr_body(S, b, itnlim, atol, btol, conlim, p, x, se, R, trace, npairs, pi, pj, cov);
+}
+
+static int lsqr_body(const gsr_oracle_system *S, const double *b, int64_t itnlim, double atol,
+                     double btol, double conlim, const double *p, double *x, double *se,
+                     gsr_oracle_result *R, double *trace, int64_t npairs, const int64_t *pi,
+                     const int64_t *pj, double *cov)
 {
     const int64_t n = gsr_oracle_ncols(S);
     const int64_t m = S->n_obs + S->n_con;
@@ -254,6 +288,8 @@ int gsr_oracle_lsqr(const gsr_oracle_system *S, const double *b, int64_t itnlim,
         x[j] = 0.0;
         se[j] = 0.0; /* holds var until the finish step */
     }
+    for (int64_t q = 0; q < npairs; ++q)
+        cov[q] = 0.0; /* holds sum_k d_k[i] d_k[j] until the finish step */
     memcpy(u, b, sizeof(double) * (size_t)m);
     double alpha = 0.0;
     double beta = gsr_oracle_norm(u, m);
@@ -305,6 +341,11 @@ int gsr_oracle_lsqr(const gsr_oracle_system *S, const double *b, int64_t itnlim,
             /* step 4: update x, w, var */
             const double t1 = phi / rho;
             const double t2 = -theta / rho;
+            for (int64_t q = 0; q < npairs; ++q) { /* before w is overwritten: d_k = w_k / rho_k */
+                const double di = w[pi[q]] / rho;
+                const double dj = w[pj[q]] / rho;
+                cov[q] = cov[q] + di * dj;
+            }
             for (int64_t j = 0; j < n; ++j) {
                 const double dk = w[j] / rho;
                 x[j] = x[j] + t1 * w[j];
@@ -355,12 +396,17 @@ int gsr_oracle_lsqr(const gsr_oracle_system *S, const double *b, int64_t itnlim,
             s = rnorm / sqrt((double)(m - n));
         for (int64_t j = 0; j < n; ++j)
             se[j] = sqrt(se[j]) * s;
+        for (int64_t q = 0; q < npairs; ++q)
+            cov[q] = cov[q] * (s * s);
     }
-    if (p)
+    if (p) {
         for (int64_t j = 0; j < n; ++j) {
             x[j] = p[j] * x[j];
             se[j] = p[j] * se[j];
         }
+        for (int64_t q = 0; q < npairs; ++q)
+            cov[q] = p[pi[q]] * p[pj[q]] * cov[q];
+    }
     R->istop = istop;
     R->itn = itn;
     R->anorm = anorm;

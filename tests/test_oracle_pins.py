@@ -175,6 +175,44 @@ def test_lsqr_matches_dense_least_squares(precond, ncon):
     assert np.linalg.norm(r.x - d["x_true"]) <= 0.05 * np.linalg.norm(d["x_true"])
 
 
+def test_covariances_against_krylov_closed_form():
+    """Covariances of couples of unknowns (Alg. 1 l.26-27; R26): the off-diagonal entries of
+    sum_{i<=k} d_i d_i^T = V_k (B_k^T B_k)^-1 V_k^T (dense, re-orthogonalised Golub-Kahan; nothing of the LSQR
+    recurrences; at k = n that matrix is (A'^T A')^-1, checked on the dense side), scaled by the TRUE residual of the
+    dense Krylov solution over (m - n) and by p_i p_j, while the oracle's Lanczos vectors are still orthogonal
+    (k <= 20, as for the variances).  Also: cov(i, i) = se_i^2, cov(i, j) = cov(j, i), |cov(i, j)| <= se_i se_j
+    (the estimate is positive semi-definite), and a solve with couples returns x / se bit for bit as one without."""
+    cfg = synth.mini(seed=9, n_stars=3, obs=16, n_dof_att=5, n_instr=6)
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    p = S.precondition()
+    A = dense(S)
+    n = S.n
+    B, V, beta = _golub_kahan_reorth(A, b, n)
+    np.testing.assert_allclose(V @ np.linalg.inv(B.T @ B) @ V.T, np.linalg.inv(A.T @ A), rtol=0, atol=1e-9)
+    rng = np.random.default_rng(5)
+    pi = np.concatenate([rng.integers(0, n, 40), np.arange(6)])
+    pj = np.concatenate([rng.integers(0, n, 40), np.arange(6)])        # the last six couples are (i, i)
+    for k in (1, 2, 5, 10, 20):
+        Bk, Vk = B[:k + 1, :k], V[:, :k]
+        e1 = np.zeros(k + 1)
+        e1[0] = beta
+        zk = Vk @ np.linalg.lstsq(Bk, e1, rcond=None)[0]
+        C_ref = Vk @ np.linalg.inv(Bk.T @ Bk) @ Vk.T
+        s2 = np.linalg.norm(b - A @ zk) ** 2 / (S.m_tot - n)
+        cov_ref = p[pi] * p[pj] * s2 * C_ref[pi, pj]
+        rk = S.lsqr(b, k, 0.0, 0.0, pairs=(pi, pj))
+        scale = p[pi] * p[pj] * s2 * np.sqrt(C_ref[pi, pi] * C_ref[pj, pj])      # |cov| <= this (Cauchy-Schwarz)
+        assert np.all(np.abs(rk.cov - cov_ref) <= 1e-9 * scale), (k, np.max(np.abs(rk.cov - cov_ref) / scale))
+        np.testing.assert_allclose(rk.cov[-6:], rk.se[:6] ** 2, rtol=1e-13)
+        assert np.all(np.abs(rk.cov) <= rk.se[pi] * rk.se[pj] * (1 + 1e-12))
+        r0 = S.lsqr(b, k, 0.0, 0.0)
+        assert np.array_equal(r0.x, rk.x) and np.array_equal(r0.se, rk.se) and r0.itn == rk.itn
+        rt = S.lsqr(b, k, 0.0, 0.0, pairs=(pj, pi))
+        assert np.array_equal(rt.cov, rk.cov)
+    assert (cov_ref[:40] < 0).any() and (cov_ref[:40] > 0).any()    # real off-diagonal entries of both signs were compared
+
+
 def test_lsqr_planted_noiseless():
     cfg = dataclasses.replace(synth.mini(seed=2), noise_sigma=0.0)
     S, d = oracle_system(cfg)
