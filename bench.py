@@ -390,12 +390,12 @@ def main_ours(args):
                                   if att_copy else rb["k_aprod2_redatt"])
     moved_gb = (moved * m + 12 * 8 * G.n) / 1e9
     traffic, traffic_src = None, None      # ncu-measured DRAM bytes per launch of the dominant kernel
-    tpath = os.path.join(ROOT, "profiles", "r02_traffic.csv")
-    if os.path.exists(tpath):
+    tpath = os.path.join(ROOT, "profiles", "r03_traffic.csv")
+    if os.path.exists(tpath) and prod:
         for ln in open(tpath).read().splitlines()[1:]:
             w, kn, bts = ln.split(",")[:3]
-            if w == args.workload and kn == dom:
-                traffic, traffic_src = float(bts) / 1e9, "profiles/r02_traffic.csv (one ncu --set full capture, see r02_traffic.md)"
+            if w == args.workload and kn == dom and (w != "skewed" or abs(args.skew_alpha - 1.47) < 1e-9):
+                traffic, traffic_src = float(bts) / 1e9, "profiles/r03_traffic.csv (one ncu --set full capture, see r03_ncu_full_summary.md)"
     roofline = {"bound": "hbm", "kernel": dom, "achieved": k[dom]["gbs"], "peak": peak, "unit": "GB/s",
                 "frac": k[dom]["gbs"] / peak, "traffic": traffic, "traffic_unit": "GB per launch (ncu dram read+write)",
                 "traffic_source": traffic_src, "peak_source": peak_src, "nominal_peak": NOMINAL_HBM_GBS,

@@ -222,6 +222,20 @@ int32_t gsr_aprod2(gsr_handle *h, const double *y, double *x);
 int32_t gsr_lsqr(gsr_handle *h, int64_t itnlim, double atol, double btol, double conlim,
                  gsr_result *result);
 
+/* Covariances between couples of unknowns ("the covariances between the different couples of
+ * unknowns are calculated"; Alg. 1 l.26-27).  The paper names neither the couples nor a formula:
+ * the couples are the caller's, and the estimate is the one LSQR's variances are the diagonal of (Paige & Saunders'
+ * sum_k d_k d_k^T, d_k = w_k / rho_k, which tends to (A'^T A')^-1), scaled like the standard errors:
+ *     cov(i, j) = p_i p_j * rnorm^2 / (m_tot - n) * sum_k d_k[i] d_k[j]     (rnorm^2 alone when m_tot <= n),
+ * so that cov(i, i) = se_i^2 (reading R26).
+ * gsr_set_cov_pairs: npairs couples (pi[q], pj[q]) of column indices in [0, n), i64, host or device; the library
+ * copies them.  They stay set for every later gsr_lsqr on this handle until replaced; npairs = 0 clears them.
+ * GSR_EINDEX (gsr_last_error names the couple) for an index out of range.  Each iteration then costs one extra
+ * kernel of npairs threads.  gsr_get_cov: the npairs covariances of the last gsr_lsqr, f64, host or device;
+ * GSR_ESTATE before a solve with couples set. */
+int32_t gsr_set_cov_pairs(gsr_handle *h, int64_t npairs, const int64_t *pi, const int64_t *pj);
+int32_t gsr_get_cov(gsr_handle *h, double *out);
+
 /* Per-iteration log of the last gsr_lsqr: up to max_itn rows of 5 doubles
  * (rnorm, arnorm, anorm, acond, xnorm) to a HOST buffer; returns rows written in
  * *n_written.  Only the last GSR_TRACE_CAP iterations are kept. */

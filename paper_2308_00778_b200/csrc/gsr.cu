@@ -79,6 +79,10 @@ struct gsr_handle {
     int64_t *insPtr = nullptr;
     int insNB = 1, insW = 1, insNG = 1;   // column buckets, columns per bucket, CTAs per bucket
     bool useInsT = false;
+    int64_t nPairs = 0;          // couples of unknowns whose covariance gsr_lsqr estimates (gsr_set_cov_pairs)
+    int64_t *pairI = nullptr, *pairJ = nullptr;
+    double *covAcc = nullptr, *covOut = nullptr;
+    bool covValid = false;
     int l2Persist = 0;          // bench knob: 1 = persisting L2 window over xPack (attitude unknowns of the fused pass), 2 = over insRep
     bool fusedNoPriv = false;   // bench knob: fused pass without the shared-memory instrument table (REDs only), 256 threads x 2 CTAs per SM
     Scalars *S = nullptr;
@@ -496,6 +500,9 @@ int32_t gsr_destroy(gsr_handle *h)
                     h->u, h->v, h->w, h->z, h->var, h->carryFirst, h->carryLast, h->globPartial,
                     h->sqPartialU, h->sqPartialV, h->ddPartial, h->coefOne, h->coefTime, h->trace,
                     h->S, h->badDev, h->attT, h->insRep, h->sT, h->permT, h->stageV, h->stageC, h->xPack, h->xPack4, h->t, h->coefRaw, h->uT, h->insVal, h->insMeta, h->insPtr};
+    void *covPtrs[] = {h->pairI, h->pairJ, h->covAcc, h->covOut};
+    for (void *q : covPtrs)
+        if (q) cudaFree(q);
     for (void *q : ptrs)
         if (q) cudaFree(q);
     if (h->hostS) cudaFreeHost(h->hostS);
@@ -875,6 +882,14 @@ bool canFuse(const gsr_handle *h)
     return h->prod && !(h->L.flags & GSR_FLAG_NO_FUSE) && h->useAttT && h->L.n_obs > 0;
 }
 
+// covariance accumulation of the iteration (only when couples are set): before k_update overwrites w
+int enqueueCov(gsr_handle *h)
+{
+    if (h->nPairs <= 0) return 0;
+    k_cov_update<<<gridFor(h->nPairs, 256, h->smCount * 8), 256, 0, h->stream>>>(h->w, h->pairI, h->pairJ, h->nPairs, h->S, h->covAcc);
+    return 1;
+}
+
 int enqueueIterationFused(gsr_handle *h)
 {
     Scalars *S = h->S;
@@ -911,6 +926,7 @@ int enqueueIterationFused(gsr_handle *h)
     // v^ <- a2_cx*v^ + a2_cy*t  (= A^T u - beta v with the lazy scales), sum v^2
     k_combine_sumsq<<<h->gridVec, 256, 0, st>>>(h->v, h->t, h->n, &S->a2_cx, h->sqPartialV, done);
     k_scalar<<<1, 256, 0, st>>>(PH_AFTER_APROD2, S, h->sqPartialV, h->gridVec, nullptr, 0);
+    nk += enqueueCov(h);
     k_update<<<h->gridVec, 256, 0, st>>>(h->z, h->w, h->v, h->var, h->n, S, h->ddPartial);
     k_scalar<<<1, 256, 0, st>>>(PH_AFTER_UPDATE, S, h->ddPartial, h->gridVec, h->trace, GSR_TRACE_CAP);
     return nk;
@@ -928,6 +944,7 @@ int enqueueIteration(gsr_handle *h)
     nk += enqueueAprod2<false>(h, h->u, h->v, &S->a2_cx, done, true);
     k_sumsq<<<h->gridVec, 256, 0, h->stream>>>(h->v, h->n, h->sqPartialV, done);
     k_scalar<<<1, 256, 0, h->stream>>>(PH_AFTER_APROD2, S, h->sqPartialV, h->gridVec, nullptr, 0);
+    nk += enqueueCov(h);
     k_update<<<h->gridVec, 256, 0, h->stream>>>(h->z, h->w, h->v, h->var, h->n, S, h->ddPartial);
     k_scalar<<<1, 256, 0, h->stream>>>(PH_AFTER_UPDATE, S, h->ddPartial, h->gridVec, h->trace, GSR_TRACE_CAP);
     return nk + 5;
@@ -1062,6 +1079,7 @@ int32_t gsr_lsqr(gsr_handle *h, int64_t itnlim, double atol, double btol, double
     CK(cudaMemsetAsync(h->v, 0, size_t(h->n) * sizeof(double), st));
     CK(cudaMemsetAsync(h->z, 0, size_t(h->n) * sizeof(double), st));
     CK(cudaMemsetAsync(h->var, 0, size_t(h->n) * sizeof(double), st));
+    if (h->nPairs > 0) CK(cudaMemsetAsync(h->covAcc, 0, size_t(h->nPairs) * sizeof(double), st));
     k_sumsq<<<h->gridVec, 256, 0, st>>>(h->u, h->mTot, h->sqPartialV, nullptr);
     k_scalar<<<1, 256, 0, st>>>(PH_INIT_BETA, h->S, h->sqPartialV, h->gridVec, nullptr, 0);
     enqueueAprod2<false>(h, h->u, h->v, &h->S->a2_cx, nullptr, false);
@@ -1136,7 +1154,11 @@ int32_t gsr_lsqr(gsr_handle *h, int64_t itnlim, double atol, double btol, double
 
     // finish (Alg. 1 l.27): x = p (.) z, se; staged in v / w when the outputs are host memory
     k_finish<<<h->gridVec, 256, 0, st>>>(h->z, h->var, h->p, h->v, R->se ? h->w : nullptr, h->n, h->mTot, h->S);
+    if (h->nPairs > 0)
+        k_cov_finish<<<gridFor(h->nPairs, 256, h->smCount * 8), 256, 0, st>>>(h->covAcc, h->pairI, h->pairJ, h->nPairs, h->p, h->n,
+                                                                             h->mTot, h->S, h->covOut);
     CK(cudaGetLastError());
+    h->covValid = h->nPairs > 0;
     CK(cudaMemcpyAsync(R->x, h->v, size_t(h->n) * sizeof(double), cudaMemcpyDefault, st));
     if (R->se) CK(cudaMemcpyAsync(R->se, h->w, size_t(h->n) * sizeof(double), cudaMemcpyDefault, st));
     CK(cudaMemcpyAsync(&h->hostS[0], h->S, sizeof(Scalars), cudaMemcpyDeviceToHost, st));
@@ -1145,6 +1167,53 @@ int32_t gsr_lsqr(gsr_handle *h, int64_t itnlim, double atol, double btol, double
     R->istop = F.istop; R->itn = F.itn; R->anorm = F.anorm; R->acond = F.acond;
     R->rnorm = F.rnorm; R->arnorm = F.arnorm; R->xnorm = F.xnorm;
     h->lastItn = F.itn;
+    return GSR_OK;
+}
+
+int32_t gsr_set_cov_pairs(gsr_handle *h, int64_t npairs, const int64_t *pi, const int64_t *pj)
+{
+    if (!h || npairs < 0 || (npairs > 0 && (!pi || !pj))) return GSR_EINVAL;
+    int rc = enter(h);
+    if (rc) return rc;
+    CK(cudaStreamSynchronize(h->stream));
+    if (h->iterGraph) {   // the captured iteration holds (or lacks) the covariance node
+        cudaGraphExecDestroy(h->iterGraph);
+        h->iterGraph = nullptr;
+    }
+    void *old[] = {h->pairI, h->pairJ, h->covAcc, h->covOut};
+    for (void *q : old)
+        if (q) cudaFree(q);
+    h->pairI = h->pairJ = nullptr;
+    h->covAcc = h->covOut = nullptr;
+    h->nPairs = 0;
+    h->covValid = false;
+    if (npairs == 0) return GSR_OK;
+    CK(dalloc(&h->pairI, npairs));
+    CK(dalloc(&h->pairJ, npairs));
+    CK(dalloc(&h->covAcc, npairs));
+    CK(dalloc(&h->covOut, npairs));
+    CK(cudaMemcpyAsync(h->pairI, pi, size_t(npairs) * sizeof(int64_t), cudaMemcpyDefault, h->stream));
+    CK(cudaMemcpyAsync(h->pairJ, pj, size_t(npairs) * sizeof(int64_t), cudaMemcpyDefault, h->stream));
+    const unsigned long long none = ~0ull;
+    CK(cudaMemcpyAsync(h->badDev, &none, sizeof(none), cudaMemcpyHostToDevice, h->stream));
+    k_validate_pairs<<<gridFor(npairs, 256, h->smCount * 8), 256, 0, h->stream>>>(h->pairI, h->pairJ, npairs, h->n, h->badDev);
+    CK(cudaGetLastError());
+    unsigned long long bad = none;
+    CK(cudaMemcpyAsync(&bad, h->badDev, sizeof(bad), cudaMemcpyDeviceToHost, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
+    if (bad != none) return fail(h, GSR_EINDEX, "couple %lld names an unknown outside [0, n)", (long long)bad);
+    h->nPairs = npairs;
+    return GSR_OK;
+}
+
+int32_t gsr_get_cov(gsr_handle *h, double *out)
+{
+    if (!h || !out) return GSR_EINVAL;
+    if (!h->covValid) return fail(h, GSR_ESTATE, "no covariances: gsr_set_cov_pairs, then gsr_lsqr");
+    int rc = enter(h);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(out, h->covOut, size_t(h->nPairs) * sizeof(double), cudaMemcpyDefault, h->stream));
+    CK(cudaStreamSynchronize(h->stream));
     return GSR_OK;
 }
 

@@ -1345,6 +1345,37 @@ __global__ void k_init_w(double *__restrict__ w, const double *__restrict__ vhat
         w[j] = vhat[j] * ia;
 }
 
+// gsr_set_cov_pairs: first couple with an index outside [0, n)
+__global__ void k_validate_pairs(const int64_t *__restrict__ pi, const int64_t *__restrict__ pj, int64_t npairs, int64_t n,
+                                 unsigned long long *bad)
+{
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < npairs; q += int64_t(gridDim.x) * blockDim.x)
+        if (pi[q] < 0 || pi[q] >= n || pj[q] < 0 || pj[q] >= n) atomicMin(bad, (unsigned long long)q);
+}
+
+// Covariances of the caller's couples of unknowns (Alg. 1 l.26; R26), accumulated
+// beside the variances: acc[q] += d_k[i] d_k[j] with d_k = w_k / rho_k.  Runs BEFORE k_update of the same iteration (which
+// overwrites w), after the scalar kernel that set inv_rho.  One thread per couple; couples are few (<< n).
+__global__ void k_cov_update(const double *__restrict__ w, const int64_t *__restrict__ pi, const int64_t *__restrict__ pj,
+                             int64_t npairs, const Scalars *__restrict__ S, double *__restrict__ acc)
+{
+    if (S->done) return;
+    const double ir = S->inv_rho;
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < npairs; q += int64_t(gridDim.x) * blockDim.x)
+        acc[q] = fma(w[pi[q]] * ir, w[pj[q]] * ir, acc[q]);
+}
+
+// Alg. 1 l.27 for the couples: cov(i, j) = p_i p_j s^2 acc, s as in k_finish, so that cov(i, i) = se_i^2.
+__global__ void k_cov_finish(const double *__restrict__ acc, const int64_t *__restrict__ pi, const int64_t *__restrict__ pj,
+                             int64_t npairs, const double *__restrict__ p, int64_t n, int64_t mTot,
+                             const Scalars *__restrict__ S, double *__restrict__ out)
+{
+    double s = S->rnorm;
+    if (mTot > n) s = s / sqrt(double(mTot - n));
+    for (int64_t q = int64_t(blockIdx.x) * blockDim.x + threadIdx.x; q < npairs; q += int64_t(gridDim.x) * blockDim.x)
+        out[q] = p[pi[q]] * p[pj[q]] * (acc[q] * (s * s));
+}
+
 // Alg. 1 l.27: x = p (.) z, se = p (.) sqrt(var) * rnorm / sqrt(m - n).
 __global__ void k_finish(const double *__restrict__ z, const double *__restrict__ var,
                          const double *__restrict__ p, double *__restrict__ xOut,

@@ -34,6 +34,7 @@ SYMBOLS = [
     "gsr_upload", "gsr_upload_rows", "gsr_upload_finish", "gsr_upload_constraints", "gsr_set_b",
     "gsr_get_star_rowptr", "gsr_precondition", "gsr_get_colscale", "gsr_get_values",
     "gsr_aprod1", "gsr_aprod2", "gsr_lsqr", "gsr_get_trace", "gsr_path_info", "gsr_last_timing",
+    "gsr_set_cov_pairs", "gsr_get_cov",
 ]
 # the measurement hook of include/gsr_bench.h
 BENCH_SYMBOLS = ["gsr_bench_set", "gsr_time_aprod"]
@@ -96,6 +97,8 @@ def load_library():
         "gsr_aprod2": (I32, [P, P, P]),
         "gsr_lsqr": (I32, [P, I64, D, D, D, C.POINTER(_Result)]),
         "gsr_get_trace": (I32, [P, P, I64, C.POINTER(I64)]),
+        "gsr_set_cov_pairs": (I32, [P, I64, P, P]),
+        "gsr_get_cov": (I32, [P, P]),
         "gsr_path_info": (I32, [P]),
         "gsr_last_timing": (I32, [P, C.POINTER(D), C.POINTER(I64)]),
         "gsr_time_aprod": (I32, [P, I32, I32, C.POINTER(D)]),
@@ -273,6 +276,17 @@ class Gsr:
         nw = C.c_int64()
         self._ck(self.lib.gsr_get_trace(self._h, out.ctypes.data, max_itn, C.byref(nw)))
         return out[: nw.value]
+
+    def gsr_set_cov_pairs(self, pi, pj):
+        """Couples (pi[q], pj[q]) of unknowns whose covariance the following gsr_lsqr calls estimate (i64, host or device)."""
+        npairs = 0 if pi is None else int(pi.shape[0])
+        self._n_pairs = npairs
+        self._ck(self.lib.gsr_set_cov_pairs(self._h, npairs, _ptr(pi, torch.int64, "pi"), _ptr(pj, torch.int64, "pj")))
+
+    def gsr_get_cov(self):
+        out = torch.empty(getattr(self, "_n_pairs", 0), dtype=torch.float64, device=self.device)
+        self._ck(self.lib.gsr_get_cov(self._h, out.data_ptr()))
+        return out
 
     def gsr_path_info(self):
         return int(self.lib.gsr_path_info(self._h))

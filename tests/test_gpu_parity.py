@@ -299,6 +299,56 @@ def test_lsqr_unpreconditioned_and_host_output():
         assert r2.kernel_launches > 0 and r2.loop_ms > 0
 
 
+@pytest.mark.parametrize("name", ["mini_con", "powerlaw"])
+def test_covariances_of_couples(name):
+    """gsr_set_cov_pairs / gsr_get_cov (Alg. 1 l.26-27; R26) against the oracle's
+    gsr_oracle_lsqr_cov: couples drawn over all sections plus some (i, i); tolerance SE_TOL relative to se_i se_j (the
+    Cauchy-Schwarz scale of a covariance); fused and two-product iteration; cov(i, i) = se_i^2; couples persist over
+    solves and can be cleared; a couple outside [0, n) is GSR_EINDEX."""
+    gsr = gsr_mod()
+    cfg = CASES[name]["cfg"]
+    S, d = oracle_system(cfg)
+    b = make_b(S, d)
+    rng = np.random.default_rng(12)
+    pi = np.concatenate([rng.integers(0, S.n, 500), np.arange(0, S.n, max(1, S.n // 40))]).astype(np.int64)
+    pj = np.concatenate([rng.integers(0, S.n, 500), np.arange(0, S.n, max(1, S.n // 40))]).astype(np.int64)
+    S.precondition()
+    ro = S.lsqr(b, 20, 0.0, 0.0, pairs=(pi, pj))
+    scale = ro.se[pi] * ro.se[pj]
+    for flags in (0, gsr.GSR_FLAG_NO_FUSE):
+        with make_gpu(S, {**d, "values": S.V}, b, flags=flags) as G:       # the preconditioned matrix: p = 1 on the device
+            with pytest.raises(gsr.GsrError) as e:
+                G.gsr_get_cov()
+            assert e.value.code == gsr.GSR_ESTATE
+            G.gsr_set_cov_pairs(pi, pj)
+            for _ in range(2):                                              # the couples stay set; the sums start at zero
+                r = G.gsr_lsqr(20, 0.0, 0.0)
+                cov = G.gsr_get_cov().cpu().numpy() * S.p[pi] * S.p[pj]
+                assert (r.istop, r.itn) == (ro.istop, ro.itn) == (7, 20)
+                assert np.all(np.abs(cov - ro.cov) <= SE_TOL * scale), float(np.max(np.abs(cov - ro.cov) / scale))
+                se = r.se.cpu().numpy() * S.p
+                np.testing.assert_allclose(cov[500:], se[pi[500:]] ** 2, rtol=1e-12)
+                assert rel(r.x.cpu().numpy() * S.p, ro.x) <= X_TOL
+            bad = pj.copy()
+            bad[7] = S.n
+            with pytest.raises(gsr.GsrError) as e:
+                G.gsr_set_cov_pairs(pi, bad)
+            assert e.value.code == gsr.GSR_EINDEX and "couple 7" in str(e.value)
+            G.gsr_set_cov_pairs(None, None)
+            r = G.gsr_lsqr(20, 0.0, 0.0)
+            assert rel(r.x.cpu().numpy() * S.p, ro.x) <= X_TOL
+            with pytest.raises(gsr.GsrError):
+                G.gsr_get_cov()
+    # with the device's own preconditioner: cov carries p_i p_j
+    S2, _ = oracle_system(cfg)
+    with make_gpu(S2, d, b) as G:
+        G.gsr_precondition()
+        G.gsr_set_cov_pairs(dev(pi), dev(pj))                               # device arrays
+        G.gsr_lsqr(20, 0.0, 0.0)
+        cov = G.gsr_get_cov().cpu().numpy()
+        assert np.all(np.abs(cov - ro.cov) <= SE_TOL * scale)
+
+
 def test_b_zero_gives_istop0():
     cfg = CASES["mini"]["cfg"]
     S, d = oracle_system(cfg)
