@@ -1208,8 +1208,9 @@ int32_t gsr_set_cov_pairs(gsr_handle *h, int64_t npairs, const int64_t *pi, cons
 
 int32_t gsr_get_cov(gsr_handle *h, double *out)
 {
-    if (!h || !out) return GSR_EINVAL;
+    if (!h) return GSR_EINVAL;
     if (!h->covValid) return fail(h, GSR_ESTATE, "no covariances: gsr_set_cov_pairs, then gsr_lsqr");
+    if (!out) return fail(h, GSR_EINVAL, "gsr_get_cov: out is NULL");
     int rc = enter(h);
     if (rc) return rc;
     CK(cudaMemcpyAsync(out, h->covOut, size_t(h->nPairs) * sizeof(double), cudaMemcpyDefault, h->stream));
